@@ -1,0 +1,439 @@
+"""Pins of the CPU oracle against what the mathematics fixes.
+
+PAPER.md prints no formula and no number, so every pin is a closed form, an invariant, a dense /
+brute-force solve on tiny inputs, or a library-routine restatement (numpy / scipy).  None of them
+re-calls the oracle's own routine to produce the expected value.
+"""
+import math
+
+import numpy as np
+import pytest
+import scipy.fft
+import scipy.linalg
+import scipy.special
+
+from paper_1601_04640_b200.inputs import IMAG, REAL, Workload, axis_coords, initial_psi, random_psi, workload
+
+
+def small3d(n=16, mode=IMAG, G=0.0, D=0.0, dx=0.5, dt=0.025, trap=(1.0, 1.0, 0.5), cutoff=0.0):
+    return Workload("t", 3, n, n, n, dx, dx, dx, dt, *trap, G, D, G, D, mode, 1, 11, 1, cutoff=cutoff)
+
+
+def small2d(n=32, mode=REAL, G=0.0, D=0.0, dx=0.25, dt=0.01, trap=(1.0, 1.5, 0.0)):
+    return Workload("t", 2, n, n, 1, dx, dx, 1.0, dt, *trap, G, D, G, D, mode, 1, 12, 1)
+
+
+# ------------------------------------------------------------------ P4: DFT
+def test_fft_matches_bruteforce_dft_tiny(ob):
+    rng = np.random.default_rng(0)
+    a = rng.standard_normal((4, 8, 16)) + 1j * rng.standard_normal((4, 8, 16))
+    # brute force straight from the definition, python-side
+    nz, ny, nx = a.shape
+    Wz = np.exp(-2j * np.pi * np.outer(np.arange(nz), np.arange(nz)) / nz)
+    Wy = np.exp(-2j * np.pi * np.outer(np.arange(ny), np.arange(ny)) / ny)
+    Wx = np.exp(-2j * np.pi * np.outer(np.arange(nx), np.arange(nx)) / nx)
+    ref = np.einsum("ai,bj,ck,ijk->abc", Wz, Wy, Wx, a)
+    for naive in (False, True):
+        out = ob.fft(a, sign=-1, naive=naive)
+        assert np.max(np.abs(out - ref)) / np.max(np.abs(ref)) < 1e-13
+        back = ob.fft(out, sign=+1, naive=naive) / a.size
+        assert np.max(np.abs(back - a)) < 1e-13
+
+
+def test_fft_against_library_and_invariants(ob):
+    rng = np.random.default_rng(1)
+    a = rng.standard_normal((16, 32, 64)) + 1j * rng.standard_normal((16, 32, 64))
+    out = ob.fft(a, -1)
+    ref = scipy.fft.fftn(a)
+    assert np.max(np.abs(out - ref)) / np.max(np.abs(ref)) < 1e-13
+    inv = ob.fft(a, +1)
+    assert np.max(np.abs(inv - scipy.fft.ifftn(a) * a.size)) / np.max(np.abs(inv)) < 1e-13
+    # Parseval
+    assert abs(np.sum(np.abs(out) ** 2) / a.size - np.sum(np.abs(a) ** 2)) < 1e-9 * np.sum(np.abs(a) ** 2)
+    # delta <-> constant
+    d = np.zeros((8, 8, 8), complex)
+    d[0, 0, 0] = 1.0
+    assert np.max(np.abs(ob.fft(d, -1) - 1.0)) < 1e-15
+    # shifted delta -> pure phase with the forward sign convention exp(-2 pi i m j / N)
+    d = np.zeros((1, 1, 16), complex)
+    d[0, 0, 3] = 1.0
+    ph = np.exp(-2j * np.pi * 3 * np.arange(16) / 16)
+    assert np.max(np.abs(ob.fft(d, -1)[0, 0] - ph)) < 4e-15   # ph itself carries the rounding of its angle
+    # real input -> Hermitian spectrum
+    r = rng.standard_normal((8, 8, 16))
+    R = ob.fft(r, -1)
+    Rm = np.conj(R[(-np.arange(8)) % 8][:, (-np.arange(8)) % 8][:, :, (-np.arange(16)) % 16])
+    assert np.max(np.abs(R - Rm)) < 1e-12
+
+
+# ------------------------------------------------------------------ P3: Crank-Nicolson sweep
+@pytest.mark.parametrize("a", [0.025, 0.125j, 0.4, 2.5j])
+@pytest.mark.parametrize("N", [3, 4, 17, 64])
+def test_cn_line_against_dense_solve(ob, a, N):
+    rng = np.random.default_rng(N)
+    psi = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    M = N - 2
+    L = 2 * np.eye(M) - np.eye(M, k=1) - np.eye(M, k=-1)          # -delta^2 on the interior
+    rhs = a * psi[:-2] + (1 - 2 * a) * psi[1:-1] + a * psi[2:]      # uses the actual end values
+    ref = np.zeros(N, complex)
+    ref[1:-1] = np.linalg.solve(np.eye(M) + a * L, rhs)
+    out = ob.cn_line(psi, a)
+    assert out[0] == 0 and out[-1] == 0
+    assert np.max(np.abs(out - ref)) < 1e-14 * max(1.0, np.max(np.abs(ref)))
+
+
+@pytest.mark.parametrize("a", [0.025, 0.125j])
+def test_cn_line_sine_mode_closed_form(ob, a):
+    N = 34
+    M = N - 2
+    j = np.arange(N)
+    for m in (1, 2, 7, M):
+        mode = np.sin(np.pi * j * m / (M + 1))
+        mode[0] = mode[-1] = 0.0
+        lam = 4 * np.sin(np.pi * m / (2 * (M + 1))) ** 2
+        mult = (1 - a * lam) / (1 + a * lam)
+        out = ob.cn_line(mode.astype(complex), a)
+        assert np.max(np.abs(out - mult * mode)) < 5e-15
+        if isinstance(a, complex):
+            assert abs(abs(mult) - 1.0) < 1e-15                     # unitary in real time
+
+
+def test_cn_sweeps_axes_strides_and_commutation(ob):
+    w = Workload("t", 3, 8, 16, 32, 0.3, 0.4, 0.5, 0.02, 1, 1, 1, 0, 0, 0, 0, REAL, 1, 5, 1)
+    p = ob.params_of(w)
+    psi = random_psi(w, 3)
+    # each axis sweep == the line solver applied along that numpy axis (numpy axis 2 is x)
+    for axis, npax, h in ((0, 2, w.dx), (1, 1, w.dy), (2, 0, w.dz)):
+        a = 1j * w.dt / (4 * h * h)
+        N = psi.shape[npax]
+        M = N - 2
+        A = np.eye(M) * (1 + 2 * a) - a * (np.eye(M, k=1) + np.eye(M, k=-1))
+        B = np.eye(M) * (1 - 2 * a) + a * (np.eye(M, k=1) + np.eye(M, k=-1))
+        mv = np.moveaxis(psi, npax, 0)
+        rhs = np.tensordot(B, mv[1:-1], axes=1)
+        rhs[0] += a * mv[0]
+        rhs[-1] += a * mv[-1]
+        sol = np.linalg.solve(A, rhs.reshape(M, -1)).reshape(rhs.shape)
+        ref = np.zeros_like(mv)
+        ref[1:-1] = sol
+        ref = np.moveaxis(ref, 0, npax)
+        out = ob.cn_sweep(p, psi, axis)
+        assert np.max(np.abs(out - ref)) < 1e-14
+    # the three sweeps commute (constant coefficients, separable, Dirichlet)
+    xyz = ob.cn_sweep(p, ob.cn_sweep(p, ob.cn_sweep(p, psi, 0), 1), 2)
+    zyx = ob.cn_sweep(p, ob.cn_sweep(p, ob.cn_sweep(p, psi, 2), 1), 0)
+    assert np.max(np.abs(xyz - zyx)) < 1e-15 * 10
+
+
+def test_cn_real_time_conserves_plain_sum_norm(ob):
+    w = small3d(16, REAL)
+    p = ob.params_of(w)
+    psi = random_psi(w, 9)
+    for ax in range(3):                     # zero faces first so that the map is the Cayley transform
+        psi = ob.cn_sweep(p, psi, ax)
+    n0 = ob.norm(p, psi)
+    out = psi
+    for ax in range(3):
+        out = ob.cn_sweep(p, out, ax)
+    assert abs(ob.norm(p, out) / n0 - 1) < 1e-14
+
+
+# ------------------------------------------------------------------ P6: dipolar kernels
+def test_erfcx_against_scipy(ob):
+    for x in [0.0, 1e-8, 0.3, 1.0, 2.999, 3.0, 3.001, 5.0, 10.0, 26.0, 27.0, 31.4, 100.0, 1e4]:
+        ref = scipy.special.erfcx(x)
+        assert abs(ob.erfcx(x) - ref) <= 2e-15 * ref + 1e-300, x
+
+
+def test_vdd3d_properties(ob):
+    assert ob.vdd3d(0, 0, 0) == 0.0
+    assert ob.vdd3d(0, 0, 1.7) == pytest.approx(2.0, abs=1e-15)      # k along the dipoles
+    assert ob.vdd3d(1.3, 0, 0) == pytest.approx(-1.0, abs=1e-15)     # k perpendicular
+    assert ob.vdd3d(1.0, 1.0, 1.0) == pytest.approx(0.0, abs=1e-15)  # magic angle
+    for s in ((-1, 1, 1), (1, -1, 1), (1, 1, -1)):
+        assert ob.vdd3d(0.3 * s[0], 0.7 * s[1], 1.1 * s[2]) == ob.vdd3d(0.3, 0.7, 1.1)
+    # depends on kx, ky only through kx^2 + ky^2
+    assert ob.vdd3d(0.6, 0.8, 0.5) == pytest.approx(ob.vdd3d(1.0, 0.0, 0.5), abs=1e-15)
+    w = small3d(16)
+    V = ob.vdd_table(ob.params_of(w))
+    assert V.min() >= -1 - 1e-15 and V.max() <= 2 + 1e-15
+    assert V[0, 0, 0] == 0
+    assert abs(V.sum()) < 1e-11                                      # cubic grid: angular average 0
+    # index -> wavenumber map (S6): m and N-m give the same kernel; kz is numpy axis 0
+    assert np.array_equal(V[1:, :, :], V[:0:-1, :, :])
+    assert V[3, 0, 0] == pytest.approx(2.0) and V[0, 3, 0] == pytest.approx(-1.0) and V[0, 0, 3] == pytest.approx(-1.0)
+    assert ob.wavenumber(1, 16, 0.5) == pytest.approx(2 * math.pi / 8)
+    assert ob.wavenumber(15, 16, 0.5) == pytest.approx(-2 * math.pi / 8)
+
+
+def test_vdd3d_cutoff_limits(ob):
+    # kR -> infinity: untruncated kernel; kR -> 0: kernel vanishes like (kR)^2/10
+    assert ob.vdd3d(0.3, 0.2, 0.9, 1e9) == pytest.approx(ob.vdd3d(0.3, 0.2, 0.9, 0.0), rel=1e-12)
+    k = 0.1     # 1 + 3cos(x)/x^2 - 3sin(x)/x^3 = x^2/10 - x^4/280 + O(x^6)
+    assert ob.vdd3d(0, 0, k, 1.0) == pytest.approx(2.0 * (k * k / 10.0 - k ** 4 / 280.0), rel=1e-6)
+
+
+def test_vdd2d_properties(ob):
+    assert ob.vdd2d(0, 0, 1.0) == 2.0
+    xs = np.linspace(0, 60, 400)
+    h = np.array([ob.vdd2d(x, 0.0, 1.0) for x in xs])
+    assert np.all(np.diff(h) < 0)                                    # monotone decreasing
+    assert np.all(np.isfinite(h))
+    assert h[-1] > -1 and h[-1] == pytest.approx(-1.0, abs=2e-3)
+    # isotropic in the plane; scales with d_perp
+    assert ob.vdd2d(3, 4, 0.5) == pytest.approx(ob.vdd2d(5, 0, 0.5), abs=1e-15)
+    assert ob.vdd2d(2.0, 0, 1.0) == pytest.approx(ob.vdd2d(1.0, 0, 2.0), abs=1e-15)
+    # library value
+    xi = 1.3 / math.sqrt(2)
+    assert ob.vdd2d(1.3, 0, 1.0) == pytest.approx(2 - 3 * math.sqrt(math.pi) * xi * scipy.special.erfcx(xi), abs=1e-15)
+    # = Gaussian average over k_z of the 3-D kernel (defining property of the quasi-2-D reduction)
+    kz = np.linspace(-40, 40, 400001)
+    wgt = np.exp(-kz ** 2 / 2.0) / math.sqrt(2 * math.pi)            # |FT of the d_perp=1 Gaussian density|
+    kr = 1.3
+    avg = np.trapezoid((3 * kz ** 2 / (kz ** 2 + kr ** 2) - 1) * wgt, kz)
+    assert ob.vdd2d(kr, 0, 1.0) == pytest.approx(avg, abs=1e-9)
+
+
+# ------------------------------------------------------------------ P7: whole dipolar path
+def _f_dip(x):
+    s = math.sqrt(1 - x * x)
+    return (1 + 2 * x * x) / (1 - x * x) - 3 * x * x * math.atanh(s) / (1 - x * x) ** 1.5
+
+
+def test_phi_dd_gaussian_dipolar_energy_closed_form(ob):
+    # Gaussian with nu = lambda = 1, kappa = 1/2: dV sum Phi n = -f(kappa_g) prod sqrt(w_d / 2 pi),
+    # kappa_g = l_perp / l_z = sqrt(kappa / nu)   (textbook dipolar energy of a Gaussian cloud)
+    for n, R, tol in ((32, 6.0, 3e-5), (64, 12.0, 2e-7)):
+        w = small3d(n, cutoff=R)
+        p = ob.params_of(w)
+        psi = initial_psi(w, noise=0.0).real
+        dens = psi ** 2
+        phi = ob.phi_dd(p, dens)
+        e = w.cell_volume * np.sum(phi * dens)
+        ref = -_f_dip(math.sqrt(0.5)) * math.sqrt(1 / (2 * math.pi)) ** 2 * math.sqrt(0.5 / (2 * math.pi))
+        assert e == pytest.approx(ref, rel=tol)
+        assert e < 0        # cloud elongated along the dipoles: net attraction
+
+
+def test_phi_dd_bruteforce_equals_fft_and_is_real_linear(ob):
+    w = small3d(8)
+    p = ob.params_of(w)
+    rng = np.random.default_rng(5)
+    n1 = rng.random(w.shape)
+    n2 = rng.random(w.shape)
+    a = ob.phi_dd(p, n1, naive=False)
+    b = ob.phi_dd(p, n1, naive=True)
+    assert np.max(np.abs(a - b)) < 1e-13
+    # library restatement
+    V = ob.vdd_table(p)
+    ref = np.real(scipy.fft.ifftn(V * scipy.fft.fftn(n1)))
+    assert np.max(np.abs(a - ref)) < 1e-13
+    # linear; a constant density gives Phi = V(0) * const = 0 in 3-D
+    assert np.max(np.abs(ob.phi_dd(p, 2 * n1 + 3 * n2) - 2 * a - 3 * ob.phi_dd(p, n2))) < 1e-12
+    assert np.max(np.abs(ob.phi_dd(p, np.full(w.shape, 0.7)))) < 1e-14
+    # single plane wave cos(k.r): eigenfunction with eigenvalue V_dd(k)
+    iz, iy, ix = np.meshgrid(np.arange(8), np.arange(8), np.arange(8), indexing="ij")
+    m = (1, 2, 3)   # (mx, my, mz)
+    wave = np.cos(2 * np.pi * (m[0] * ix + m[1] * iy + m[2] * iz) / 8)
+    k = [2 * np.pi * mm / (8 * 0.5) for mm in m]
+    lam = 3 * k[2] ** 2 / (k[0] ** 2 + k[1] ** 2 + k[2] ** 2) - 1
+    assert np.max(np.abs(ob.phi_dd(p, wave) - lam * wave)) < 1e-13
+
+
+def test_phi_dd_2d_constant_density(ob):
+    w = small2d(16)
+    p = ob.params_of(w)
+    out = ob.phi_dd(p, np.full(w.shape, 0.25))
+    assert np.max(np.abs(out - 2.0 * 0.25)) < 1e-14                  # h(0) = 2
+
+
+# ------------------------------------------------------------------ P1: nonlinear step
+def test_nonlinear_special_cases(ob):
+    w = small3d(8, IMAG, G=3.0, D=2.0)
+    psi = random_psi(w, 1)
+    rng = np.random.default_rng(2)
+    phi = rng.standard_normal(w.shape)
+    out = ob.nonlinear(ob.params_of(w), psi, phi)
+    # phase untouched in imaginary time; decay exponent at hand-computed points
+    assert np.max(np.abs(np.angle(out * np.conj(psi)))) < 1e-15
+    c = (4, 4, 4)                                                    # centre: V = 0
+    u = w.dt * (w.G * abs(psi[c]) ** 2 + w.D * phi[c])
+    assert abs(out[c]) == pytest.approx(abs(psi[c]) * math.exp(-u), rel=1e-15)
+    q = (1, 6, 7)                                                    # (iz, iy, ix): z=-1.5, y=1, x=1.5
+    V = 0.5 * (1.0 * 1.5 ** 2 + 1.0 * 1.0 ** 2 + 0.25 * 1.5 ** 2)
+    u = w.dt * (V + w.G * abs(psi[q]) ** 2 + w.D * phi[q])
+    assert abs(out[q]) == pytest.approx(abs(psi[q]) * math.exp(-u), rel=1e-15)
+    # real time: modulus untouched, phase = -dt U; two steps of dt == one step of 2 dt
+    wr = small3d(8, REAL, G=3.0, D=2.0)
+    outr = ob.nonlinear(ob.params_of(wr), psi, phi)
+    assert np.max(np.abs(np.abs(outr) - np.abs(psi)) / np.abs(psi)) < 1e-15
+    assert np.angle(outr[q] / psi[q]) == pytest.approx(-u, abs=1e-15)
+    twice = ob.nonlinear(ob.params_of(wr), outr, phi)
+    from dataclasses import replace
+    once2 = ob.nonlinear(ob.params_of(replace(wr, dt=2 * wr.dt)), psi, phi)
+    assert np.max(np.abs(twice - once2)) < 1e-15
+
+
+# ------------------------------------------------------------------ P5: observables on a sampled Gaussian
+def test_observables_sampled_gaussian_closed_forms(ob):
+    w = Workload("t", 3, 32, 32, 32, 0.5, 0.5, 0.5, 0.025, 1.0, 1.0, 0.5, 45.0, 0.0, 45.0, 0.0, IMAG, 1, 1, 1)
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(initial_psi(w, noise=0.0))
+    r = o.observables()
+    om = (1.0, 1.0, 0.5)
+    d = (0.5, 0.5, 0.5)
+    ekin = sum((1 - math.exp(-om[i] * d[i] ** 2 / 4)) / d[i] ** 2 for i in range(3))
+    etr = sum(om) / 4
+    ec = 45.0 * math.prod(math.sqrt(x / (2 * math.pi)) for x in om)
+    assert r["norm"] == pytest.approx(1.0, abs=1e-14)
+    assert r["mu"] == pytest.approx(ekin + etr + ec, rel=2e-8)          # E_c aliasing ~1e-8 at dx = 0.5
+    assert r["energy"] == pytest.approx(ekin + etr + ec / 2, rel=2e-8)
+    assert r["rms_x"] == pytest.approx(1 / math.sqrt(2.0), rel=1e-12)
+    assert r["rms_z"] == pytest.approx(1.0, rel=1e-11)          # tail cut at |z| = 8: ~4e-12
+    assert r["rms_r"] == pytest.approx(math.sqrt(0.5 + 0.5 + 1.0), rel=1e-11)
+    assert r["density0"] == pytest.approx(math.prod(math.sqrt(x / math.pi) for x in om), rel=1e-14)
+    assert r["density_max"] == r["density0"]
+    # G = 0: kinetic and trap closed forms to round-off
+    o.set_coupling(0.0, 0.0)
+    r0 = o.observables()
+    assert r0["mu"] == pytest.approx(ekin + etr, rel=1e-11)       # z tail cut: ~2e-12
+    assert r0["energy"] == pytest.approx(r0["mu"], rel=1e-15)
+
+
+def test_observables_dipolar_term_and_mu_energy_split(ob):
+    w = small3d(32, IMAG, G=10.0, D=7.0, cutoff=6.0)
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(initial_psi(w, noise=0.0))
+    full = o.observables()
+    o.set_coupling(10.0, 0.0)
+    nod = o.observables()
+    ed = -_f_dip(math.sqrt(0.5)) * (1 / (2 * math.pi)) * math.sqrt(0.5 / (2 * math.pi)) * 7.0
+    assert full["mu"] - nod["mu"] == pytest.approx(ed, rel=1e-4)
+    assert full["energy"] - nod["energy"] == pytest.approx(ed / 2, rel=1e-4)
+
+
+# ------------------------------------------------------------------ P2: whole imaginary-time loop
+def _lowest_discrete_eig(n, d, omega):
+    x = axis_coords(n, d)[1:-1]
+    M = n - 2
+    H = (np.eye(M) * 2 - np.eye(M, k=1) - np.eye(M, k=-1)) / (2 * d * d) + np.diag(0.5 * omega ** 2 * x ** 2)
+    return np.linalg.eigvalsh(H)[0]
+
+
+def test_imag_time_noninteracting_ground_state_energy(ob):
+    exact = 2 * _lowest_discrete_eig(32, 0.5, 1.0) + _lowest_discrete_eig(32, 0.5, 0.5)
+    assert exact == pytest.approx(1.25 - (1 + 1 + 0.25) * 0.25 / 32, abs=4e-4)   # continuum + O(dx^2)
+    errs = []
+    for dt, steps in ((0.025, 600), (0.0125, 1200)):
+        w = Workload("t", 3, 32, 32, 32, 0.5, 0.5, 0.5, dt, 1.0, 1.0, 0.5, 0, 0, 0, 0, IMAG, steps, 1, 1)
+        o = ob.Oracle(ob.params_of(w))
+        o.set_psi(initial_psi(w))
+        o.step(steps)
+        r = o.observables()
+        assert r["norm"] == pytest.approx(1.0, abs=1e-14)
+        assert r["mu"] == pytest.approx(r["energy"], abs=1e-13)
+        errs.append(r["mu"] - exact)
+    assert 0 < errs[0] < 1.5e-4                      # O(dt^2) splitting bias, variational from above
+    assert 3.5 < errs[0] / errs[1] < 4.5             # quarters when dt halves
+
+
+# ------------------------------------------------------------------ P8: real time
+def test_real_time_norm_and_energy_conservation_and_phase_sign(ob):
+    w = Workload("t", 2, 64, 64, 1, 0.25, 0.25, 1.0, 0.005, 1.0, 1.5, 0.0, 20.0, 15.0, 20.0, 15.0, REAL, 1, 2, 1)
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(initial_psi(w))
+    r0 = o.observables()
+    o.step(100)
+    r1 = o.observables()
+    assert abs(r1["norm"] - 1) < 1e-14
+    assert abs(r1["energy"] - r0["energy"]) < 2e-3 * abs(r0["energy"])
+    assert abs(r1["rms_x"] - r0["rms_x"]) > 1e-3          # it does evolve
+    # phase sign: a stationary state of the discrete problem turns as exp(-i mu t)
+    wi = Workload("t", 2, 32, 32, 1, 0.4, 0.4, 1.0, 0.002, 1.0, 1.0, 0.0, 0, 0, 0, 0, IMAG, 1, 3, 1)
+    oi = ob.Oracle(ob.params_of(wi))
+    oi.set_psi(initial_psi(wi, noise=0.0))
+    oi.step(3000)
+    gs = oi.get_psi()
+    mu = oi.observables()["mu"]
+    from dataclasses import replace
+    orr = ob.Oracle(ob.params_of(replace(wi, time_mode=REAL)))
+    orr.set_psi(gs)
+    orr.step(10)
+    ph = np.vdot(gs, orr.get_psi())
+    assert abs(abs(ph) * wi.cell_volume - 1) < 1e-6
+    assert np.angle(ph) == pytest.approx(-mu * 10 * wi.dt, abs=1e-6)
+
+
+# ------------------------------------------------------------------ P9: library restatement of one step
+def _numpy_step(w, psi, G, D, V_dd):
+    """numpy/scipy restatement: rfftn/irfftn, solve_banded, numpy sums."""
+    n = np.abs(psi) ** 2
+    axes = tuple(range(psi.ndim))
+    half = V_dd[..., : w.nx // 2 + 1]
+    phi = scipy.fft.irfftn(scipy.fft.rfftn(n, axes=axes) * half, s=psi.shape, axes=axes)
+    x = axis_coords(w.nx, w.dx)
+    y = axis_coords(w.ny, w.dy)
+    if w.ndim == 3:
+        z = axis_coords(w.nz, w.dz)
+        V = 0.5 * (w.nu ** 2 * x[None, None, :] ** 2 + w.lam ** 2 * y[None, :, None] ** 2 + w.kappa ** 2 * z[:, None, None] ** 2)
+    else:
+        V = 0.5 * (w.nu ** 2 * x[None, :] ** 2 + w.lam ** 2 * y[:, None] ** 2)
+    c = 1.0 if w.time_mode == IMAG else 1j
+    psi = psi * np.exp(-c * w.dt * (V + G * n + D * phi))
+    hs = (w.dx, w.dy, w.dz)
+    for ax in range(w.ndim):
+        npax = psi.ndim - 1 - ax
+        a = c * w.dt / (4 * hs[ax] ** 2)
+        mv = np.moveaxis(psi, npax, 0)
+        N = mv.shape[0]
+        rhs = a * mv[:-2] + (1 - 2 * a) * mv[1:-1] + a * mv[2:]
+        ab = np.zeros((3, N - 2), dtype=complex)
+        ab[0, 1:] = -a
+        ab[1, :] = 1 + 2 * a
+        ab[2, :-1] = -a
+        sol = scipy.linalg.solve_banded((1, 1), ab, rhs.reshape(N - 2, -1)).reshape(rhs.shape)
+        new = np.zeros_like(mv)
+        new[1:-1] = sol
+        psi = np.moveaxis(new, 0, npax)
+    if w.time_mode == IMAG:
+        psi = psi / np.sqrt(np.sum(np.abs(psi) ** 2) * w.cell_volume)
+    return np.ascontiguousarray(psi)
+
+
+@pytest.mark.parametrize("key,mode,steps", [("C1", IMAG, 3), ("C1", REAL, 3), ("2d", REAL, 3), ("2d", IMAG, 2), ("aniso", REAL, 2)])
+def test_full_step_against_numpy_scipy_restatement(ob, key, mode, steps):
+    from dataclasses import replace
+    if key == "C1":
+        w = replace(workload("C1"), time_mode=mode)
+    elif key == "2d":
+        w = Workload("t", 2, 64, 32, 1, 0.2, 0.3, 1.0, 0.004, 1.0, 1.5, 0.0, 20.0, 15.0, 25.0, 15.0, mode, 1, 2, 1)
+    else:
+        w = Workload("t", 3, 16, 32, 8, 0.4, 0.3, 0.8, 0.01, 1.0, 1.2, 0.8, 50.0, 40.0, 50.0, 45.0, mode, 1, 4, 1)
+    p = ob.params_of(w)
+    o = ob.Oracle(p)
+    psi = random_psi(w, 21) if mode == REAL else initial_psi(w)
+    o.set_psi(psi)
+    o.set_coupling(w.G_run, w.D_run)
+    V_dd = ob.vdd_table(p)
+    ref = psi
+    for _ in range(steps):
+        ref = _numpy_step(w, ref, w.G_run, w.D_run, V_dd)
+    o.step(steps)
+    out = o.get_psi()
+    assert np.max(np.abs(out - ref)) / np.max(np.abs(ref)) < 1e-13
+
+
+def test_step_order_is_nonlinear_then_x_y_z_then_norm(ob):
+    w = small3d(16, IMAG, G=20.0, D=10.0)
+    p = ob.params_of(w)
+    psi = initial_psi(w)
+    o = ob.Oracle(p)
+    o.set_psi(psi)
+    o.step(1)
+    phi = ob.phi_dd(p, np.abs(psi) ** 2)
+    ref = ob.nonlinear(p, psi, phi)
+    for ax in range(3):
+        ref = ob.cn_sweep(p, ref, ax)
+    ref = ob.normalize(p, ref)
+    assert np.array_equal(o.get_psi(), ref)
+    assert ob.norm(p, ref) == pytest.approx(1.0, abs=1e-15)
