@@ -1,0 +1,124 @@
+/* dbec.h — C ABI of the B200-native dipolar SSCN step (arxiv 1601.04640, "DBEC-GP-CUDA").
+ *
+ * One split-step semi-implicit Crank-Nicolson (SSCN) time step of the 2-D/3-D dipolar
+ * Gross-Pitaevskii equation, in imaginary or real time ("Nature of problem",
+ * "Solution method"), behind plain pointers and sizes.  Every step of the path runs in hand-written
+ * sm_100a kernels inside libdbec.so; there is no CPU fallback and no library FFT.
+ *
+ * Problem (readings S1, S2, S3 of DESIGN.md; PAPER.md prints no formula):
+ *     i dpsi/dt = [ -1/2 Lap + V + G |psi|^2 + D Phi_dd ] psi,   int |psi|^2 = 1,
+ *     V = 1/2 (nu^2 x^2 + lambda^2 y^2 + kappa^2 z^2),
+ *     Phi_dd = F^-1[ V_dd(k) F[|psi|^2] ],  V_dd(k) = 3 k_z^2/|k|^2 - 1  (3-D; 0 at k = 0).
+ * One step (PAPER.md:67 function list; order = reading S10):
+ *     calcpsidd2 (density -> FFT -> x V_dd -> inverse FFT), calcnu (psi *= exp(-c dt (V+G n+D Phi))),
+ *     calclux, calcluy, calcluz (Crank-Nicolson tridiagonal solve on every grid line),
+ *     calcnorm (imaginary time only).  c = 1 in imaginary time, i in real time.
+ *
+ * Layout of every field: x fastest, idx = ix + NX*(iy + NY*iz); psi is complex128 stored as
+ * (re, im) pairs of IEEE doubles.  Grid coordinates x_i = (i - NX/2)*dx (reading S17).
+ *
+ * Ownership: the caller owns all device memory, including the workspace handed to dbec_create
+ * (size from dbec_workspace_bytes, 256-byte aligned); the library owns only the small host-side
+ * handle.  dbec_set_psi / dbec_get_psi copy, they never adopt the caller's buffer.
+ *
+ * Errors: every call returns 0 (DBEC_OK) or a negative code; nothing throws or aborts; NULL
+ * arguments give DBEC_EINVAL.  All work is enqueued on the CUDA stream given to dbec_create.
+ */
+#ifndef DBEC_H
+#define DBEC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DBEC_OK           0
+#define DBEC_EINVAL      -1   /* NULL pointer, bad ndim / time_mode / spacing, nsteps < 0 ...        */
+#define DBEC_ESIZE       -2   /* grid length not a supported FFT length (never silently adjusted,
+                                 contrast PAPER.md:93); supported: powers of two 16..512, NY even   */
+#define DBEC_EWORKSPACE  -3   /* workspace NULL, misaligned or smaller than dbec_workspace_bytes    */
+#define DBEC_ECUDA       -4   /* a CUDA call failed; dbec_last_cuda_error gives the CUDA code       */
+#define DBEC_ENODEVICE   -5   /* no CUDA device / not an sm_100 device                              */
+
+typedef struct dbec_handle_s* dbec_handle;
+
+typedef struct {
+    int32_t ndim;              /* 2 or 3                                                            */
+    int32_t plane;             /* 2-D only: 0 = XY (dipoles perpendicular to the plane)             */
+    int32_t nx, ny, nz;        /* nz = 1 in 2-D                                                     */
+    double  dx, dy, dz;        /* grid spacings (dz ignored in 2-D)                                 */
+    double  dt;                /* time step                                                         */
+    double  nu, lambda, kappa; /* trap anisotropies along x, y, z (reading S2)                      */
+    double  G, D;              /* coefficients of |psi|^2 and of Phi_dd (reading S3)                */
+    double  d_perp;            /* 2-D only: Gaussian width of the frozen direction (reading S21)    */
+    double  cutoff;            /* 3-D only: spherical truncation radius of V_dd, 0 = none (S5)      */
+    int32_t time_mode;         /* 0 = imaginary time, 1 = real time                                 */
+} dbec_params;
+
+/* calcmuen / calcrms; definitions in DESIGN.md "Observables" (readings S13-S16). */
+typedef struct {
+    double norm, mu, energy, rms_x, rms_y, rms_z, rms_r, density0, density_max;
+} dbec_obs;
+
+/* Bytes of device workspace dbec_create needs for these parameters (host call, no CUDA work). */
+int dbec_workspace_bytes(const dbec_params* p, size_t* bytes);
+
+/* Build a handle.  dev_workspace: DEVICE pointer, >= *bytes, 256-byte aligned, owned by the caller
+ * and kept alive until dbec_destroy.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * Builds on the device the tables the paper's CPU initialises (`pot`, `potdd`)
+ * and the Crank-Nicolson coefficients of each axis.  psi starts as all zeros. */
+int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* cuda_stream,
+                dbec_handle* out);
+
+/* Copy NX*NY*NZ complex128 values into the handle's psi.  psi_c128: HOST pointer if on_device == 0
+ * (synchronous copy), DEVICE pointer otherwise (asynchronous on the handle's stream). */
+int dbec_set_psi(dbec_handle h, const void* psi_c128, int on_device);
+
+/* Copy psi out (same pointer rules), with the deferred imaginary-time norm factor applied. */
+int dbec_get_psi(dbec_handle h, void* psi_c128, int on_device);
+
+/* Change G and D (quench / ramp, reading S18).  Takes effect from the next step. */
+int dbec_set_coupling(dbec_handle h, double G, double D);
+
+/* nsteps SSCN steps, asynchronous on the handle's stream, no host sync. */
+int dbec_step(dbec_handle h, int nsteps);
+
+/* calcmuen + calcrms on the current psi.  host_out: HOST pointer.  Synchronises
+ * the stream. */
+int dbec_observables(dbec_handle h, dbec_obs* host_out);
+
+int dbec_destroy(dbec_handle h);
+
+const char* dbec_strerror(int code);
+int dbec_last_cuda_error(dbec_handle h);     /* CUDA error code of the last DBEC_ECUDA, else 0 */
+
+/* ---- single parts of the step, exported so that each can be checked on its own ---- */
+
+/* calcpsidd2 alone: Phi_dd of the current psi into phi_f64, NX*NY*NZ doubles,
+ * DEVICE pointer, asynchronous. */
+int dbec_phi_dd(dbec_handle h, void* phi_f64_dev);
+
+/* calclux / calcluy / calcluz alone: one Crank-Nicolson sweep along axis 0, 1 or 2
+ * applied to psi in place, asynchronous. */
+int dbec_cn_sweep(dbec_handle h, int axis);
+
+/* calcnu alone: psi *= exp(-c dt (V + G|psi|^2 + D Phi_dd)) with Phi_dd of the
+ * current psi, no Crank-Nicolson sweep, asynchronous. */
+int dbec_nonlinear(dbec_handle h);
+
+/* calcnorm alone: psi <- psi / sqrt(dV sum |psi|^2); the factor is kept deferred
+ * (applied by every consumer), asynchronous. */
+int dbec_normalize(dbec_handle h);
+
+/* Number of kernel launches the library has enqueued on this handle since creation. */
+int dbec_launch_count(dbec_handle h, long long* launches);
+
+/* Name and launch count of the i-th distinct kernel (for bench.py's gpu_launches claim). */
+int dbec_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DBEC_H */
