@@ -80,16 +80,19 @@ template <int R, int S> DBEC_HD void dft_small(cd* w) {
 
 // ---- plan ----
 
-template <int R2_, int R3_> struct FftPlan {
+// PAD: pad the exchange rows so that a line stored contiguously (element stride 1) is read without
+// bank conflicts; not needed when lines are interleaved column-wise (element stride = tile width).
+template <int R2_, int R3_, bool PAD_ = true> struct FftPlan {
     static constexpr int R2 = R2_, R3 = R3_;
     static constexpr int T = R2_ * R3_;          // threads per line
     static constexpr int N = 16 * T;             // line length
-    static constexpr int P1 = T + R3_;           // row pitch of the stage-1 exchange (bank spread)
-    static constexpr int P3 = R3_ + 1;           // row pitch of the stage-2 exchange
+    static constexpr int P1 = T + (PAD_ ? R3_ : 0);   // row pitch of the stage-1 exchange
+    static constexpr int P3 = R3_ + (PAD_ ? 1 : 0);   // row pitch of the stage-2 exchange
     static constexpr int I2 = 16 / R2_;          // radix-R2 butterflies per thread in stage 2
     static constexpr int I3 = 16 / R3_;          // radix-R3 butterflies per thread in stage 3
     // shared-memory elements one line needs
-    static constexpr int SMEM = (T == 1) ? 1 : ((16 * P1 > 16 * R2_ * P3 && true) ? 16 * P1 : 16 * R2_ * P3);
+    static constexpr int SMEM_A = 16 * P1, SMEM_B = (R3_ > 1) ? 16 * R2_ * P3 : 0;
+    static constexpr int SMEM = (T == 1) ? 1 : (SMEM_A > SMEM_B ? SMEM_A : SMEM_B);
 };
 
 // stage 1: 16-point DFT over n1 and twiddle by W_N^{m k1}; twA[k1*T + m] = exp(-2 pi i m k1 / N).
