@@ -1,1 +1,1 @@
-"""B200-native dipolar SSCN step (arxiv 1601.04640): Python binding over the C-ABI library."""
+"""B200-native dipolar SSCN step (arxiv 1601.04640): libdbec.so + its ctypes binding."""

@@ -1,0 +1,362 @@
+// dbec_api.cu — the C ABI of include/dbec.h: parameter checks, workspace layout, table set-up, the
+// order of the kernels inside one SSCN step (reading S10: calcpsidd2, calcnu, calclux, calcluy,
+// calcluz, calcnorm — PAPER.md:67) and its CUDA graph.  No arithmetic of the method lives here.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+#include "dbec_internal.hpp"
+#include "cn_chunk.cuh"
+#include "host_tables.hpp"
+
+#define DBEC_VERSION 100
+#define NPARTIAL 32768
+
+static bool fft_len_ok(int n) { return n == 16 || n == 32 || n == 64 || n == 128 || n == 256 || n == 512; }
+
+static int check_params(const dbec_params* p) {
+    if (!p) return DBEC_EINVAL;
+    if (p->ndim != 2 && p->ndim != 3) return DBEC_EINVAL;
+    if (p->ndim == 2 && p->plane != 0) return DBEC_EINVAL;
+    if (p->time_mode != 0 && p->time_mode != 1) return DBEC_EINVAL;
+    if (!(p->dx > 0.0) || !(p->dy > 0.0) || !(p->dt > 0.0)) return DBEC_EINVAL;
+    if (p->ndim == 3 && !(p->dz > 0.0)) return DBEC_EINVAL;
+    if (p->ndim == 2 && !(p->d_perp > 0.0)) return DBEC_EINVAL;
+    if (p->cutoff < 0.0) return DBEC_EINVAL;
+    if (p->nx < 1 || p->ny < 1 || p->nz < 1) return DBEC_EINVAL;
+    if (p->ndim == 2 && p->nz != 1) return DBEC_EINVAL;
+    if (!fft_len_ok(p->nx) || !fft_len_ok(p->ny)) return DBEC_ESIZE;
+    if (p->ndim == 3 && !fft_len_ok(p->nz)) return DBEC_ESIZE;
+    return DBEC_OK;
+}
+
+// ---- workspace layout: one pass computes the offsets, used by both sizing and create ----
+struct Layout {
+    size_t psi, spec, vdd, phi, scal, partial, ticket, obs, tables, total;
+    size_t tab_bytes;
+};
+static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static size_t axis_table_bytes(int n) {
+    // twA, twN (cd n each); vtrap, x2 (double n each); h, pf, pb (cd n each) + pfe, pbs (cd 32 each);
+    // the same five as doubles
+    size_t b = 0;
+    b += up256(sizeof(cd) * n) * 2;
+    b += up256(sizeof(double) * n) * 2;
+    b += up256(sizeof(cd) * n) * 3 + up256(sizeof(cd) * 32) * 2;
+    b += up256(sizeof(double) * n) * 3 + up256(sizeof(double) * 32) * 2;
+    return b;
+}
+
+static void make_layout(const dbec_params* p, Layout* L) {
+    const size_t nx = p->nx, ny = p->ny, nz = p->nz;
+    const size_t nxhp = ((nx / 2 + 1) + DBEC_SPEC_COLS - 1) / DBEC_SPEC_COLS * DBEC_SPEC_COLS;
+    const size_t P = nx * ny * nz, SP = nz * ny * nxhp;
+    size_t o = 0;
+    L->psi = o;     o += up256(P * sizeof(cd));
+    L->spec = o;    o += up256(SP * sizeof(cd));
+    L->vdd = o;     o += up256(SP * sizeof(double));
+    L->phi = o;     o += up256(P * sizeof(double));
+    L->scal = o;    o += up256(SC_COUNT * sizeof(double));
+    L->partial = o; o += up256(NPARTIAL * sizeof(double));
+    L->ticket = o;  o += 256;
+    L->obs = o;     o += 256;
+    L->tables = o;
+    L->tab_bytes = axis_table_bytes(p->nx) + axis_table_bytes(p->ny) + axis_table_bytes(p->nz);
+    o += L->tab_bytes;
+    L->total = o;
+}
+
+static int cuda_fail(dbec_handle h, cudaError_t e) {
+    if (h) h->last_cuda = (int)e;
+    return DBEC_ECUDA;
+}
+#define CU(h, x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return cuda_fail(h, e_); } while (0)
+#define LAUNCH(h, x) do { int rc_ = (x); if (rc_) return cuda_fail(h, (cudaError_t)rc_); } while (0)
+
+// Upload one axis' tables; returns bytes consumed.
+static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, char* dev, size_t* used) {
+    using namespace dbec_host;
+    AxisTables& A = h->ax[axis];
+    A.n = n;
+    std::vector<zc> twN, twA, hh, pf, pb;
+    std::vector<double> vtrap(n), x2(n);
+    if (n >= 16) { make_twN(n, twN); make_twA(n, twN, twA); }
+    else { twN.assign(n, zc(1.0, 0.0)); twA = twN; }
+    for (int i = 0; i < n; ++i) {
+        const double x = (double)(i - n / 2) * d;           // reading S17
+        x2[i] = (n > 1) ? x * x : 0.0;
+        vtrap[i] = (n > 1) ? 0.5 * omega * omega * x * x : 0.0;
+    }
+    const double ar = h->p.dt / (4.0 * d * d);              // a = c dt / (4 h^2), c = 1 or i
+    const zc a = h->p.time_mode == 0 ? zc(ar, 0.0) : zc(0.0, ar);
+    if (n >= 16) make_cn(n, CN_L, a, hh, pf, pb);
+    else { hh.assign(n, zc(0, 0)); pf = hh; pb = hh; }
+    std::vector<zc> pfe(32, zc(0, 0)), pbs(32, zc(0, 0));
+    for (int c = 0; c < n / CN_L; ++c) { pfe[c] = pf[c * CN_L + CN_L - 1]; pbs[c] = pb[c * CN_L]; }
+    const zc kap = (1.0 - 2.0 * a) / a;
+    A.kap = cmake(kap.real(), kap.imag());
+
+    size_t o = 0;
+    auto put = [&](const void* src, size_t bytes, const void** slot) -> cudaError_t {
+        *slot = dev + o;
+        cudaError_t e = cudaMemcpyAsync(dev + o, src, bytes, cudaMemcpyHostToDevice, h->stream);
+        o += up256(bytes);
+        return e;
+    };
+    auto re = [](const std::vector<zc>& v) { std::vector<double> r(v.size()); for (size_t i = 0; i < v.size(); ++i) r[i] = v[i].real(); return r; };
+    std::vector<double> h_re = re(hh), pf_re = re(pf), pb_re = re(pb), pfe_re = re(pfe), pbs_re = re(pbs);
+    CU(h, put(twA.data(), sizeof(zc) * n, (const void**)&A.twA));
+    CU(h, put(twN.data(), sizeof(zc) * n, (const void**)&A.twN));
+    CU(h, put(vtrap.data(), sizeof(double) * n, (const void**)&A.vtrap));
+    CU(h, put(x2.data(), sizeof(double) * n, (const void**)&A.x2));
+    CU(h, put(hh.data(), sizeof(zc) * n, (const void**)&A.h));
+    CU(h, put(pf.data(), sizeof(zc) * n, (const void**)&A.pf));
+    CU(h, put(pb.data(), sizeof(zc) * n, (const void**)&A.pb));
+    CU(h, put(pfe.data(), sizeof(zc) * 32, (const void**)&A.pfe));
+    CU(h, put(pbs.data(), sizeof(zc) * 32, (const void**)&A.pbs));
+    CU(h, put(h_re.data(), sizeof(double) * n, (const void**)&A.h_re));
+    CU(h, put(pf_re.data(), sizeof(double) * n, (const void**)&A.pf_re));
+    CU(h, put(pb_re.data(), sizeof(double) * n, (const void**)&A.pb_re));
+    CU(h, put(pfe_re.data(), sizeof(double) * 32, (const void**)&A.pfe_re));
+    CU(h, put(pbs_re.data(), sizeof(double) * 32, (const void**)&A.pbs_re));
+    // the host vectors must outlive the asynchronous copies from pageable memory: those copies are
+    // staged synchronously by the runtime, but be explicit
+    CU(h, cudaStreamSynchronize(h->stream));
+    *used = o;
+    return DBEC_OK;
+}
+
+static int write_scalars(dbec_handle h, bool reset_scale) {
+    double v[SC_COUNT] = {0};
+    if (!reset_scale) {
+        CU(h, cudaMemcpyAsync(v, h->scal, sizeof(v), cudaMemcpyDeviceToHost, h->stream));
+        CU(h, cudaStreamSynchronize(h->stream));
+    } else {
+        v[SC_S] = 1.0; v[SC_S2] = 1.0;
+    }
+    v[SC_G] = h->p.G; v[SC_D] = h->p.D;
+    CU(h, cudaMemcpyAsync(h->scal, v, sizeof(v), cudaMemcpyHostToDevice, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
+// One SSCN step as a sequence of launches (reading S10).
+static int enqueue_step(dbec_handle h) {
+    const bool imag = h->p.time_mode == 0;
+    const int last_axis = h->p.ndim == 3 ? 2 : 1;
+    LAUNCH(h, dbec_launch_density_fft(h));
+    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    LAUNCH(h, dbec_launch_nonlinear(h, h->fuse_cnx));
+    if (!h->fuse_cnx) LAUNCH(h, dbec_launch_cn(h, 0, 0));
+    for (int ax = 1; ax <= last_axis; ++ax) LAUNCH(h, dbec_launch_cn(h, ax, imag && ax == last_axis));
+    return DBEC_OK;
+}
+
+extern "C" {
+
+int dbec_version(void) { return DBEC_VERSION; }
+
+const char* dbec_strerror(int code) {
+    switch (code) {
+        case DBEC_OK: return "ok";
+        case DBEC_EINVAL: return "invalid argument";
+        case DBEC_ESIZE: return "unsupported grid length (powers of two 16..512 only)";
+        case DBEC_EWORKSPACE: return "workspace missing, misaligned or too small";
+        case DBEC_ECUDA: return "CUDA error (see dbec_last_cuda_error)";
+        case DBEC_ENODEVICE: return "no sm_100 CUDA device";
+        default: return "unknown error";
+    }
+}
+
+int dbec_workspace_bytes(const dbec_params* p, size_t* bytes) {
+    if (!bytes) return DBEC_EINVAL;
+    int rc = check_params(p);
+    if (rc) return rc;
+    Layout L;
+    make_layout(p, &L);
+    *bytes = L.total;
+    return DBEC_OK;
+}
+
+int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* cuda_stream, dbec_handle* out) {
+    if (!out) return DBEC_EINVAL;
+    *out = nullptr;
+    int rc = check_params(p);
+    if (rc) return rc;
+    Layout L;
+    make_layout(p, &L);
+    if (!dev_workspace || ((uintptr_t)dev_workspace & 255) || bytes < L.total) return DBEC_EWORKSPACE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return DBEC_ENODEVICE;
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return DBEC_ENODEVICE;
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (major != 10) return DBEC_ENODEVICE;          // sm_100a code only, no fallback
+
+    dbec_handle h = new (std::nothrow) dbec_handle_s;
+    if (!h) return DBEC_EINVAL;
+    memset(h, 0, sizeof(*h));
+    h->p = *p;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->nx = p->nx; h->ny = p->ny; h->nz = p->nz;
+    h->nxhp = ((p->nx / 2 + 1) + DBEC_SPEC_COLS - 1) / DBEC_SPEC_COLS * DBEC_SPEC_COLS;
+    h->P = (long long)p->nx * p->ny * p->nz;
+    h->SP = (long long)p->nz * p->ny * h->nxhp;
+    h->dV = p->ndim == 3 ? p->dx * p->dy * p->dz : p->dx * p->dy;
+    char* w = (char*)dev_workspace;
+    h->psi = (cd*)(w + L.psi);
+    h->spec = (cd*)(w + L.spec);
+    h->vdd = (double*)(w + L.vdd);
+    h->phi = (double*)(w + L.phi);
+    h->scal = (double*)(w + L.scal);
+    h->partial = (double*)(w + L.partial);
+    h->ticket = (unsigned int*)(w + L.ticket);
+    h->obs_dev = (double*)(w + L.obs);
+    h->npartial = NPARTIAL;
+    const char* fe = getenv("DBEC_FUSE_CNX");
+    h->fuse_cnx = fe ? atoi(fe) : 1;
+    const char* ge = getenv("DBEC_GRAPH");
+    h->use_graph = ge ? atoi(ge) : 1;
+
+#define FAIL(code) do { delete h; return (code); } while (0)
+    if (cudaMemsetAsync(h->psi, 0, sizeof(cd) * h->P, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
+    if (cudaMemsetAsync(h->ticket, 0, 256, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
+    if (cudaMemsetAsync(h->spec, 0, sizeof(cd) * h->SP, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
+    char* t = w + L.tables;
+    const double om[3] = {p->nu, p->lambda, p->kappa};
+    const double dd[3] = {p->dx, p->dy, p->ndim == 3 ? p->dz : 1.0};
+    const int nn[3] = {p->nx, p->ny, p->nz};
+    for (int ax = 0; ax < 3; ++ax) {
+        size_t used = 0;
+        rc = upload_axis(h, ax, nn[ax], dd[ax], (p->ndim == 2 && ax == 2) ? 0.0 : om[ax], t, &used);
+        if (rc) FAIL(rc);
+        t += used;
+    }
+    if (write_scalars(h, true)) FAIL(DBEC_ECUDA);
+    if (dbec_launch_build_vdd(h)) FAIL(DBEC_ECUDA);
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
+#undef FAIL
+    *out = h;
+    return DBEC_OK;
+}
+
+int dbec_destroy(dbec_handle h) {
+    if (!h) return DBEC_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    delete h;
+    return DBEC_OK;
+}
+
+int dbec_last_cuda_error(dbec_handle h) { return h ? h->last_cuda : 0; }
+
+int dbec_set_psi(dbec_handle h, const void* psi, int on_device) {
+    if (!h || !psi) return DBEC_EINVAL;
+    CU(h, cudaMemcpyAsync(h->psi, psi, sizeof(cd) * h->P, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                          h->stream));
+    // a fresh field carries no deferred norm factor
+    double one[2] = {1.0, 1.0};
+    CU(h, cudaMemcpyAsync(h->scal + SC_S, one, sizeof(one), cudaMemcpyHostToDevice, h->stream));
+    if (!on_device) CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
+int dbec_get_psi(dbec_handle h, void* psi, int on_device) {
+    if (!h || !psi) return DBEC_EINVAL;
+    if (h->p.time_mode == 0) LAUNCH(h, dbec_launch_apply_scale(h));     // s is 1 for ever in real time
+    CU(h, cudaMemcpyAsync(psi, h->psi, sizeof(cd) * h->P, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                          h->stream));
+    if (!on_device) CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
+int dbec_set_coupling(dbec_handle h, double G, double D) {
+    if (!h) return DBEC_EINVAL;
+    h->p.G = G; h->p.D = D;
+    double v[2] = {G, D};
+    CU(h, cudaMemcpyAsync(h->scal + SC_G, v, sizeof(v), cudaMemcpyHostToDevice, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
+int dbec_step(dbec_handle h, int nsteps) {
+    if (!h || nsteps < 0) return DBEC_EINVAL;
+    if (!h->use_graph) {
+        for (int i = 0; i < nsteps; ++i) { int rc = enqueue_step(h); if (rc) return rc; }
+        return DBEC_OK;
+    }
+    if (!h->graph_exec) {
+        // warm every kernel once outside capture is not needed: launches inside a capture are recorded,
+        // not executed; function attributes (dynamic shared memory) are set by the launchers up front.
+        cudaGraph_t g = nullptr;
+        const long long before = h->launches;
+        CU(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+        int rc = enqueue_step(h);
+        cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+        h->launches_per_step = (int)(h->launches - before);
+        h->launches = before;
+        if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+        if (e != cudaSuccess) return cuda_fail(h, e);
+        e = cudaGraphInstantiate(&h->graph_exec, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) return cuda_fail(h, e);
+    }
+    for (int i = 0; i < nsteps; ++i) {
+        CU(h, cudaGraphLaunch(h->graph_exec, h->stream));
+        h->launches += h->launches_per_step;
+    }
+    return DBEC_OK;
+}
+
+int dbec_phi_dd(dbec_handle h, void* phi_f64_dev) {
+    if (!h || !phi_f64_dev) return DBEC_EINVAL;
+    LAUNCH(h, dbec_launch_density_fft(h));
+    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    LAUNCH(h, dbec_launch_phi_out(h, (double*)phi_f64_dev));
+    return DBEC_OK;
+}
+
+int dbec_cn_sweep(dbec_handle h, int axis) {
+    if (!h || axis < 0 || axis > 2 || (h->p.ndim == 2 && axis == 2)) return DBEC_EINVAL;
+    LAUNCH(h, dbec_launch_cn(h, axis, 0));
+    return DBEC_OK;
+}
+
+int dbec_nonlinear(dbec_handle h) {
+    if (!h) return DBEC_EINVAL;
+    LAUNCH(h, dbec_launch_density_fft(h));
+    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    LAUNCH(h, dbec_launch_nonlinear(h, 0));
+    return DBEC_OK;
+}
+
+int dbec_normalize(dbec_handle h) {
+    if (!h) return DBEC_EINVAL;
+    LAUNCH(h, dbec_launch_normalize(h));
+    return DBEC_OK;
+}
+
+int dbec_observables(dbec_handle h, dbec_obs* out) {
+    if (!h || !out) return DBEC_EINVAL;
+    LAUNCH(h, dbec_launch_density_fft(h));
+    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    LAUNCH(h, dbec_launch_phi_out(h, h->phi));
+    LAUNCH(h, dbec_launch_observables(h));
+    double v[16];
+    CU(h, cudaMemcpyAsync(v, h->obs_dev, sizeof(double) * 9, cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    out->norm = v[0]; out->mu = v[1]; out->energy = v[2];
+    out->rms_x = v[3]; out->rms_y = v[4]; out->rms_z = v[5]; out->rms_r = v[6];
+    out->density0 = v[7]; out->density_max = v[8];
+    return DBEC_OK;
+}
+
+int dbec_launch_count(dbec_handle h, long long* launches) {
+    if (!h || !launches) return DBEC_EINVAL;
+    *launches = h->launches;
+    return DBEC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,72 @@
+// dbec_internal.hpp — what the translation units of libdbec.so share: the host-side handle and the
+// launcher prototypes.  Product path only; nothing here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/dbec.h"
+#include "cplx.cuh"
+
+#define DBEC_MAX_N 512          // longest supported grid line (16 values per thread x 32 lanes)
+#define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
+
+// Device scalars every kernel reads (so that a captured CUDA graph never bakes them in).
+//   [0] s      deferred norm factor: true psi = s * stored psi (calcnorm; 1 in real time)
+//   [1] s^2
+//   [2] G      coefficient of |psi|^2            (dbec_set_coupling)
+//   [3] D      coefficient of Phi_dd
+enum { SC_S = 0, SC_S2 = 1, SC_G = 2, SC_D = 3, SC_COUNT = 8 };
+
+// Per-axis tables on the device.
+struct AxisTables {
+    int n;                  // points along the axis
+    const cd* twA;          // stage-1 FFT twiddles, order [k1][m]           (n entries)
+    const cd* twN;          // exp(-2 pi i j / n)                              (n entries)
+    const double* vtrap;    // 1/2 omega^2 x_i^2                               (n entries)
+    const double* x2;       // x_i^2                                           (n entries)
+    // Crank-Nicolson tables (cn_chunk.cuh): real in imaginary time, complex in real time; stored as
+    // complex in both cases, the imaginary-time kernels read the real parts only through *_re.
+    // pfe[c] = PF at the last point of chunk c, pbs[c] = PB at the first point of chunk c.
+    const cd* h;  const cd* pf;  const cd* pb;  const cd* pfe;  const cd* pbs;
+    const double* h_re; const double* pf_re; const double* pb_re; const double* pfe_re; const double* pbs_re;
+    cd kap;                 // (1 - 2a)/a
+};
+
+struct dbec_handle_s {
+    dbec_params p;
+    cudaStream_t stream;
+    int last_cuda;
+    long long launches;
+    // geometry
+    int nx, ny, nz, nxhp;           // nxhp = padded half-spectrum row length (multiple of DBEC_SPEC_COLS)
+    long long P;                    // nx*ny*nz
+    long long SP;                   // nz*ny*nxhp
+    double dV;
+    // device memory (all inside the caller's workspace)
+    cd* psi;                        // [nz][ny][nx]
+    cd* spec;                       // [nz][ny][nxhp] half spectrum of the density
+    double* vdd;                    // [nz][ny][nxhp] V_dd(k)/P
+    double* phi;                    // [nz][ny][nx] Phi_dd (observables / dbec_phi_dd only)
+    double* scal;                   // SC_COUNT doubles
+    double* partial;                // reduction partials
+    unsigned int* ticket;           // last-block tickets
+    double* obs_dev;                // 16 doubles
+    AxisTables ax[3];
+    int npartial;
+    // CUDA graph of one step
+    cudaGraphExec_t graph_exec;
+    int launches_per_step;
+    int use_graph;                  // env DBEC_GRAPH (default 1): replay one captured step per dbec_step iteration
+    int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
+};
+
+// ---- launchers (each returns a cudaError_t as int; all asynchronous on h->stream) ----
+int dbec_launch_density_fft(dbec_handle_s* h);             // a1: psi -> spec (forward transforms done, all axes)
+int dbec_launch_kernel_mul_inverse(dbec_handle_s* h);      // a2 + inverse transforms except x (fused with the last forward)
+int dbec_launch_nonlinear(dbec_handle_s* h, int fuse_cnx); // a3 (x, C2R) + a4 [+ a5]
+int dbec_launch_phi_out(dbec_handle_s* h, double* phi);    // a3 writing Phi_dd only
+int dbec_launch_cn(dbec_handle_s* h, int axis, int with_norm);   // a5..a7 (+ a8 partial sums and factor)
+int dbec_launch_normalize(dbec_handle_s* h);               // a8 alone
+int dbec_launch_apply_scale(dbec_handle_s* h);             // psi <- s psi, s <- 1
+int dbec_launch_observables(dbec_handle_s* h);             // a9 (expects h->phi filled)
+int dbec_launch_build_vdd(dbec_handle_s* h);               // potdd table

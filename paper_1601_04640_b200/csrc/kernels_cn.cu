@@ -1,0 +1,339 @@
+// kernels_cn.cu — Crank-Nicolson sweeps (calclux / calcluy / calcluz), the norm
+// (calcnorm) and the observables (calcmuen, calcrms).
+//
+// The paper gives each grid line to one thread that runs the whole "recursive relation" and keeps
+// its coefficient array in global memory.  Here a line is cut into chunks of 16 points
+// held in registers, one thread per chunk, and the chunks are tied together by an exact carry
+// recurrence over the chunk ends (cn_chunk.cuh), so a tile of lines is read once and written once:
+//   k_cn_strided   y or z sweep: a tile of COLS neighbouring lines; every global access is a run of
+//                  COLS consecutive complex128 values (COLS x 16 B).  Optionally accumulates the
+//                  block's sum of |psi|^2 and lets the last block turn the partial sums into the
+//                  deferred norm factor (imaginary time), so that calcnorm costs no pass of its own.
+//   k_cn_x         x sweep alone: lines are contiguous; coalesced loads, transposition through a
+//                  padded shared row (cn_line_smem.cuh).
+#include "dbec_internal.hpp"
+#include "cn_chunk.cuh"
+#include "cn_line_smem.cuh"
+
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
+
+// Sum over the block in a fixed order (warp shuffles, then warp 0 over the warp sums).
+template <int NT> __device__ __forceinline__ double block_sum(double x, double* red) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    constexpr int NW = (NT + 31) / 32;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) red[w] = x;
+    __syncthreads();
+    double t = (threadIdx.x < NW) ? red[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    }
+    return t;   // valid in thread 0
+}
+
+__device__ __forceinline__ double block_max(double x, double* red) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_down_sync(0xffffffffu, x, o));
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (l == 0) red[w] = x;
+    __syncthreads();
+    double t = (threadIdx.x < nw) ? red[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t = fmax(t, __shfl_down_sync(0xffffffffu, t, o));
+    }
+    return t;
+}
+
+// The last block to finish adds the per-block partial sums in index order and writes the deferred
+// norm factor s = 1/sqrt(dV sum |psi|^2)   (calcnorm; reading S13).
+__device__ __forceinline__ void norm_finish(double part, double* __restrict__ partial, unsigned int* ticket,
+                                            double* __restrict__ scal, double dV, double* red) {
+    __shared__ bool last;
+    const unsigned int nb = gridDim.x * gridDim.y;
+    const unsigned int b = blockIdx.y * gridDim.x + blockIdx.x;
+    if (threadIdx.x == 0) {
+        partial[b] = part;
+        __threadfence();
+        last = (atomicAdd(ticket, 1u) == nb - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double acc = 0.0;
+    for (unsigned int i = threadIdx.x; i < nb; i += blockDim.x) acc += __ldcg(partial + i);
+    // fixed order: thread t owns indices t, t+NT, ...; then the block tree
+    double tot;
+    {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+        __syncthreads();
+        if (l == 0) red[w] = acc;
+        __syncthreads();
+        tot = 0.0;
+        if (threadIdx.x == 0)
+            for (int i = 0; i < nw; ++i) tot += red[i];
+    }
+    if (threadIdx.x == 0) {
+        const double s = 1.0 / sqrt(tot * dV);
+        scal[SC_S] = s;
+        scal[SC_S2] = s * s;
+        *ticket = 0u;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// strided sweeps
+// ------------------------------------------------------------------------------------------------
+template <bool RT, int NCH, int COLS, bool NORM>
+__global__ void __launch_bounds__(NCH* COLS)
+k_cn_strided(cd* __restrict__ psi, CnTab<RT> cn, long long line_stride, long long outer_stride,
+             double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV) {
+    typedef typename CnCoef<RT>::type CT;
+    __shared__ cd edge[2][NCH][COLS];     // first and last point of every chunk (halo of the neighbours)
+    __shared__ cd ends[2][NCH][COLS];     // zero-start chunk results for the carries
+    __shared__ double red[32];
+    const int col = threadIdx.x % COLS, c = threadIdx.x / COLS;
+    cd* g = psi + (long long)blockIdx.y * outer_stride + (long long)blockIdx.x * COLS + col +
+            (long long)(c * CN_L) * line_stride;
+    cd u[CN_L];
+#pragma unroll
+    for (int i = 0; i < CN_L; ++i) u[i] = g[i * line_stride];
+    if (NCH > 1) {
+        edge[0][c][col] = u[0];
+        edge[1][c][col] = u[CN_L - 1];
+        __syncthreads();
+    }
+    const cd lo = (c > 0) ? edge[1][c - 1][col] : cmake(0.0, 0.0);
+    const cd hi = (c < NCH - 1) ? edge[0][c + 1][col] : cmake(0.0, 0.0);
+    const int j0 = c * CN_L;
+    cn_chunk_forward<CT>(u, lo, hi, cn.kap, cn.h + j0);
+    cd din = cmake(0.0, 0.0), uin = cmake(0.0, 0.0);
+    if (NCH > 1) {
+        ends[0][c][col] = u[CN_L - 1];
+        __syncthreads();
+        din = cn_carry_forward<CT>(c, &ends[0][0][col], COLS, cn.pfe);
+    }
+    cn_chunk_backward<CT>(u, din, cn.h + j0, cn.pf + j0);
+    if (NCH > 1) {
+        ends[1][c][col] = u[0];
+        __syncthreads();
+        uin = cn_carry_backward<CT>(c, NCH, &ends[1][0][col], COLS, cn.pbs);
+    }
+    cn_chunk_fix<CT>(u, uin, cn.pb + j0);
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < CN_L; ++i) {
+        g[i * line_stride] = u[i];
+        if (NORM) acc += cnorm2(u[i]);
+    }
+    if (NORM) {
+        const double part = block_sum<NCH * COLS>(acc, red);
+        norm_finish(part, partial, ticket, scal, dV, red);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// x sweep alone
+// ------------------------------------------------------------------------------------------------
+template <bool RT, int T, int LPB, bool NORM>
+__global__ void __launch_bounds__(T* LPB)
+k_cn_x(cd* __restrict__ psi, CnTab<RT> cn, int nlines, double* __restrict__ partial, unsigned int* ticket,
+       double* __restrict__ scal, double dV) {
+    extern __shared__ cd smem[];
+    __shared__ double red[32];
+    constexpr int N = 16 * T;
+    const int lp = threadIdx.x / T, m = threadIdx.x % T;
+    long long line = (long long)blockIdx.x * LPB + lp;
+    const bool active = line < nlines;
+    if (!active) line = 0;
+    cd* sm = smem + lp * (N + 3 * T);
+    cd* g = psi + line * N;
+    cd q[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) q[j] = g[j * T + m];
+    cn_line_via_smem<RT, T>(q, m, sm, cn);
+    double acc = 0.0;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        if (active) { g[j * T + m] = q[j]; if (NORM) acc += cnorm2(q[j]); }
+    }
+    if (NORM) {
+        const double part = block_sum<T * LPB>(acc, red);
+        norm_finish(part, partial, ticket, scal, dV, red);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// calcnorm alone, psi <- s psi, and the observables
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_norm(const cd* __restrict__ psi, long long P, double* __restrict__ partial, unsigned int* ticket,
+       double* __restrict__ scal, double dV) {
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < P; i += (long long)gridDim.x * 256)
+        acc += cnorm2(psi[i]);
+    const double part = block_sum<256>(acc, red);
+    norm_finish(part, partial, ticket, scal, dV, red);
+}
+
+__global__ void __launch_bounds__(256) k_apply_scale(cd* __restrict__ psi, long long P, const double* __restrict__ scal) {
+    const double s = scal[SC_S];
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < P; i += (long long)gridDim.x * 256)
+        psi[i] = cmul(s, psi[i]);
+}
+__global__ void k_reset_scale(double* scal) { scal[SC_S] = 1.0; scal[SC_S2] = 1.0; }
+
+// Observable partial sums (reading S13, S14; definitions in DESIGN.md "Observables"), per block:
+//   0 sum n   1 sum x^2 n   2 sum y^2 n   3 sum z^2 n   4 sum n^2   5 sum Phi n
+//   6 sum |psi(x+1)-psi|^2   7 same along y   8 same along z   9 max n
+enum { OB_N = 0, OB_X2, OB_Y2, OB_Z2, OB_N2, OB_PHIN, OB_KX, OB_KY, OB_KZ, OB_MAX, OB_COUNT };
+
+__global__ void __launch_bounds__(256)
+k_obs_partial(const cd* __restrict__ psi, const double* __restrict__ phi, const double* __restrict__ scal,
+              const double* __restrict__ x2, const double* __restrict__ y2, const double* __restrict__ z2,
+              int nx, int ny, int nz, double* __restrict__ partial) {
+    __shared__ double red[32];
+    const long long P = (long long)nx * ny * nz;
+    const double s2 = scal[SC_S2];
+    double a[OB_COUNT];
+#pragma unroll
+    for (int k = 0; k < OB_COUNT; ++k) a[k] = 0.0;
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < P; i += (long long)gridDim.x * 256) {
+        const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((long long)nx * ny));
+        const cd p = psi[i];
+        const double n = s2 * cnorm2(p);
+        a[OB_N] += n;
+        a[OB_X2] += x2[ix] * n;
+        a[OB_Y2] += y2[iy] * n;
+        a[OB_Z2] += z2[iz] * n;
+        a[OB_N2] += n * n;
+        a[OB_PHIN] += phi[i] * n;
+        if (ix + 1 < nx) a[OB_KX] += s2 * cnorm2(csub(psi[i + 1], p));
+        if (iy + 1 < ny) a[OB_KY] += s2 * cnorm2(csub(psi[i + nx], p));
+        if (iz + 1 < nz) a[OB_KZ] += s2 * cnorm2(csub(psi[i + (long long)nx * ny], p));
+        a[OB_MAX] = fmax(a[OB_MAX], n);
+    }
+#pragma unroll
+    for (int k = 0; k < OB_COUNT; ++k) {
+        const double t = (k == OB_MAX) ? block_max(a[k], red) : block_sum<256>(a[k], red);
+        if (threadIdx.x == 0) partial[(long long)k * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+// One block: fixed-order sums over the block partials, then the observables.
+__global__ void __launch_bounds__(256)
+k_obs_final(const double* __restrict__ partial, int nb, const cd* __restrict__ psi, const double* __restrict__ scal,
+            long long centre, double dV, double dx, double dy, double dz, int ndim, double nu, double lam,
+            double kap, double* __restrict__ out) {
+    __shared__ double red[32];
+    __shared__ double tot[OB_COUNT];
+    for (int k = 0; k < OB_COUNT; ++k) {
+        double acc = 0.0;
+        for (int i = threadIdx.x; i < nb; i += 256)
+            acc = (k == OB_MAX) ? fmax(acc, partial[(long long)k * nb + i]) : acc + partial[(long long)k * nb + i];
+        const double t = (k == OB_MAX) ? block_max(acc, red) : block_sum<256>(acc, red);
+        if (threadIdx.x == 0) tot[k] = t;
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    const double G = scal[SC_G], D = scal[SC_D], s2 = scal[SC_S2];
+    const double S = dV * tot[OB_N];
+    const double sx2 = dV * tot[OB_X2], sy2 = dV * tot[OB_Y2], sz2 = (ndim == 3) ? dV * tot[OB_Z2] : 0.0;
+    const double ekin = 0.5 * dV * (tot[OB_KX] / (dx * dx) + tot[OB_KY] / (dy * dy) +
+                                    (ndim == 3 ? tot[OB_KZ] / (dz * dz) : 0.0));
+    const double etr = 0.5 * (nu * nu * sx2 + lam * lam * sy2 + kap * kap * sz2);
+    const double ec = G * dV * tot[OB_N2];
+    const double ed = D * dV * tot[OB_PHIN];
+    out[0] = S;
+    out[1] = (ekin + etr + ec + ed) / S;
+    out[2] = (ekin + etr + 0.5 * ec + 0.5 * ed) / S;
+    out[3] = sqrt(sx2 / S);
+    out[4] = sqrt(sy2 / S);
+    out[5] = sqrt(sz2 / S);
+    out[6] = sqrt((sx2 + sy2 + sz2) / S);
+    out[7] = s2 * cnorm2(psi[centre]);
+    out[8] = tot[OB_MAX];
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+template <bool RT, int NCH, bool NORM> static int launch_cn_strided(dbec_handle_s* h, int axis) {
+    constexpr int COLS = (NCH >= 16) ? 16 : (NCH >= 4 ? 32 : 64);      // 256 / 128 / 64..128 threads
+    long long line_stride, outer_stride, ncols;
+    int nouter;
+    if (axis == 1) { line_stride = h->nx; outer_stride = (long long)h->nx * h->ny; ncols = h->nx; nouter = h->nz; }
+    else { line_stride = (long long)h->nx * h->ny; outer_stride = 0; ncols = line_stride; nouter = 1; }
+    // COLS must divide the column count: nx >= 16 and for z: nx*ny >= 256
+    if (ncols % COLS) return (int)cudaErrorInvalidValue;
+    dim3 grid((unsigned)(ncols / COLS), (unsigned)nouter);
+    if (NORM && (long long)grid.x * grid.y > h->npartial) return (int)cudaErrorInvalidValue;
+    k_cn_strided<RT, NCH, COLS, NORM><<<grid, NCH * COLS, 0, h->stream>>>(
+        h->psi, make_cntab<RT>(h->ax[axis]), line_stride, outer_stride, h->partial, h->ticket, h->scal, h->dV);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <bool RT, int NCH, bool NORM> static int launch_cn_x(dbec_handle_s* h) {
+    constexpr int T = NCH, LPB = 256 / T;
+    const int nlines = h->ny * h->nz;
+    const size_t sm = (size_t)LPB * (16 * T + 3 * T) * sizeof(cd);
+    auto k = k_cn_x<RT, T, LPB, NORM>;
+    if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const int nb = (nlines + LPB - 1) / LPB;
+    if (NORM && nb > h->npartial) return (int)cudaErrorInvalidValue;
+    k<<<nb, T * LPB, sm, h->stream>>>(h->psi, make_cntab<RT>(h->ax[0]), nlines, h->partial, h->ticket, h->scal, h->dV);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <bool RT, bool NORM> static int launch_cn_rt(dbec_handle_s* h, int axis) {
+    const int n = h->ax[axis].n;
+#define CASE_(nch) case nch * 16: return axis == 0 ? launch_cn_x<RT, nch, NORM>(h) : launch_cn_strided<RT, nch, NORM>(h, axis)
+    switch (n) {
+        CASE_(1); CASE_(2); CASE_(4); CASE_(8); CASE_(16); CASE_(32);
+        default: return (int)cudaErrorInvalidValue;
+    }
+#undef CASE_
+}
+
+int dbec_launch_cn(dbec_handle_s* h, int axis, int with_norm) {
+    if (h->p.time_mode == 1) return with_norm ? launch_cn_rt<true, true>(h, axis) : launch_cn_rt<true, false>(h, axis);
+    return with_norm ? launch_cn_rt<false, true>(h, axis) : launch_cn_rt<false, false>(h, axis);
+}
+
+int dbec_launch_normalize(dbec_handle_s* h) {
+    // true psi = s * stored psi: bring the stored field to s = 1 first, then take the norm factor
+    int rc = dbec_launch_apply_scale(h);
+    if (rc) return rc;
+    int nb = h->npartial < 148 * 8 ? h->npartial : 148 * 8;
+    k_norm<<<nb, 256, 0, h->stream>>>(h->psi, h->P, h->partial, h->ticket, h->scal, h->dV);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_apply_scale(dbec_handle_s* h) {
+    k_apply_scale<<<148 * 8, 256, 0, h->stream>>>(h->psi, h->P, h->scal);
+    k_reset_scale<<<1, 1, 0, h->stream>>>(h->scal);
+    h->launches += 2;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_observables(dbec_handle_s* h) {
+    int nb = h->npartial / OB_COUNT;
+    if (nb > 148 * 8) nb = 148 * 8;
+    k_obs_partial<<<nb, 256, 0, h->stream>>>(h->psi, h->phi, h->scal, h->ax[0].x2, h->ax[1].x2, h->ax[2].x2, h->nx,
+                                             h->ny, h->nz, h->partial);
+    const long long centre = (h->nx / 2) + (long long)h->nx * ((h->ny / 2) + (long long)h->ny * (h->p.ndim == 3 ? h->nz / 2 : 0));
+    k_obs_final<<<1, 256, 0, h->stream>>>(h->partial, nb, h->psi, h->scal, centre, h->dV, h->p.dx, h->p.dy, h->p.dz,
+                                          h->p.ndim, h->p.nu, h->p.lambda, h->p.kappa, h->obs_dev);
+    h->launches += 2;
+    return (int)cudaGetLastError();
+}

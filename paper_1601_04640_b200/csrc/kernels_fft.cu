@@ -1,0 +1,388 @@
+// kernels_fft.cu — the dipolar mean field (calcpsidd2) and the nonlinear
+// step (calcnu) as hand-written sm_100a kernels.  No library FFT.
+//
+//   k_density_fftx   a1, x axis: n = |s psi|^2 fused into a forward real-to-complex transform.  Two
+//                    real grid lines ride one complex FFT (re = line y, im = line y+1) and are split
+//                    by Hermitian symmetry ("density ... purely real ... Hermitian").
+//   k_fft_strided    a1/a3 along y or z on the half spectrum: tiles of 8 columns x N rows held in
+//                    registers, 128-byte coalesced rows.  MODE_FMI chains forward transform, the
+//                    multiply by V_dd(k)/P (a2, PAPER.md:63 "convolution theorem", :75 `potdd`) and
+//                    the inverse transform of the same axis while the line stays on chip.
+//   k_ifftx_nonlin   a3 x axis (complex-to-real, two lines per FFT) fused with
+//                    psi <- s psi exp(-c dt (V + G n + D Phi))   (a4), optionally followed by the
+//                    Crank-Nicolson sweep along x on the same line (a5), or writing Phi_dd only.
+#include "dbec_internal.hpp"
+#include "fft_line.cuh"
+#include "cn_chunk.cuh"
+#include "cn_line_smem.cuh"
+
+// One line FFT in registers with its shared-memory exchanges.  SYNC = 0: the T threads of a line sit
+// in one warp (__syncwarp); SYNC = 1: block-wide barrier (tile kernels).
+template <class P, int S, int SYNC>
+__device__ __forceinline__ void fft_line(cd (&v)[16], int m, cd* sm, int es, const cd* __restrict__ twA,
+                                         const cd* __restrict__ twN) {
+    fft_stage1<P, S>(v, m, twA);
+    if (P::T > 1) {
+        fft_x1_write<P>(v, m, sm, es);
+        if (SYNC) __syncthreads(); else __syncwarp();
+        fft_stage2<P, S>(v, m, sm, es, twN);
+        if (P::R3 > 1) {
+            if (SYNC) __syncthreads(); else __syncwarp();
+            fft_x2_write<P>(v, m, sm, es);
+            if (SYNC) __syncthreads(); else __syncwarp();
+            fft_stage3<P, S>(v, m, sm, es);
+        }
+    }
+}
+
+template <class P> struct XLine {
+    // shared elements per line pair of the contiguous-x kernels: FFT exchange or one padded line
+    static constexpr int PADN = P::N + 3 * P::T;   // padded line + two rows of chunk ends (cn_line_smem.cuh)
+    static constexpr int SM = (P::SMEM > PADN ? P::SMEM : PADN);
+};
+
+// ------------------------------------------------------------------------------------------------
+// a1, x axis
+// ------------------------------------------------------------------------------------------------
+template <class P, int LP>
+__global__ void __launch_bounds__(P::T* LP)
+k_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA,
+               const cd* __restrict__ twN, const double* __restrict__ scal, int npairs, int nxhp) {
+    extern __shared__ cd smem[];
+    constexpr int T = P::T, N = P::N;
+    const int lp = threadIdx.x / T, m = threadIdx.x % T;
+    const long long pair = (long long)blockIdx.x * LP + lp;
+    const bool active = pair < npairs;
+    cd* sm = smem + lp * XLine<P>::SM;
+    const double s2 = scal[SC_S2];
+    const cd* pa = psi + (active ? pair : 0) * 2 * N;
+    const cd* pb = pa + N;
+    cd v[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        cd a = pa[j * T + m], b = pb[j * T + m];
+        v[j] = cmake(s2 * cnorm2(a), s2 * cnorm2(b));
+    }
+    fft_line<P, -1, 0>(v, m, sm, 1, twA, twN);
+    __syncwarp();
+    // Z[k] to shared memory so that each thread can reach its mirror Z[N-k]
+#pragma unroll
+    for (int j = 0; j < 16; ++j) sm[j * T + m] = v[j];
+    __syncwarp();
+    cd* oa = spec + (active ? pair : 0) * 2 * nxhp;
+    cd* ob = oa + nxhp;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const int k = j * T + m;
+        if (k <= N / 2) {
+            cd z = v[j], zp = sm[(N - k) & (N - 1)];
+            // X_a = (Z[k] + conj Z[N-k])/2,  X_b = (Z[k] - conj Z[N-k])/(2i)
+            cd xa = cmake(0.5 * (z.x + zp.x), 0.5 * (z.y - zp.y));
+            cd xb = cmake(0.5 * (z.y + zp.y), -0.5 * (z.x - zp.x));
+            if (active) { oa[k] = xa; ob[k] = xb; }
+        } else if (k < nxhp) {
+            if (active) { oa[k] = cmake(0.0, 0.0); ob[k] = cmake(0.0, 0.0); }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// strided transforms on the half spectrum
+// ------------------------------------------------------------------------------------------------
+enum { MODE_FWD = 0, MODE_INV = 1, MODE_FMI = 2 };
+
+// A line's point j sits at  base + j*line_stride,  base = outer*outer_stride + column;  a tile is
+// DBEC_SPEC_COLS consecutive columns.  TILES tiles per block.
+template <class P, int MODE, int TILES>
+__global__ void __launch_bounds__(P::T* DBEC_SPEC_COLS* TILES)
+k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twA,
+              const cd* __restrict__ twN, long long line_stride, long long outer_stride, int ntiles_x,
+              long long ntiles) {
+    extern __shared__ cd smem[];
+    constexpr int T = P::T, C = DBEC_SPEC_COLS;
+    const int tl = threadIdx.x / (T * C), r = threadIdx.x % (T * C);
+    const int col = r % C, m = r / C;
+    long long tile = (long long)blockIdx.x * TILES + tl;
+    const bool active = tile < ntiles;
+    if (!active) tile = 0;
+    const long long outer = tile / ntiles_x, tx = tile % ntiles_x;
+    const long long base = outer * outer_stride + tx * C + col;
+    cd* sm = smem + tl * (P::SMEM * C) + col;
+    cd* g = spec + base;
+    cd v[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = g[(long long)(j * T + m) * line_stride];
+    if (MODE == MODE_FWD || MODE == MODE_FMI) fft_line<P, -1, 1>(v, m, sm, C, twA, twN);
+    if (MODE == MODE_FMI) {
+        const double* w = vdd + base;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) v[j] = cmul(w[(long long)(j * T + m) * line_stride], v[j]);
+        if (T > 1) __syncthreads();
+    }
+    if (MODE == MODE_INV || MODE == MODE_FMI) fft_line<P, +1, 1>(v, m, sm, C, twA, twN);
+    if (active) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) g[(long long)(j * T + m) * line_stride] = v[j];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3 (x axis, complex-to-real) + a4 (+ a5)
+// ------------------------------------------------------------------------------------------------
+enum { NL_STEP = 0, NL_STEP_CNX = 1, NL_PHI = 2 };
+
+template <class P, int LP, bool RT, int MODE>
+__global__ void __launch_bounds__(P::T* LP)
+k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out,
+               const cd* __restrict__ twA, const cd* __restrict__ twN, const double* __restrict__ scal,
+               const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+               double dt, int npairs, int nxhp, int ny, CnTab<RT> cn) {
+    extern __shared__ cd smem[];
+    constexpr int T = P::T, N = P::N;
+    const int lp = threadIdx.x / T, m = threadIdx.x % T;
+    long long pair = (long long)blockIdx.x * LP + lp;
+    const bool active = pair < npairs;
+    if (!active) pair = 0;
+    cd* sm = smem + lp * XLine<P>::SM;
+    const cd* sa = spec + pair * 2 * nxhp;
+    const cd* sb = sa + nxhp;
+    cd v[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const int k = j * T + m;
+        if (k <= N / 2) {
+            cd a = sa[k], b = sb[k];
+            v[j] = cmake(a.x - b.y, a.y + b.x);          // X_a + i X_b
+        } else {
+            cd a = sa[N - k], b = sb[N - k];
+            v[j] = cmake(a.x + b.y, b.x - a.y);          // conj X_a + i conj X_b
+        }
+    }
+    fft_line<P, +1, 0>(v, m, sm, 1, twA, twN);
+    // v[j] = (Phi_dd on line y, Phi_dd on line y+1) at x = j*T + m   (1/P is inside the V_dd table)
+    if (MODE == NL_PHI) {
+        double* fa = phi_out + pair * 2 * N;
+        double* fb = fa + N;
+        if (active) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) { fa[j * T + m] = v[j].x; fb[j * T + m] = v[j].y; }
+        }
+        return;
+    }
+    const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
+    const long long row = pair * 2;
+    const int y = (int)(row % ny), z = (int)(row / ny);
+    const double va = vy[y] + vz[z], vb = vy[y + 1] + vz[z];
+    cd* pa = psi + row * N;
+    cd* pb = pa + N;
+    cd qa[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const int k = j * T + m;
+        const double vxk = vx[k];
+        cd a = pa[k], b = pb[k];
+        const double ua = dt * (vxk + va + G * (s2 * cnorm2(a)) + D * v[j].x);
+        const double ub = dt * (vxk + vb + G * (s2 * cnorm2(b)) + D * v[j].y);
+        if (RT) {
+            double sn, cs;
+            sincos(ua, &sn, &cs);
+            qa[j] = cmul(s, cmul(a, cmake(cs, -sn)));
+            sincos(ub, &sn, &cs);
+            v[j] = cmul(s, cmul(b, cmake(cs, -sn)));
+        } else {
+            qa[j] = cmul(s * exp(-ua), a);
+            v[j] = cmul(s * exp(-ub), b);
+        }
+    }
+    if (MODE == NL_STEP) {
+        if (active) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) { pa[j * T + m] = qa[j]; pb[j * T + m] = v[j]; }
+        }
+    } else {
+        __syncwarp();
+        cn_line_via_smem<RT, T>(qa, m, sm, cn);
+        if (active) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) pa[j * T + m] = qa[j];
+        }
+        __syncwarp();
+        cn_line_via_smem<RT, T>(v, m, sm, cn);
+        if (active) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) pb[j * T + m] = v[j];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// V_dd table (the paper's `potdd`), half spectrum, scaled by 1/P (reading S8)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double wavenumber(int mi, int n, double d) {     // reading S6
+    int mt = (mi < n / 2) ? mi : mi - n;
+    if (n == 1) mt = 0;
+    return 6.283185307179586476925286766559 * (double)mt / ((double)n * d);
+}
+
+__global__ void k_build_vdd(double* __restrict__ vdd, int ndim, int nx, int ny, int nz, int nxhp, double dx,
+                            double dy, double dz, double d_perp, double cutoff, double invP) {
+    const long long total = (long long)nz * ny * nxhp;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int mx = (int)(i % nxhp);
+        const int my = (int)((i / nxhp) % ny);
+        const int mz = (int)(i / ((long long)nxhp * ny));
+        double v = 0.0;
+        if (mx <= nx / 2) {
+            const double kx = wavenumber(mx, nx, dx), ky = wavenumber(my, ny, dy);
+            if (ndim == 2) {                                                  // reading S21
+                const double xi = sqrt(kx * kx + ky * ky) * d_perp * 0.70710678118654752440;
+                v = 2.0 - 3.0 * 1.7724538509055160272981674833411 * xi * erfcx(xi);
+            } else {
+                const double kz = wavenumber(mz, nz, dz);
+                const double k2 = kx * kx + ky * ky + kz * kz;
+                if (k2 > 0.0) {                                               // readings S3, S4
+                    v = 3.0 * kz * kz / k2 - 1.0;
+                    if (cutoff > 0.0) {                                       // reading S5
+                        const double kr = sqrt(k2) * cutoff;
+                        v *= 1.0 + 3.0 * cos(kr) / (kr * kr) - 3.0 * sin(kr) / (kr * kr * kr);
+                    }
+                }
+            }
+        }
+        vdd[i] = v * invP;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
+
+template <class K> static int set_smem(K kernel, size_t bytes) {
+    if (bytes > 48 * 1024)
+        CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return 0;
+}
+
+template <int N> struct PlanOf;
+template <> struct PlanOf<16>  { typedef FftPlan<1, 1, true> X;  typedef FftPlan<1, 1, false> S; };
+template <> struct PlanOf<32>  { typedef FftPlan<2, 1, true> X;  typedef FftPlan<2, 1, false> S; };
+template <> struct PlanOf<64>  { typedef FftPlan<4, 1, true> X;  typedef FftPlan<4, 1, false> S; };
+template <> struct PlanOf<128> { typedef FftPlan<8, 1, true> X;  typedef FftPlan<8, 1, false> S; };
+template <> struct PlanOf<256> { typedef FftPlan<16, 1, true> X; typedef FftPlan<16, 1, false> S; };
+template <> struct PlanOf<512> { typedef FftPlan<16, 2, true> X; typedef FftPlan<16, 2, false> S; };
+
+#define DISPATCH_N(n, CALL)                                  \
+    switch (n) {                                             \
+        case 16:  { constexpr int N_ = 16;  CALL; } break;   \
+        case 32:  { constexpr int N_ = 32;  CALL; } break;   \
+        case 64:  { constexpr int N_ = 64;  CALL; } break;   \
+        case 128: { constexpr int N_ = 128; CALL; } break;   \
+        case 256: { constexpr int N_ = 256; CALL; } break;   \
+        case 512: { constexpr int N_ = 512; CALL; } break;   \
+        default: return (int)cudaErrorInvalidValue;          \
+    }
+
+static const int XTHREADS = 256;   // threads per block of the contiguous-x kernels
+
+template <int N> static int launch_density_fftx(dbec_handle_s* h) {
+    typedef typename PlanOf<N>::X P;
+    constexpr int LP = XTHREADS / P::T;
+    const int npairs = h->ny * h->nz / 2;
+    const int lp = npairs < LP ? npairs : LP;   // tiny grids: fewer pairs than a block holds
+    (void)lp;
+    const size_t sm = (size_t)LP * XLine<P>::SM * sizeof(cd);
+    auto k = k_density_fftx<P, LP>;
+    int rc = set_smem(k, sm);
+    if (rc) return rc;
+    k<<<(npairs + LP - 1) / LP, P::T * LP, sm, h->stream>>>(h->psi, h->spec, h->ax[0].twA, h->ax[0].twN, h->scal,
+                                                            npairs, h->nxhp);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int axis) {
+    typedef typename PlanOf<N>::S P;
+    constexpr int C = DBEC_SPEC_COLS;
+    constexpr int TILES = (P::T * C >= 128) ? 1 : 128 / (P::T * C);
+    long long line_stride, outer_stride, ntiles;
+    int ntx;
+    if (axis == 1) {        // y lines: for each z, columns = kx
+        line_stride = h->nxhp; outer_stride = (long long)h->ny * h->nxhp; ntx = h->nxhp / C;
+        ntiles = (long long)ntx * h->nz;
+    } else {                // z lines: columns = (ky, kx) flattened
+        line_stride = (long long)h->ny * h->nxhp; outer_stride = 0; ntx = (int)(line_stride / C);
+        ntiles = ntx;
+    }
+    const size_t sm = (size_t)TILES * P::SMEM * C * sizeof(cd);
+    auto k = k_fft_strided<P, MODE, TILES>;
+    int rc = set_smem(k, sm);
+    if (rc) return rc;
+    k<<<(unsigned)((ntiles + TILES - 1) / TILES), P::T * C * TILES, sm, h->stream>>>(
+        h->spec, h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, double* phi) {
+    typedef typename PlanOf<N>::X P;
+    constexpr int LP = XTHREADS / P::T;
+    const int npairs = h->ny * h->nz / 2;
+    const size_t sm = (size_t)LP * XLine<P>::SM * sizeof(cd);
+    auto k = k_ifftx_nonlin<P, LP, RT, MODE>;
+    int rc = set_smem(k, sm);
+    if (rc) return rc;
+    k<<<(npairs + LP - 1) / LP, P::T * LP, sm, h->stream>>>(
+        h->spec, h->psi, phi, h->ax[0].twA, h->ax[0].twN, h->scal, h->ax[0].vtrap, h->ax[1].vtrap,
+        h->ax[2].vtrap, h->p.dt, npairs, h->nxhp, h->ny, make_cntab<RT>(h->ax[0]));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_density_fft(dbec_handle_s* h) {
+    int rc;
+    DISPATCH_N(h->nx, rc = launch_density_fftx<N_>(h));
+    if (rc) return rc;
+    if (h->p.ndim == 3) {
+        DISPATCH_N(h->ny, rc = (launch_fft_strided<N_, MODE_FWD>(h, 1)));
+    }
+    return rc;
+}
+
+int dbec_launch_kernel_mul_inverse(dbec_handle_s* h) {
+    int rc;
+    if (h->p.ndim == 3) {
+        DISPATCH_N(h->nz, rc = (launch_fft_strided<N_, MODE_FMI>(h, 2)));
+        if (rc) return rc;
+        DISPATCH_N(h->ny, rc = (launch_fft_strided<N_, MODE_INV>(h, 1)));
+    } else {
+        DISPATCH_N(h->ny, rc = (launch_fft_strided<N_, MODE_FMI>(h, 1)));
+    }
+    return rc;
+}
+
+int dbec_launch_nonlinear(dbec_handle_s* h, int fuse_cnx) {
+    int rc;
+    if (h->p.time_mode == 1) {
+        if (fuse_cnx) { DISPATCH_N(h->nx, rc = (launch_ifftx<N_, true, NL_STEP_CNX>(h, nullptr))); }
+        else          { DISPATCH_N(h->nx, rc = (launch_ifftx<N_, true, NL_STEP>(h, nullptr))); }
+    } else {
+        if (fuse_cnx) { DISPATCH_N(h->nx, rc = (launch_ifftx<N_, false, NL_STEP_CNX>(h, nullptr))); }
+        else          { DISPATCH_N(h->nx, rc = (launch_ifftx<N_, false, NL_STEP>(h, nullptr))); }
+    }
+    return rc;
+}
+
+int dbec_launch_phi_out(dbec_handle_s* h, double* phi) {
+    int rc;
+    DISPATCH_N(h->nx, rc = (launch_ifftx<N_, false, NL_PHI>(h, phi)));
+    return rc;
+}
+
+int dbec_launch_build_vdd(dbec_handle_s* h) {
+    k_build_vdd<<<148 * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->nx, h->ny, h->nz, h->nxhp, h->p.dx, h->p.dy,
+                                                 h->p.dz, h->p.d_perp, h->p.cutoff, 1.0 / (double)h->P);
+    h->launches++;
+    return (int)cudaGetLastError();
+}

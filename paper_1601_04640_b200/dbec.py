@@ -1,0 +1,200 @@
+"""Thin Python binding of libdbec.so (include/dbec.h): argument marshalling only.
+
+torch is used for device memory (the workspace the caller owns) and the CUDA stream; every step of
+the path runs in the library's sm_100a kernels.  There is no CPU fallback: importing works without a
+GPU (so that the symbols can be checked), creating a simulation does not.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdbec.so")
+
+DBEC_OK, DBEC_EINVAL, DBEC_ESIZE, DBEC_EWORKSPACE, DBEC_ECUDA, DBEC_ENODEVICE = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi", "dbec_set_coupling",
+           "dbec_step", "dbec_observables", "dbec_destroy", "dbec_strerror", "dbec_last_cuda_error",
+           "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
+           "dbec_version"]
+
+
+class DbecParams(C.Structure):
+    _fields_ = [("ndim", C.c_int32), ("plane", C.c_int32),
+                ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("dt", C.c_double),
+                ("nu", C.c_double), ("lam", C.c_double), ("kappa", C.c_double),
+                ("G", C.c_double), ("D", C.c_double),
+                ("d_perp", C.c_double), ("cutoff", C.c_double),
+                ("time_mode", C.c_int32)]
+
+
+class DbecObs(C.Structure):
+    _fields_ = [(k, C.c_double) for k in
+                ("norm", "mu", "energy", "rms_x", "rms_y", "rms_z", "rms_r", "density0", "density_max")]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class DbecError(RuntimeError):
+    def __init__(self, code, what, cuda=0):
+        self.code = code
+        self.cuda = cuda
+        msg = lib().dbec_strerror(code).decode()
+        super().__init__(f"{what}: {msg} (code {code}" + (f", CUDA error {cuda})" if cuda else ")"))
+
+
+_lib = None
+
+
+def lib():
+    """Load libdbec.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH) or os.environ.get("DBEC_REBUILD"):
+            _build.build()
+        L = C.CDLL(LIB_PATH)
+        pp, vp = C.POINTER(DbecParams), C.c_void_p
+        L.dbec_workspace_bytes.argtypes = [pp, C.POINTER(C.c_size_t)]
+        L.dbec_create.argtypes = [pp, vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.dbec_set_psi.argtypes = [vp, vp, C.c_int]
+        L.dbec_get_psi.argtypes = [vp, vp, C.c_int]
+        L.dbec_set_coupling.argtypes = [vp, C.c_double, C.c_double]
+        L.dbec_step.argtypes = [vp, C.c_int]
+        L.dbec_observables.argtypes = [vp, C.POINTER(DbecObs)]
+        L.dbec_destroy.argtypes = [vp]
+        L.dbec_strerror.argtypes = [C.c_int]
+        L.dbec_strerror.restype = C.c_char_p
+        L.dbec_last_cuda_error.argtypes = [vp]
+        L.dbec_phi_dd.argtypes = [vp, vp]
+        L.dbec_cn_sweep.argtypes = [vp, C.c_int]
+        L.dbec_nonlinear.argtypes = [vp]
+        L.dbec_normalize.argtypes = [vp]
+        L.dbec_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.dbec_version.argtypes = []
+        _lib = L
+    return _lib
+
+
+def params(ndim, nx, ny, nz, dx, dy, dz, dt, nu, lam, kappa, G, D, time_mode,
+           d_perp=1.0, cutoff=0.0, plane=0) -> DbecParams:
+    return DbecParams(ndim, plane, nx, ny, nz, dx, dy, dz, dt, nu, lam, kappa, G, D, d_perp, cutoff, time_mode)
+
+
+def params_of(w, G=None, D=None) -> DbecParams:
+    """DbecParams from an object with the attribute names of inputs.Workload (duck-typed)."""
+    return params(w.ndim, w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.dt, w.nu, w.lam, w.kappa,
+                  w.G if G is None else G, w.D if D is None else D, w.time_mode,
+                  d_perp=w.d_perp, cutoff=w.cutoff)
+
+
+def workspace_bytes(p: DbecParams) -> int:
+    n = C.c_size_t(0)
+    rc = lib().dbec_workspace_bytes(C.byref(p), C.byref(n))
+    if rc:
+        raise DbecError(rc, "dbec_workspace_bytes")
+    return int(n.value)
+
+
+class Dbec:
+    """One simulation on the current CUDA device.  Methods mirror the C entry points."""
+
+    def __init__(self, p: DbecParams, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1601_04640_b200 needs a CUDA device (sm_100a); there is no CPU path")
+        self._torch = torch
+        self.p = p
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        nbytes = workspace_bytes(p)
+        # caller-owned workspace; torch allocations are 512-byte aligned
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        assert self.workspace.data_ptr() % 256 == 0
+        self._h = C.c_void_p()
+        rc = lib().dbec_create(C.byref(p), C.c_void_p(self.workspace.data_ptr()), nbytes,
+                               C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
+        if rc:
+            raise DbecError(rc, "dbec_create")
+        self.shape = (p.nz, p.ny, p.nx) if p.ndim == 3 else (p.ny, p.nx)
+        self.npoints = p.nx * p.ny * p.nz
+
+    # -- helpers
+    def _ck(self, rc, what):
+        if rc:
+            raise DbecError(rc, what, lib().dbec_last_cuda_error(self._h) if self._h else 0)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().dbec_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ptr(self, a):
+        """(pointer, on_device) of a numpy array or a torch tensor holding npoints complex128."""
+        torch = self._torch
+        if isinstance(a, np.ndarray):
+            assert a.dtype == np.complex128 and a.flags.c_contiguous and a.size == self.npoints
+            return a.ctypes.data, 0
+        assert a.dtype == torch.complex128 and a.is_contiguous() and a.numel() == self.npoints
+        return a.data_ptr(), 1 if a.is_cuda else 0
+
+    # -- C entry points
+    def set_psi(self, psi):
+        if isinstance(psi, np.ndarray):
+            psi = np.ascontiguousarray(psi, dtype=np.complex128)
+        ptr, dev = self._ptr(psi)
+        self._ck(lib().dbec_set_psi(self._h, C.c_void_p(ptr), dev), "dbec_set_psi")
+
+    def get_psi(self, out=None):
+        if out is None:
+            out = np.empty(self.shape, dtype=np.complex128)
+        ptr, dev = self._ptr(out)
+        self._ck(lib().dbec_get_psi(self._h, C.c_void_p(ptr), dev), "dbec_get_psi")
+        return out
+
+    def set_coupling(self, G, D):
+        self._ck(lib().dbec_set_coupling(self._h, float(G), float(D)), "dbec_set_coupling")
+
+    def step(self, n=1):
+        self._ck(lib().dbec_step(self._h, int(n)), "dbec_step")
+
+    def observables(self) -> dict:
+        o = DbecObs()
+        self._ck(lib().dbec_observables(self._h, C.byref(o)), "dbec_observables")
+        return o.as_dict()
+
+    def phi_dd(self):
+        out = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)
+        self._ck(lib().dbec_phi_dd(self._h, C.c_void_p(out.data_ptr())), "dbec_phi_dd")
+        return out
+
+    def cn_sweep(self, axis):
+        self._ck(lib().dbec_cn_sweep(self._h, int(axis)), "dbec_cn_sweep")
+
+    def nonlinear(self):
+        self._ck(lib().dbec_nonlinear(self._h), "dbec_nonlinear")
+
+    def normalize(self):
+        self._ck(lib().dbec_normalize(self._h), "dbec_normalize")
+
+    def launch_count(self) -> int:
+        n = C.c_longlong(0)
+        self._ck(lib().dbec_launch_count(self._h, C.byref(n)), "dbec_launch_count")
+        return int(n.value)
+
+    def synchronize(self):
+        self.stream.synchronize()

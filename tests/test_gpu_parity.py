@@ -1,0 +1,223 @@
+"""GPU parity: the CUDA path (through the C ABI of include/dbec.h) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances: BASELINE.json `north_star` — psi after one step
+within 1e-12 relative max-abs; mu, energy, rms within 1e-9 relative.  Single parts use the same
+1e-12 bar.
+"""
+import numpy as np
+import pytest
+
+from paper_1601_04640_b200.inputs import IMAG, REAL, Workload, initial_psi, random_psi, workload
+
+pytestmark = pytest.mark.gpu
+
+PSI_TOL = 1e-12
+OBS_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def gp():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1601_04640_b200 import dbec
+    dbec.lib()
+    return dbec
+
+
+def relerr(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def grid3(nx, ny, nz, mode, G=30.0, D=20.0, dx=0.4, dt=None, trap=(1.0, 1.2, 0.7), cutoff=0.0, d=None):
+    d = d or (dx, dx, dx)
+    dt = dt if dt is not None else (0.1 if mode == IMAG else 0.5) * d[0] ** 2
+    return Workload("t3", 3, nx, ny, nz, d[0], d[1], d[2], dt, *trap, G, D, G, D, mode, 1, 21, 1, cutoff=cutoff)
+
+
+def grid2(nx, ny, mode, G=20.0, D=15.0, dx=0.2, dt=None, trap=(1.0, 1.5, 0.0)):
+    dt = dt if dt is not None else (0.1 if mode == IMAG else 0.5) * dx ** 2
+    return Workload("t2", 2, nx, ny, 1, dx, dx, 1.0, dt, *trap, G, D, G, D, mode, 1, 22, 1)
+
+
+SHAPES3 = [(16, 16, 16), (32, 32, 32), (64, 16, 32), (16, 64, 128), (128, 32, 16), (256, 16, 16), (16, 256, 32),
+           (32, 16, 512), (512, 32, 16)]
+SHAPES2 = [(16, 16), (32, 64), (128, 32), (512, 16), (16, 512), (256, 256)]
+
+
+def all_small_workloads():
+    out = []
+    for mode in (IMAG, REAL):
+        for s in SHAPES3:
+            out.append(grid3(*s, mode))
+        for s in SHAPES2:
+            out.append(grid2(*s, mode))
+    return out
+
+
+def wid(w):
+    return f"{w.ndim}d-{w.nx}x{w.ny}x{w.nz}-{'imag' if w.time_mode == IMAG else 'real'}"
+
+
+@pytest.mark.parametrize("w", all_small_workloads(), ids=wid)
+def test_cn_sweeps_match_oracle(gp, ob, w):
+    psi0 = random_psi(w, 5)
+    sim = gp.Dbec(gp.params_of(w))
+    for axis in range(w.ndim):
+        sim.set_psi(psi0)
+        sim.cn_sweep(axis)
+        got = sim.get_psi()
+        ref = ob.cn_sweep(ob.params_of(w), psi0, axis)
+        assert relerr(got, ref) < PSI_TOL, f"axis {axis}"
+    sim.close()
+
+
+@pytest.mark.parametrize("w", all_small_workloads()[::2] + [grid3(32, 32, 32, IMAG, cutoff=5.0)], ids=wid)
+def test_phi_dd_matches_oracle(gp, ob, w):
+    psi0 = random_psi(w, 6)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    got = sim.phi_dd().cpu().numpy()
+    ref = ob.phi_dd(ob.params_of(w), np.abs(psi0) ** 2)
+    assert relerr(got, ref) < PSI_TOL
+    sim.close()
+
+
+@pytest.mark.parametrize("w", all_small_workloads()[1::3], ids=wid)
+def test_nonlinear_matches_oracle(gp, ob, w):
+    psi0 = random_psi(w, 7)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    sim.nonlinear()
+    got = sim.get_psi()
+    p = ob.params_of(w)
+    ref = ob.nonlinear(p, psi0, ob.phi_dd(p, np.abs(psi0) ** 2))
+    assert relerr(got, ref) < PSI_TOL
+    sim.close()
+
+
+def test_normalize_matches_oracle(gp, ob):
+    w = grid3(32, 16, 64, IMAG)
+    psi0 = 1.7 * random_psi(w, 8)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    sim.normalize()
+    got = sim.get_psi()
+    ref = ob.normalize(ob.params_of(w), psi0)
+    assert relerr(got, ref) < PSI_TOL
+    assert abs(sim.observables()["norm"] - 1.0) < 1e-13
+    sim.close()
+
+
+def one_step_pair(gp, ob, w, psi0, steps=1):
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    if (w.G_run, w.D_run) != (w.G, w.D):
+        sim.set_coupling(w.G_run, w.D_run)
+    sim.step(steps)
+    got = sim.get_psi()
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(psi0)
+    if (w.G_run, w.D_run) != (w.G, w.D):
+        o.set_coupling(w.G_run, w.D_run)
+    o.step(steps)
+    ref = o.get_psi()
+    return sim, o, got, ref
+
+
+@pytest.mark.parametrize("w", all_small_workloads(), ids=wid)
+def test_one_step_small_grids(gp, ob, w):
+    psi0 = random_psi(w, 9) if w.time_mode == REAL else initial_psi(w)
+    sim, o, got, ref = one_step_pair(gp, ob, w, psi0)
+    assert relerr(got, ref) < PSI_TOL
+    a, b = sim.observables(), o.observables()
+    for k in b:
+        if w.ndim == 2 and k == "rms_z":
+            continue
+        assert abs(a[k] - b[k]) <= OBS_TOL * max(abs(b[k]), 1e-300), k
+    sim.close()
+    o.close()
+
+
+@pytest.mark.parametrize("key", ["C1", "C2", "C3", "C4"])
+def test_one_step_baseline_configs(gp, ob, key):
+    """Full-size BASELINE.json configs, one step, every grid point compared."""
+    w = workload(key)
+    psi0 = initial_psi(w)
+    sim, o, got, ref = one_step_pair(gp, ob, w, psi0)
+    assert relerr(got, ref) < PSI_TOL
+    a, b = sim.observables(), o.observables()
+    for k in ("norm", "mu", "energy", "rms_x", "rms_y", "rms_z", "rms_r", "density0", "density_max"):
+        if w.ndim == 2 and k == "rms_z":
+            continue
+        assert abs(a[k] - b[k]) <= OBS_TOL * abs(b[k]), k
+    sim.close()
+    o.close()
+
+
+def test_fused_and_unfused_x_sweep_agree(gp, monkeypatch):
+    w = workload("C1")
+    psi0 = initial_psi(w)
+    outs = []
+    for fuse in ("1", "0"):
+        monkeypatch.setenv("DBEC_FUSE_CNX", fuse)
+        sim = gp.Dbec(gp.params_of(w))
+        sim.set_psi(psi0)
+        sim.step(3)
+        outs.append(sim.get_psi())
+        sim.close()
+    assert relerr(outs[0], outs[1]) < PSI_TOL
+
+
+def test_graph_and_plain_launches_agree_bitwise(gp, monkeypatch):
+    w = workload("C1")
+    psi0 = initial_psi(w)
+    outs = []
+    for g in ("1", "0"):
+        monkeypatch.setenv("DBEC_GRAPH", g)
+        sim = gp.Dbec(gp.params_of(w))
+        sim.set_psi(psi0)
+        sim.step(5)
+        outs.append(sim.get_psi())
+        sim.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_full_run_C1_observables(gp, ob):
+    w = workload("C1")
+    psi0 = initial_psi(w)
+    sim, o, got, ref = one_step_pair(gp, ob, w, psi0, steps=w.steps)
+    assert relerr(got, ref) < 1e-10
+    a, b = sim.observables(), o.observables()
+    for k in ("norm", "mu", "energy", "rms_x", "rms_y", "rms_z", "rms_r", "density0"):
+        assert abs(a[k] - b[k]) <= OBS_TOL * abs(b[k]), k
+    sim.close()
+    o.close()
+
+
+def test_real_time_norm_conserved_on_gpu(gp):
+    w = workload("C2")
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(initial_psi(w))
+    sim.set_coupling(w.G_run, w.D_run)
+    sim.step(100)
+    assert abs(sim.observables()["norm"] - 1.0) < 1e-12
+    sim.close()
+
+
+def test_errors_and_edge_cases(gp):
+    import ctypes as C
+    L = gp.lib()
+    p = gp.params(3, 48, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0)
+    n = C.c_size_t()
+    assert L.dbec_workspace_bytes(C.byref(p), C.byref(n)) == gp.DBEC_ESIZE
+    p = gp.params(3, 32, 32, 32, .5, .5, .5, -1.0, 1, 1, .5, 1, 1, 0)
+    assert L.dbec_workspace_bytes(C.byref(p), C.byref(n)) == gp.DBEC_EINVAL
+    p = gp.params(3, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0)
+    h = C.c_void_p()
+    assert L.dbec_create(C.byref(p), None, 0, None, C.byref(h)) == gp.DBEC_EWORKSPACE
+    assert L.dbec_step(None, 1) == gp.DBEC_EINVAL
+    sim = gp.Dbec(p)
+    assert L.dbec_step(sim._h, -1) == gp.DBEC_EINVAL
+    sim.step(0)                      # zero steps: nothing happens
+    assert np.all(sim.get_psi() == 0)
+    assert sim.launch_count() >= 1
+    sim.close()
