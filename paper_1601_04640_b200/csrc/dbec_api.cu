@@ -219,6 +219,8 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->fuse_cnx = fe ? atoi(fe) : 1;
     const char* ge = getenv("DBEC_GRAPH");
     h->use_graph = ge ? atoi(ge) : 1;
+    // the legacy default stream cannot be captured: plain launches there
+    if (h->stream == nullptr || h->stream == cudaStreamLegacy) h->use_graph = 0;
 
 #define FAIL(code) do { delete h; return (code); } while (0)
     if (cudaMemsetAsync(h->psi, 0, sizeof(cd) * h->P, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);

@@ -92,15 +92,17 @@ __device__ __forceinline__ void norm_finish(double part, double* __restrict__ pa
 // ------------------------------------------------------------------------------------------------
 template <bool RT, int NCH, int COLS, bool NORM>
 __global__ void __launch_bounds__(NCH* COLS)
-k_cn_strided(cd* __restrict__ psi, CnTab<RT> cn, long long line_stride, long long outer_stride,
+k_cn_strided(cd* __restrict__ psi, CnTab<RT> cn, long long line_stride, long long outer_stride, long long ncols,
              double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV) {
     typedef typename CnCoef<RT>::type CT;
     __shared__ cd edge[2][NCH][COLS];     // first and last point of every chunk (halo of the neighbours)
     __shared__ cd ends[2][NCH][COLS];     // zero-start chunk results for the carries
     __shared__ double red[32];
     const int col = threadIdx.x % COLS, c = threadIdx.x / COLS;
-    cd* g = psi + (long long)blockIdx.y * outer_stride + (long long)blockIdx.x * COLS + col +
-            (long long)(c * CN_L) * line_stride;
+    long long gcol = (long long)blockIdx.x * COLS + col;
+    const bool active = gcol < ncols;          // narrow grids: a tile may be wider than the grid
+    if (!active) gcol = 0;
+    cd* g = psi + (long long)blockIdx.y * outer_stride + gcol + (long long)(c * CN_L) * line_stride;
     cd u[CN_L];
 #pragma unroll
     for (int i = 0; i < CN_L; ++i) u[i] = g[i * line_stride];
@@ -129,8 +131,10 @@ k_cn_strided(cd* __restrict__ psi, CnTab<RT> cn, long long line_stride, long lon
     double acc = 0.0;
 #pragma unroll
     for (int i = 0; i < CN_L; ++i) {
-        g[i * line_stride] = u[i];
-        if (NORM) acc += cnorm2(u[i]);
+        if (active) {
+            g[i * line_stride] = u[i];
+            if (NORM) acc += cnorm2(u[i]);
+        }
     }
     if (NORM) {
         const double part = block_sum<NCH * COLS>(acc, red);
@@ -271,12 +275,10 @@ template <bool RT, int NCH, bool NORM> static int launch_cn_strided(dbec_handle_
     int nouter;
     if (axis == 1) { line_stride = h->nx; outer_stride = (long long)h->nx * h->ny; ncols = h->nx; nouter = h->nz; }
     else { line_stride = (long long)h->nx * h->ny; outer_stride = 0; ncols = line_stride; nouter = 1; }
-    // COLS must divide the column count: nx >= 16 and for z: nx*ny >= 256
-    if (ncols % COLS) return (int)cudaErrorInvalidValue;
-    dim3 grid((unsigned)(ncols / COLS), (unsigned)nouter);
+    dim3 grid((unsigned)((ncols + COLS - 1) / COLS), (unsigned)nouter);
     if (NORM && (long long)grid.x * grid.y > h->npartial) return (int)cudaErrorInvalidValue;
     k_cn_strided<RT, NCH, COLS, NORM><<<grid, NCH * COLS, 0, h->stream>>>(
-        h->psi, make_cntab<RT>(h->ax[axis]), line_stride, outer_stride, h->partial, h->ticket, h->scal, h->dV);
+        h->psi, make_cntab<RT>(h->ax[axis]), line_stride, outer_stride, ncols, h->partial, h->ticket, h->scal, h->dV);
     h->launches++;
     return (int)cudaGetLastError();
 }

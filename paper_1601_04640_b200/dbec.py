@@ -114,7 +114,9 @@ class Dbec:
         self.p = p
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        # a stream of its own by default: the step is replayed as a CUDA graph, which the legacy default
+        # stream cannot capture
+        self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
         nbytes = workspace_bytes(p)
         # caller-owned workspace; torch allocations are 512-byte aligned
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
@@ -157,13 +159,19 @@ class Dbec:
         if isinstance(psi, np.ndarray):
             psi = np.ascontiguousarray(psi, dtype=np.complex128)
         ptr, dev = self._ptr(psi)
+        if dev:
+            self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
         self._ck(lib().dbec_set_psi(self._h, C.c_void_p(ptr), dev), "dbec_set_psi")
 
     def get_psi(self, out=None):
         if out is None:
             out = np.empty(self.shape, dtype=np.complex128)
         ptr, dev = self._ptr(out)
+        if dev:
+            self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
         self._ck(lib().dbec_get_psi(self._h, C.c_void_p(ptr), dev), "dbec_get_psi")
+        if dev:
+            self._torch.cuda.current_stream(self.device).wait_stream(self.stream)
         return out
 
     def set_coupling(self, G, D):
@@ -179,7 +187,9 @@ class Dbec:
 
     def phi_dd(self):
         out = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)
+        self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
         self._ck(lib().dbec_phi_dd(self._h, C.c_void_p(out.data_ptr())), "dbec_phi_dd")
+        self._torch.cuda.current_stream(self.device).wait_stream(self.stream)
         return out
 
     def cn_sweep(self, axis):
