@@ -115,7 +115,14 @@ int dbec_normalize(dbec_handle h);
 /* Number of kernel launches the library has enqueued on this handle since creation. */
 int dbec_launch_count(dbec_handle h, long long* launches);
 
-/* Name and launch count of the i-th distinct kernel (for bench.py's gpu_launches claim). */
+/* Measurement aid (bench.py's roofline leg): nsteps steps with plain launches and a CUDA event pair
+ * around every kernel.  ms_per_slot: HOST pointer to DBEC_KERNEL_SLOTS doubles receiving the total
+ * milliseconds spent in each kernel slot over the nsteps steps; launches_per_slot: HOST pointer to
+ * DBEC_KERNEL_SLOTS counts.  Synchronises the stream.  Slot names from dbec_kernel_name. */
+#define DBEC_KERNEL_SLOTS 8
+int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long* launches_per_slot);
+const char* dbec_kernel_name(int slot);
+
 int dbec_version(void);
 
 #ifdef __cplusplus

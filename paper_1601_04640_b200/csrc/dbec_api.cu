@@ -142,15 +142,46 @@ static int write_scalars(dbec_handle h, bool reset_scale) {
     return DBEC_OK;
 }
 
+// Kernel slots of one step (dbec_step_profile / dbec_kernel_name).
+enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z };
+static const char* const kernel_names[DBEC_MAX_KERNELS] = {
+    "k_density_fftx", "k_fft_strided<y,fwd>", "k_fft_strided<last,fwd*Vdd*inv>", "k_fft_strided<y,inv>",
+    "k_ifftx_nonlin", "k_cn_x", "k_cn_strided<y>", "k_cn_strided<z>"};
+
+#define KLAUNCH(h, slot, x)                                                                      \
+    do {                                                                                         \
+        if ((h)->prof_on) cudaEventRecord((h)->prof_ev[2 * (h)->prof_n], (h)->stream);           \
+        int rc_ = (x);                                                                           \
+        if (rc_) return cuda_fail(h, (cudaError_t)rc_);                                          \
+        if ((h)->prof_on) {                                                                      \
+            cudaEventRecord((h)->prof_ev[2 * (h)->prof_n + 1], (h)->stream);                     \
+            (h)->prof_slot[(h)->prof_n++] = (slot);                                              \
+        }                                                                                        \
+    } while (0)
+
+// calcpsidd2 up to the x-inverse: density -> half spectrum -> x V_dd -> back along z, y.
+static int enqueue_dipolar_spectrum(dbec_handle h) {
+    KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
+    if (h->p.ndim == 3) {
+        KLAUNCH(h, KS_FFT_Y_FWD, dbec_launch_fft_strided(h, 1, 0));
+        KLAUNCH(h, KS_FFT_LAST_FMI, dbec_launch_fft_strided(h, 2, 2));
+        KLAUNCH(h, KS_FFT_Y_INV, dbec_launch_fft_strided(h, 1, 1));
+    } else {
+        KLAUNCH(h, KS_FFT_LAST_FMI, dbec_launch_fft_strided(h, 1, 2));
+    }
+    return DBEC_OK;
+}
+
 // One SSCN step as a sequence of launches (reading S10).
 static int enqueue_step(dbec_handle h) {
     const bool imag = h->p.time_mode == 0;
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
-    LAUNCH(h, dbec_launch_density_fft(h));
-    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
-    LAUNCH(h, dbec_launch_nonlinear(h, h->fuse_cnx));
-    if (!h->fuse_cnx) LAUNCH(h, dbec_launch_cn(h, 0, 0));
-    for (int ax = 1; ax <= last_axis; ++ax) LAUNCH(h, dbec_launch_cn(h, ax, imag && ax == last_axis));
+    int rc = enqueue_dipolar_spectrum(h);
+    if (rc) return rc;
+    KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
+    if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, dbec_launch_cn(h, 0, 0));
+    for (int ax = 1; ax <= last_axis; ++ax)
+        KLAUNCH(h, ax == 1 ? KS_CN_Y : KS_CN_Z, dbec_launch_cn(h, ax, imag && ax == last_axis));
     return DBEC_OK;
 }
 
@@ -314,8 +345,7 @@ int dbec_step(dbec_handle h, int nsteps) {
 
 int dbec_phi_dd(dbec_handle h, void* phi_f64_dev) {
     if (!h || !phi_f64_dev) return DBEC_EINVAL;
-    LAUNCH(h, dbec_launch_density_fft(h));
-    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
     LAUNCH(h, dbec_launch_phi_out(h, (double*)phi_f64_dev));
     return DBEC_OK;
 }
@@ -328,8 +358,7 @@ int dbec_cn_sweep(dbec_handle h, int axis) {
 
 int dbec_nonlinear(dbec_handle h) {
     if (!h) return DBEC_EINVAL;
-    LAUNCH(h, dbec_launch_density_fft(h));
-    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
     LAUNCH(h, dbec_launch_nonlinear(h, 0));
     return DBEC_OK;
 }
@@ -342,8 +371,7 @@ int dbec_normalize(dbec_handle h) {
 
 int dbec_observables(dbec_handle h, dbec_obs* out) {
     if (!h || !out) return DBEC_EINVAL;
-    LAUNCH(h, dbec_launch_density_fft(h));
-    LAUNCH(h, dbec_launch_kernel_mul_inverse(h));
+    { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
     LAUNCH(h, dbec_launch_phi_out(h, h->phi));
     LAUNCH(h, dbec_launch_observables(h));
     double v[16];
@@ -353,6 +381,35 @@ int dbec_observables(dbec_handle h, dbec_obs* out) {
     out->rms_x = v[3]; out->rms_y = v[4]; out->rms_z = v[5]; out->rms_r = v[6];
     out->density0 = v[7]; out->density_max = v[8];
     return DBEC_OK;
+}
+
+// nsteps steps with plain launches and a CUDA event pair around every kernel.  ms_per_slot receives
+// DBEC_MAX_KERNELS doubles: total milliseconds spent in each kernel slot over the nsteps steps;
+// launches_per_slot the launch counts.  Synchronises the stream.
+int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long* launches_per_slot) {
+    if (!h || nsteps < 0 || !ms_per_slot || !launches_per_slot) return DBEC_EINVAL;
+    for (int i = 0; i < DBEC_MAX_KERNELS; ++i) { ms_per_slot[i] = 0.0; launches_per_slot[i] = 0; }
+    for (int i = 0; i < 2 * DBEC_MAX_KERNELS; ++i) CU(h, cudaEventCreate(&h->prof_ev[i]));
+    int rc = DBEC_OK;
+    for (int s = 0; s < nsteps && rc == DBEC_OK; ++s) {
+        h->prof_on = 1; h->prof_n = 0;
+        rc = enqueue_step(h);
+        h->prof_on = 0;
+        if (rc) break;
+        if (cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = DBEC_ECUDA; break; }
+        for (int k = 0; k < h->prof_n; ++k) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, h->prof_ev[2 * k], h->prof_ev[2 * k + 1]);
+            ms_per_slot[h->prof_slot[k]] += ms;
+            launches_per_slot[h->prof_slot[k]] += 1;
+        }
+    }
+    for (int i = 0; i < 2 * DBEC_MAX_KERNELS; ++i) cudaEventDestroy(h->prof_ev[i]);
+    return rc;
+}
+
+const char* dbec_kernel_name(int slot) {
+    return (slot >= 0 && slot < DBEC_MAX_KERNELS) ? kernel_names[slot] : "";
 }
 
 int dbec_launch_count(dbec_handle h, long long* launches) {

@@ -8,6 +8,7 @@
 #include "cplx.cuh"
 
 #define DBEC_MAX_N 512          // longest supported grid line (16 values per thread x 32 lanes)
+#define DBEC_MAX_KERNELS 8      // kernels in one step (slots of dbec_step_profile)
 #define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
 
 // Device scalars every kernel reads (so that a captured CUDA graph never bakes them in).
@@ -56,13 +57,18 @@ struct dbec_handle_s {
     // CUDA graph of one step
     cudaGraphExec_t graph_exec;
     int launches_per_step;
+    // per-kernel timing (dbec_step_profile): event pairs around every launch of a step
+    int prof_on, prof_n;
+    cudaEvent_t prof_ev[2 * DBEC_MAX_KERNELS];
+    int prof_slot[DBEC_MAX_KERNELS];
     int use_graph;                  // env DBEC_GRAPH (default 1): replay one captured step per dbec_step iteration
     int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
 };
 
 // ---- launchers (each returns a cudaError_t as int; all asynchronous on h->stream) ----
-int dbec_launch_density_fft(dbec_handle_s* h);             // a1: psi -> spec (forward transforms done, all axes)
-int dbec_launch_kernel_mul_inverse(dbec_handle_s* h);      // a2 + inverse transforms except x (fused with the last forward)
+int dbec_launch_density_fftx(dbec_handle_s* h);            // a1, x axis: psi -> half spectrum
+int dbec_launch_fft_strided(dbec_handle_s* h, int axis, int mode);   // a1/a3 along y or z; mode 0 forward, 1 inverse,
+                                                           // 2 forward * V_dd(k)/P * inverse (a2 fused)
 int dbec_launch_nonlinear(dbec_handle_s* h, int fuse_cnx); // a3 (x, C2R) + a4 [+ a5]
 int dbec_launch_phi_out(dbec_handle_s* h, double* phi);    // a3 writing Phi_dd only
 int dbec_launch_cn(dbec_handle_s* h, int axis, int with_norm);   // a5..a7 (+ a8 partial sums and factor)

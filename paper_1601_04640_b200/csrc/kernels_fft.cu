@@ -340,25 +340,19 @@ template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, do
     return (int)cudaGetLastError();
 }
 
-int dbec_launch_density_fft(dbec_handle_s* h) {
+int dbec_launch_density_fftx(dbec_handle_s* h) {
     int rc;
     DISPATCH_N(h->nx, rc = launch_density_fftx<N_>(h));
-    if (rc) return rc;
-    if (h->p.ndim == 3) {
-        DISPATCH_N(h->ny, rc = (launch_fft_strided<N_, MODE_FWD>(h, 1)));
-    }
     return rc;
 }
 
-int dbec_launch_kernel_mul_inverse(dbec_handle_s* h) {
+// mode: 0 forward, 1 inverse, 2 forward * V_dd * inverse; axis 1 (y) or 2 (z)
+int dbec_launch_fft_strided(dbec_handle_s* h, int axis, int mode) {
     int rc;
-    if (h->p.ndim == 3) {
-        DISPATCH_N(h->nz, rc = (launch_fft_strided<N_, MODE_FMI>(h, 2)));
-        if (rc) return rc;
-        DISPATCH_N(h->ny, rc = (launch_fft_strided<N_, MODE_INV>(h, 1)));
-    } else {
-        DISPATCH_N(h->ny, rc = (launch_fft_strided<N_, MODE_FMI>(h, 1)));
-    }
+    const int n = axis == 1 ? h->ny : h->nz;
+    if (mode == MODE_FWD) { DISPATCH_N(n, rc = (launch_fft_strided<N_, MODE_FWD>(h, axis))); }
+    else if (mode == MODE_INV) { DISPATCH_N(n, rc = (launch_fft_strided<N_, MODE_INV>(h, axis))); }
+    else { DISPATCH_N(n, rc = (launch_fft_strided<N_, MODE_FMI>(h, axis))); }
     return rc;
 }
 

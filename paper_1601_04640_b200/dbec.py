@@ -21,7 +21,8 @@ DBEC_OK, DBEC_EINVAL, DBEC_ESIZE, DBEC_EWORKSPACE, DBEC_ECUDA, DBEC_ENODEVICE = 
 EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi", "dbec_set_coupling",
            "dbec_step", "dbec_observables", "dbec_destroy", "dbec_strerror", "dbec_last_cuda_error",
            "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
-           "dbec_version"]
+           "dbec_version", "dbec_step_profile", "dbec_kernel_name"]
+KERNEL_SLOTS = 8
 
 
 class DbecParams(C.Structure):
@@ -79,6 +80,9 @@ def lib():
         L.dbec_normalize.argtypes = [vp]
         L.dbec_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.dbec_version.argtypes = []
+        L.dbec_step_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.dbec_kernel_name.argtypes = [C.c_int]
+        L.dbec_kernel_name.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -205,6 +209,13 @@ class Dbec:
         n = C.c_longlong(0)
         self._ck(lib().dbec_launch_count(self._h, C.byref(n)), "dbec_launch_count")
         return int(n.value)
+
+    def step_profile(self, n=1) -> dict:
+        """{kernel name: (total ms, launches)} over n steps, CUDA events around every launch."""
+        ms = (C.c_double * KERNEL_SLOTS)()
+        cnt = (C.c_longlong * KERNEL_SLOTS)()
+        self._ck(lib().dbec_step_profile(self._h, int(n), ms, cnt), "dbec_step_profile")
+        return {lib().dbec_kernel_name(i).decode(): (ms[i], cnt[i]) for i in range(KERNEL_SLOTS) if cnt[i]}
 
     def synchronize(self):
         self.stream.synchronize()
