@@ -91,7 +91,7 @@ __device__ __forceinline__ void norm_finish(double part, double* __restrict__ pa
 // strided sweeps
 // ------------------------------------------------------------------------------------------------
 template <bool RT, int NCH, int COLS, bool NORM>
-__global__ void __launch_bounds__(NCH* COLS)
+__global__ void __launch_bounds__(NCH* COLS, (NCH * COLS <= 256 ? 2 : 1))
 k_cn_strided(cd* __restrict__ psi, CnTab<RT> cn, long long line_stride, long long outer_stride, long long ncols,
              double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV) {
     typedef typename CnCoef<RT>::type CT;
@@ -151,17 +151,20 @@ k_cn_x(cd* __restrict__ psi, CnTab<RT> cn, int nlines, double* __restrict__ part
        double* __restrict__ scal, double dV) {
     extern __shared__ cd smem[];
     __shared__ double red[32];
+    typedef typename CnCoef<RT>::type CT;
     constexpr int N = 16 * T;
     const int lp = threadIdx.x / T, m = threadIdx.x % T;
     long long line = (long long)blockIdx.x * LPB + lp;
     const bool active = line < nlines;
     if (!active) line = 0;
-    cd* sm = smem + lp * (N + 3 * T);
+    const CnTab<RT> cs = cn_stage_tables<RT, N>(cn, (CT*)smem);
+    cd* sm = smem + (3 * cn_tab_elems(N) * sizeof(CT)) / sizeof(cd) + lp * (N + 3 * T);
     cd* g = psi + line * N;
     cd q[16];
 #pragma unroll
     for (int j = 0; j < 16; ++j) q[j] = g[j * T + m];
-    cn_line_via_smem<RT, T>(q, m, sm, cn);
+    __syncthreads();
+    cn_line_via_smem<RT, T, 17>(q, m, sm, cs);
     double acc = 0.0;
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
@@ -286,7 +289,8 @@ template <bool RT, int NCH, bool NORM> static int launch_cn_strided(dbec_handle_
 template <bool RT, int NCH, bool NORM> static int launch_cn_x(dbec_handle_s* h) {
     constexpr int T = NCH, LPB = 256 / T;
     const int nlines = h->ny * h->nz;
-    const size_t sm = (size_t)LPB * (16 * T + 3 * T) * sizeof(cd);
+    const size_t sm = (size_t)LPB * (16 * T + 3 * T) * sizeof(cd) +
+                      3 * cn_tab_elems(16 * T) * sizeof(typename CnCoef<RT>::type);
     auto k = k_cn_x<RT, T, LPB, NORM>;
     if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const int nb = (nlines + LPB - 1) / LPB;

@@ -138,12 +138,18 @@ k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __rest
                const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
                double dt, int npairs, int nxhp, int ny, CnTab<RT> cn) {
     extern __shared__ cd smem[];
+    typedef typename CnCoef<RT>::type CT;
     constexpr int T = P::T, N = P::N;
     const int lp = threadIdx.x / T, m = threadIdx.x % T;
     long long pair = (long long)blockIdx.x * LP + lp;
     const bool active = pair < npairs;
     if (!active) pair = 0;
+    CnTab<RT> cs = cn;
     cd* sm = smem + lp * XLine<P>::SM;
+    if (MODE == NL_STEP_CNX) {
+        cs = cn_stage_tables<RT, N>(cn, (CT*)smem);
+        sm += (3 * cn_tab_elems(N) * sizeof(CT)) / sizeof(cd);
+    }
     const cd* sa = spec + pair * 2 * nxhp;
     const cd* sb = sa + nxhp;
     cd v[16];
@@ -158,6 +164,7 @@ k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __rest
             v[j] = cmake(a.x + b.y, b.x - a.y);          // conj X_a + i conj X_b
         }
     }
+    if (MODE == NL_STEP_CNX) __syncthreads();            // staged tables visible
     fft_line<P, +1, 0>(v, m, sm, 1, twA, twN);
     // v[j] = (Phi_dd on line y, Phi_dd on line y+1) at x = j*T + m   (1/P is inside the V_dd table)
     if (MODE == NL_PHI) {
@@ -172,45 +179,34 @@ k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __rest
     const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
     const long long row = pair * 2;
     const int y = (int)(row % ny), z = (int)(row / ny);
-    const double va = vy[y] + vz[z], vb = vy[y + 1] + vz[z];
-    cd* pa = psi + row * N;
-    cd* pb = pa + N;
-    cd qa[16];
+    const double vzz = vz[z];
+    if (MODE == NL_STEP_CNX) __syncwarp();               // FFT exchange rows are reused by the sweep
 #pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        const int k = j * T + m;
-        const double vxk = vx[k];
-        cd a = pa[k], b = pb[k];
-        const double ua = dt * (vxk + va + G * (s2 * cnorm2(a)) + D * v[j].x);
-        const double ub = dt * (vxk + vb + G * (s2 * cnorm2(b)) + D * v[j].y);
-        if (RT) {
-            double sn, cs;
-            sincos(ua, &sn, &cs);
-            qa[j] = cmul(s, cmul(a, cmake(cs, -sn)));
-            sincos(ub, &sn, &cs);
-            v[j] = cmul(s, cmul(b, cmake(cs, -sn)));
-        } else {
-            qa[j] = cmul(s * exp(-ua), a);
-            v[j] = cmul(s * exp(-ub), b);
+    for (int l = 0; l < 2; ++l) {
+        cd* p = psi + (row + l) * N;
+        const double vrow = vy[y + l] + vzz;
+        cd q[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) q[j] = p[j * T + m];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const double phi = l == 0 ? v[j].x : v[j].y;
+            const double u = dt * (vx[j * T + m] + vrow + G * (s2 * cnorm2(q[j])) + D * phi);
+            if (RT) {
+                double sn, cs_;
+                sincos(u, &sn, &cs_);
+                q[j] = cmul(s, cmul(q[j], cmake(cs_, -sn)));
+            } else {
+                q[j] = cmul(s * exp(-u), q[j]);
+            }
         }
-    }
-    if (MODE == NL_STEP) {
+        if (MODE == NL_STEP_CNX) {
+            cn_line_via_smem<RT, T, 17>(q, m, sm, cs);
+            __syncwarp();
+        }
         if (active) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) { pa[j * T + m] = qa[j]; pb[j * T + m] = v[j]; }
-        }
-    } else {
-        __syncwarp();
-        cn_line_via_smem<RT, T>(qa, m, sm, cn);
-        if (active) {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) pa[j * T + m] = qa[j];
-        }
-        __syncwarp();
-        cn_line_via_smem<RT, T>(v, m, sm, cn);
-        if (active) {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) pb[j * T + m] = v[j];
+            for (int j = 0; j < 16; ++j) p[j * T + m] = q[j];
         }
     }
 }
@@ -284,7 +280,8 @@ template <> struct PlanOf<512> { typedef FftPlan<16, 2, true> X; typedef FftPlan
         default: return (int)cudaErrorInvalidValue;          \
     }
 
-static const int XTHREADS = 256;   // threads per block of the contiguous-x kernels
+static const int XTHREADS = 256;   // threads per block of k_density_fftx
+static const int NLTHREADS = 128;  // threads per block of k_ifftx_nonlin
 
 template <int N> static int launch_density_fftx(dbec_handle_s* h) {
     typedef typename PlanOf<N>::X P;
@@ -327,9 +324,10 @@ template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int a
 
 template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, double* phi) {
     typedef typename PlanOf<N>::X P;
-    constexpr int LP = XTHREADS / P::T;
+    constexpr int LP = NLTHREADS / P::T;
     const int npairs = h->ny * h->nz / 2;
-    const size_t sm = (size_t)LP * XLine<P>::SM * sizeof(cd);
+    const size_t sm = (size_t)LP * XLine<P>::SM * sizeof(cd) +
+                      (MODE == NL_STEP_CNX ? 3 * cn_tab_elems(N) * sizeof(typename CnCoef<RT>::type) : 0);
     auto k = k_ifftx_nonlin<P, LP, RT, MODE>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
