@@ -39,6 +39,7 @@ template <class P> struct XLine {
     // shared elements per line pair of the contiguous-x kernels: FFT exchange or one padded line
     static constexpr int PADN = P::N + 3 * P::T;   // padded line + two rows of chunk ends (cn_line_smem.cuh)
     static constexpr int SM = (P::SMEM > PADN ? P::SMEM : PADN);
+    static constexpr int SMF = (P::SMEM > P::N ? P::SMEM : P::N);   // k_density_fftx: exchange rows or Z[N]
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -53,7 +54,7 @@ k_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __re
     const int lp = threadIdx.x / T, m = threadIdx.x % T;
     const long long pair = (long long)blockIdx.x * LP + lp;
     const bool active = pair < npairs;
-    cd* sm = smem + lp * XLine<P>::SM;
+    cd* sm = smem + lp * XLine<P>::SMF;
     const double s2 = scal[SC_S2];
     const cd* pa = psi + (active ? pair : 0) * 2 * N;
     const cd* pb = pa + N;
@@ -130,9 +131,12 @@ k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* _
 // a3 (x axis, complex-to-real) + a4 (+ a5)
 // ------------------------------------------------------------------------------------------------
 enum { NL_STEP = 0, NL_STEP_CNX = 1, NL_PHI = 2 };
+#ifndef NL_MINB
+#define NL_MINB 4
+#endif
 
 template <class P, int LP, bool RT, int MODE>
-__global__ void __launch_bounds__(P::T* LP)
+__global__ void __launch_bounds__(P::T* LP, NL_MINB)
 k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out,
                const cd* __restrict__ twA, const cd* __restrict__ twN, const double* __restrict__ scal,
                const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
@@ -289,7 +293,7 @@ template <int N> static int launch_density_fftx(dbec_handle_s* h) {
     const int npairs = h->ny * h->nz / 2;
     const int lp = npairs < LP ? npairs : LP;   // tiny grids: fewer pairs than a block holds
     (void)lp;
-    const size_t sm = (size_t)LP * XLine<P>::SM * sizeof(cd);
+    const size_t sm = (size_t)LP * XLine<P>::SMF * sizeof(cd);
     auto k = k_density_fftx<P, LP>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
