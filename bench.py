@@ -180,6 +180,22 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(x, world, device="cpu"):
+    """Max of a per-rank float over all ranks (the only collective of the benchmark; timing plumbing)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(npoints, steps, world, seconds):
+    """Replicas only: every rank advances its own npoints-grid `steps` times; the job took `seconds`."""
+    return world * npoints * steps / seconds
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
@@ -223,11 +239,8 @@ def run_ours(args, w):
         sampler.mark_stop()
     ms = e0.elapsed_time(e1)
     launches = sim.launch_count() - l0
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * w.npoints * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, dev)
+    value = whole_job_value(w.npoints, args.steps, world, ms * 1e-3)
     obs = sim.observables()
 
     # ---- end to end through the C ABI with host buffers ----
@@ -246,10 +259,7 @@ def run_ours(args, w):
         sim.get_psi(host_out.numpy())      # D2H of the step's result (synchronises)
     barrier()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * w.npoints * e2e_steps / float(t.item())
+    e2e_value = whole_job_value(w.npoints, e2e_steps, world, max_over_ranks(e2e_s, world, dev))
 
     # ---- per-kernel roofline (rank 0) ----
     line = None

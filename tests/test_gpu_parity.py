@@ -3,6 +3,9 @@ element on the same seeded inputs.  Tolerances: BASELINE.json `north_star` — p
 within 1e-12 relative max-abs; mu, energy, rms within 1e-9 relative.  Single parts use the same
 1e-12 bar.
 """
+import json
+import os
+
 import numpy as np
 import pytest
 
@@ -220,4 +223,35 @@ def test_errors_and_edge_cases(gp):
     sim.step(0)                      # zero steps: nothing happens
     assert np.all(sim.get_psi() == 0)
     assert sim.launch_count() >= 1
+    sim.close()
+
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.mark.parametrize("key", ["C1", "C2", "C3", "C4", "C5"])
+def test_full_run_observables_against_oracle_golden(gp, key):
+    """BASELINE.json: mu, energy, rms after the full run within 1e-9 relative.  The expected values were
+    written by tests/golden/make_golden.py, which calls only oracle/ (full oracle runs of C3-C5 take
+    tens of minutes, too long for this suite)."""
+    path = os.path.join(GOLDEN, f"{key}.json")
+    if not os.path.exists(path):
+        pytest.skip(f"no oracle golden file for {key} yet")
+    with open(path) as f:
+        gold = json.load(f)
+    w = workload(key)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(initial_psi(w))
+    if (w.G_run, w.D_run) != (w.G, w.D):
+        sim.set_coupling(w.G_run, w.D_run)
+    done = 0
+    for row in gold["observables"]:
+        sim.step(row["step"] - done)
+        done = row["step"]
+        a = sim.observables()
+        for k in ("norm", "mu", "energy", "rms_x", "rms_y", "rms_z", "rms_r", "density0"):
+            if w.ndim == 2 and k == "rms_z":
+                continue
+            assert abs(a[k] - row[k]) <= OBS_TOL * abs(row[k]), (key, row["step"], k, a[k], row[k])
+    assert done == w.steps
     sim.close()

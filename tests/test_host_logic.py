@@ -1,0 +1,123 @@
+"""CPU-only checks of the product's host side: the C-ABI library loads and exports every symbol that
+include/dbec.h declares, host-only entry points validate their arguments, there is no CPU fallback,
+and bench.py's multi-rank plumbing (replicas only: max-over-ranks time, whole-job value) works with
+world_size 2 over gloo."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gp():
+    from paper_1601_04640_b200 import dbec
+    dbec.lib()
+    return dbec
+
+
+def test_library_exports_every_declared_symbol(gp):
+    hdr = open(os.path.join(ROOT, "include", "dbec.h")).read()
+    declared = set(re.findall(r"\b(dbec_[a-z_0-9]+)\s*\(", hdr))
+    assert {"dbec_create", "dbec_set_psi", "dbec_step", "dbec_observables"} <= declared
+    L = gp.lib()
+    for name in sorted(declared):
+        assert hasattr(L, name), name
+    assert declared == set(gp.EXPORTS)
+    assert L.dbec_version() >= 100
+
+
+def test_workspace_bytes_validation_is_host_only(gp):
+    L = gp.lib()
+    n = C.c_size_t()
+    ok = gp.params(3, 256, 256, 256, .1, .1, .1, .005, 1, 1.2, .8, 200, 150, 1)
+    assert L.dbec_workspace_bytes(C.byref(ok), C.byref(n)) == gp.DBEC_OK
+    # psi + half spectrum + V_dd table + phi
+    P, SP = 256 ** 3, 256 * 256 * 136
+    assert n.value >= 16 * P + 16 * SP + 8 * SP + 8 * P
+    assert n.value < 16 * P + 16 * SP + 8 * SP + 8 * P + (4 << 20)
+    assert L.dbec_workspace_bytes(None, C.byref(n)) == gp.DBEC_EINVAL
+    assert L.dbec_workspace_bytes(C.byref(ok), None) == gp.DBEC_EINVAL
+    for bad, code in [
+        (gp.params(3, 48, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # not 2^k
+        (gp.params(3, 1024, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),    # too long
+        (gp.params(3, 32, 32, 8, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # too short
+        (gp.params(2, 32, 32, 2, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),      # 2-D with nz != 1
+        (gp.params(4, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
+        (gp.params(3, 32, 32, 32, 0., .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
+        (gp.params(3, 32, 32, 32, .5, .5, .5, 0., 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
+        (gp.params(3, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 2), gp.DBEC_EINVAL),      # time_mode
+        (gp.params(2, 32, 32, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=1), gp.DBEC_EINVAL),  # XZ: not built
+    ]:
+        assert L.dbec_workspace_bytes(C.byref(bad), C.byref(n)) == code
+    assert b"grid length" in L.dbec_strerror(gp.DBEC_ESIZE)
+
+
+def test_null_handles_are_rejected(gp):
+    L = gp.lib()
+    assert L.dbec_step(None, 1) == gp.DBEC_EINVAL
+    assert L.dbec_set_psi(None, None, 0) == gp.DBEC_EINVAL
+    assert L.dbec_observables(None, None) == gp.DBEC_EINVAL
+    assert L.dbec_destroy(None) == gp.DBEC_EINVAL
+    assert L.dbec_last_cuda_error(None) == 0
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the behaviour on a box without a GPU")
+def test_no_cpu_fallback(gp):
+    p = gp.params(3, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0)
+    with pytest.raises(RuntimeError, match="no CPU path"):
+        gp.Dbec(p)
+    # straight through the C ABI: an aligned, large enough (fake) workspace gets as far as the device check
+    h = C.c_void_p()
+    rc = gp.lib().dbec_create(C.byref(p), C.c_void_p(1 << 20), C.c_size_t(1 << 40), None, C.byref(h))
+    assert rc == gp.DBEC_ENODEVICE and not h.value
+
+
+def _rank_main(rank, world, port, q):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    ms = bench.max_over_ranks(10.0 + 5.0 * rank, world)            # slowest rank decides
+    q.put((rank, ms, bench.whole_job_value(1000, 4, world, ms * 1e-3)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_replica_timing_plumbing_gloo_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    for rank, ms, value in out:
+        assert ms == 15.0
+        assert value == pytest.approx(2 * 1000 * 4 / 0.015)
+
+
+def test_reference_arm_is_silent_on_other_ranks():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_reference_arm_prints_one_json_line():
+    import json
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "2",
+                        "--warmup", "1", "--workload", "C1"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle"
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["value"] > 0
