@@ -159,15 +159,23 @@ static const char* const kernel_names[DBEC_MAX_KERNELS] = {
         }                                                                                        \
     } while (0)
 
+static int launch_fft_pass(dbec_handle h, int axis, int mode) {
+    return dbec_tma_supported(h, axis) ? dbec_launch_fft_tma(h, axis, mode, 0, h->nz) : dbec_launch_fft_strided(h, axis, mode);
+}
+static int launch_cn_pass(dbec_handle h, int axis, int with_norm) {
+    return (axis > 0 && dbec_tma_supported(h, axis)) ? dbec_launch_cn_tma(h, axis, with_norm, 0, h->nz)
+                                                     : dbec_launch_cn(h, axis, with_norm);
+}
+
 // calcpsidd2 up to the x-inverse: density -> half spectrum -> x V_dd -> back along z, y.
 static int enqueue_dipolar_spectrum(dbec_handle h) {
     KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
     if (h->p.ndim == 3) {
-        KLAUNCH(h, KS_FFT_Y_FWD, dbec_launch_fft_strided(h, 1, 0));
-        KLAUNCH(h, KS_FFT_LAST_FMI, dbec_launch_fft_strided(h, 2, 2));
-        KLAUNCH(h, KS_FFT_Y_INV, dbec_launch_fft_strided(h, 1, 1));
+        KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0));
+        KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 2, 2));
+        KLAUNCH(h, KS_FFT_Y_INV, launch_fft_pass(h, 1, 1));
     } else {
-        KLAUNCH(h, KS_FFT_LAST_FMI, dbec_launch_fft_strided(h, 1, 2));
+        KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 1, 2));
     }
     return DBEC_OK;
 }
@@ -179,9 +187,9 @@ static int enqueue_step(dbec_handle h) {
     int rc = enqueue_dipolar_spectrum(h);
     if (rc) return rc;
     KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
-    if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, dbec_launch_cn(h, 0, 0));
+    if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, launch_cn_pass(h, 0, 0));
     for (int ax = 1; ax <= last_axis; ++ax)
-        KLAUNCH(h, ax == 1 ? KS_CN_Y : KS_CN_Z, dbec_launch_cn(h, ax, imag && ax == last_axis));
+        KLAUNCH(h, ax == 1 ? KS_CN_Y : KS_CN_Z, launch_cn_pass(h, ax, imag && ax == last_axis));
     return DBEC_OK;
 }
 
@@ -226,9 +234,9 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
     if (major != 10) return DBEC_ENODEVICE;          // sm_100a code only, no fallback
 
-    dbec_handle h = new (std::nothrow) dbec_handle_s;
+    dbec_handle h = new (std::nothrow) dbec_handle_s();
     if (!h) return DBEC_EINVAL;
-    memset(h, 0, sizeof(*h));
+    cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
     h->p = *p;
     h->stream = (cudaStream_t)cuda_stream;
     h->nx = p->nx; h->ny = p->ny; h->nz = p->nz;
@@ -250,6 +258,8 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->fuse_cnx = fe ? atoi(fe) : 1;
     const char* ge = getenv("DBEC_GRAPH");
     h->use_graph = ge ? atoi(ge) : 1;
+    const char* te = getenv("DBEC_TMA");
+    h->use_tma = te ? atoi(te) : 1;
     // the legacy default stream cannot be captured: plain launches there
     if (h->stream == nullptr || h->stream == cudaStreamLegacy) h->use_graph = 0;
 
@@ -267,6 +277,7 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
         if (rc) FAIL(rc);
         t += used;
     }
+    if (h->use_tma && dbec_make_tensor_maps(h)) FAIL(DBEC_ECUDA);
     if (write_scalars(h, true)) FAIL(DBEC_ECUDA);
     if (dbec_launch_build_vdd(h)) FAIL(DBEC_ECUDA);
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
@@ -352,7 +363,7 @@ int dbec_phi_dd(dbec_handle h, void* phi_f64_dev) {
 
 int dbec_cn_sweep(dbec_handle h, int axis) {
     if (!h || axis < 0 || axis > 2 || (h->p.ndim == 2 && axis == 2)) return DBEC_EINVAL;
-    LAUNCH(h, dbec_launch_cn(h, axis, 0));
+    LAUNCH(h, launch_cn_pass(h, axis, 0));
     return DBEC_OK;
 }
 

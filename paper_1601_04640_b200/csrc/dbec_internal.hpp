@@ -10,6 +10,10 @@
 #define DBEC_MAX_N 512          // longest supported grid line (16 values per thread x 32 lanes)
 #define DBEC_MAX_KERNELS 8      // kernels in one step (slots of dbec_step_profile)
 #define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
+#define DBEC_TMAP_BYTES 128     // sizeof(CUtensorMap)
+
+// Tensor maps of the handle (kernels_tma.cu): field x direction of the box rows.
+enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD_Y, TM_VDD_Z, TM_COUNT };
 
 // Device scalars every kernel reads (so that a captured CUDA graph never bakes them in).
 //   [0] s      deferred norm factor: true psi = s * stored psi (calcnorm; 1 in real time)
@@ -63,6 +67,9 @@ struct dbec_handle_s {
     int prof_slot[DBEC_MAX_KERNELS];
     int use_graph;                  // env DBEC_GRAPH (default 1): replay one captured step per dbec_step iteration
     int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
+    int use_tma;                    // env DBEC_TMA (default 1): persistent TMA-fed kernels for lines of 128..512 points
+    int num_sms;
+    alignas(64) unsigned char tmap[TM_COUNT][DBEC_TMAP_BYTES];
 };
 
 // ---- launchers (each returns a cudaError_t as int; all asynchronous on h->stream) ----
@@ -76,3 +83,8 @@ int dbec_launch_normalize(dbec_handle_s* h);               // a8 alone
 int dbec_launch_apply_scale(dbec_handle_s* h);             // psi <- s psi, s <- 1
 int dbec_launch_observables(dbec_handle_s* h);             // a9 (expects h->phi filled)
 int dbec_launch_build_vdd(dbec_handle_s* h);               // potdd table
+// persistent TMA-fed versions of the strided passes (kernels_tma.cu); z0, nzs: slab of planes (y passes)
+int dbec_make_tensor_maps(dbec_handle_s* h);
+int dbec_tma_supported(const dbec_handle_s* h, int axis);
+int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs);
+int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nzs);

@@ -1,0 +1,403 @@
+// kernels_tma.cu — the strided line passes (FFT along y/z on the half spectrum, Crank-Nicolson sweeps
+// along y/z on psi) as persistent, warp-specialised sm_100a kernels fed by the tensor memory
+// accelerator.  Same arithmetic as k_fft_strided / k_cn_strided (calcpsidd2, calcluy, calcluz —
+// PAPER.md:63, :67, :71, :79); what changes is how a tile travels:
+//
+//   global --TMA load--> shared stage --worker group: registers, in-place in the stage--> TMA store
+//
+// A tile is 8 neighbouring lines (8 x 16 B = one 128-byte row per line point), N rows.  One CTA per SM
+// walks its tiles round-robin; a loader thread keeps several stages in flight, NG worker groups each
+// transform one tile at a time, a storer thread drains finished stages.  Loads, arithmetic and stores
+// of different tiles overlap, so HBM stays busy while the Thomas recurrences and butterflies run.
+#include "dbec_internal.hpp"
+#include "fft_line.cuh"
+#include "cn_chunk.cuh"
+#include "cn_line_smem.cuh"
+#include "tma_pipe.cuh"
+
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
+
+constexpr int TCOLS = DBEC_SPEC_COLS;   // lines per tile
+
+struct TileGeom {
+    int ntiles_x;    // tiles along x (the contiguous direction)
+    int ntiles;      // all tiles of the pass (of the slab)
+    int axis;        // 1: lines along y, outer coordinate z;  2: lines along z, outer coordinate y
+    int box_rows;    // rows of one TMA box (<= 256)
+    int nbox;        // boxes per tile (N / box_rows)
+    int outer0;      // first outer coordinate (slab offset; axis 1 only)
+};
+
+struct PipeBars {
+    uint64_t* full; uint64_t* empty; uint64_t* done;
+};
+
+template <int NST> __device__ __forceinline__ PipeBars pipe_init(uint64_t* bars, int done_count) {
+    PipeBars b; b.full = bars; b.empty = bars + NST; b.done = bars + 2 * NST;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(b.full + s, 1); mbar_init(b.empty + s, 1); mbar_init(b.done + s, done_count); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    return b;
+}
+
+__device__ __forceinline__ void tile_coords(const TileGeom& tg, int t, int b, int inner, int& c0, int& c1, int& c2) {
+    const int tx = t % tg.ntiles_x, o = t / tg.ntiles_x + tg.outer0;
+    c0 = tx * inner;
+    c1 = tg.axis == 1 ? b * tg.box_rows : o;
+    c2 = tg.axis == 1 ? o : b * tg.box_rows;
+}
+
+// Loader: stage i % NST receives tile blockIdx.x + i * gridDim.x.  `extra` (optional) is a second
+// tensor map whose box lands EXTRA_OFF bytes into the stage (the V_dd tile of the fused z pass).
+template <int NST, int STAGE_BYTES, int MAIN_BYTES, int EXTRA_BYTES>
+__device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
+                                            const CUtensorMap* extra, const TileGeom& tg, int nmine) {
+    for (int i = 0; i < nmine; ++i) {
+        const int s = i % NST;
+        if (i >= NST) mbar_wait(pb.empty + s, ((i / NST) - 1) & 1);
+        mbar_expect_tx(pb.full + s, MAIN_BYTES + EXTRA_BYTES);
+        const int t = blockIdx.x + i * gridDim.x;
+        unsigned char* dst = stages + (size_t)s * STAGE_BYTES;
+        for (int b = 0; b < tg.nbox; ++b) {
+            int c0, c1, c2;
+            tile_coords(tg, t, b, 2 * TCOLS, c0, c1, c2);
+            tma_load_3d(dst + (size_t)b * (MAIN_BYTES / tg.nbox), map, c0, c1, c2, pb.full + s);
+            if (EXTRA_BYTES) {
+                tile_coords(tg, t, b, TCOLS, c0, c1, c2);
+                tma_load_3d(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.nbox), extra, c0, c1, c2, pb.full + s);
+            }
+        }
+    }
+}
+
+template <int NST, int STAGE_BYTES, int MAIN_BYTES>
+__device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
+                                            const TileGeom& tg, int nmine) {
+    for (int i = 0; i < nmine; ++i) {
+        const int s = i % NST;
+        mbar_wait(pb.done + s, (i / NST) & 1);
+        const int t = blockIdx.x + i * gridDim.x;
+        unsigned char* src = stages + (size_t)s * STAGE_BYTES;
+        for (int b = 0; b < tg.nbox; ++b) {
+            int c0, c1, c2;
+            tile_coords(tg, t, b, 2 * TCOLS, c0, c1, c2);
+            tma_store_3d(map, c0, c1, c2, src + (size_t)b * (MAIN_BYTES / tg.nbox));
+        }
+        bulk_commit();
+        if (i > 0) { bulk_wait_read<1>(); mbar_arrive(pb.empty + (i - 1) % NST); }
+    }
+    bulk_wait<0>();
+}
+
+// Sum over the block in a fixed order (same as kernels_cn.cu).
+template <int NT> __device__ __forceinline__ double block_sum_t(double x, double* red) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    constexpr int NW = (NT + 31) / 32;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) red[w] = x;
+    __syncthreads();
+    double t = (threadIdx.x < NW) ? red[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    }
+    return t;   // valid in thread 0
+}
+
+// ------------------------------------------------------------------------------------------------
+// Crank-Nicolson sweep along y or z (calcluy / calcluz)
+// ------------------------------------------------------------------------------------------------
+template <bool RT, int NCH, int NG, int NST, bool NORM>
+__global__ void __launch_bounds__(NG* NCH* TCOLS + 64, 1)
+k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, double* __restrict__ partial,
+         unsigned int* ticket, double* __restrict__ scal, double dV) {
+    typedef typename CnCoef<RT>::type CT;
+    constexpr int N = NCH * CN_L, GT = NCH * TCOLS, TILE = N * TCOLS, STAGE_BYTES = TILE * (int)sizeof(cd);
+    constexpr int NT = NG * GT + 64;
+    extern __shared__ unsigned char smraw[];
+    __shared__ double red[32];
+    __shared__ bool last;
+    unsigned char* base = (unsigned char*)(((uintptr_t)smraw + 127) & ~(uintptr_t)127);
+    cd* ends = (cd*)(base + (size_t)NST * STAGE_BYTES);
+    uint64_t* bars = (uint64_t*)(ends + NG * 2 * GT);
+    // h / PF / PB (entry k at k + k/16, so that the four chunks a warp works on hit different banks) and
+    // the chunk-end products, staged once per CTA: read straight from global memory inside the
+    // recurrences every table value costs an exposed L1/L2 round trip
+    CT* tab = (CT*)(bars + ((3 * NST + 1) & ~1));
+    constexpr int E = cn_tab_elems(N);
+    const int tid = threadIdx.x;
+    CnTab<RT> cs = cn_stage_tables<RT, N>(cn, tab);
+    for (int k = tid; k < NCH; k += NT) { tab[3 * E + k] = cn.pfe[k]; tab[3 * E + NCH + k] = cn.pbs[k]; }
+    cs.pfe = tab + 3 * E; cs.pbs = tab + 3 * E + NCH;
+    const PipeBars pb = pipe_init<NST>(bars, GT / 32);
+    const int nmine = (tg.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    double acc = 0.0;
+    if (tid < NG * GT) {
+        const int g = tid / GT, r = tid % GT, col = r % TCOLS, c = r / TCOLS, j0 = c * CN_L;
+        const int t0 = j0 + c;      // chunk c of the padded tables
+        cd* myends = ends + g * 2 * GT;
+        for (int i = g; i < nmine; i += NG) {
+            const int s = i % NST;
+            mbar_wait(pb.full + s, (i / NST) & 1);
+            cd* t = (cd*)(base + (size_t)s * STAGE_BYTES) + col;
+            cd u[CN_L];
+#pragma unroll
+            for (int k = 0; k < CN_L; ++k) u[k] = t[(j0 + k) * TCOLS];
+            const cd lo = (c > 0) ? t[(j0 - 1) * TCOLS] : cmake(0.0, 0.0);
+            const cd hi = (c < NCH - 1) ? t[(j0 + CN_L) * TCOLS] : cmake(0.0, 0.0);
+            cn_chunk_forward<CT>(u, lo, hi, cs.kap, cs.h + t0);
+            myends[c * TCOLS + col] = u[CN_L - 1];
+            named_bar_sync(1 + g, GT);
+            const cd din = cn_carry_forward<CT>(c, myends + col, TCOLS, cs.pfe);
+            cn_chunk_backward<CT>(u, din, cs.h + t0, cs.pf + t0);
+            myends[GT + c * TCOLS + col] = u[0];
+            named_bar_sync(1 + g, GT);
+            const cd uin = cn_carry_backward<CT>(c, NCH, myends + GT + col, TCOLS, cs.pbs);
+            cn_chunk_fix<CT>(u, uin, cs.pb + t0);
+#pragma unroll
+            for (int k = 0; k < CN_L; ++k) {
+                t[(j0 + k) * TCOLS] = u[k];
+                if (NORM) acc += cnorm2(u[k]);
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(pb.done + s);
+        }
+    } else if (tid == NG * GT) {
+        pipe_loader<NST, STAGE_BYTES, STAGE_BYTES, 0>(pb, base, &map, nullptr, tg, nmine);
+    } else if (tid == NG * GT + 32) {
+        pipe_storer<NST, STAGE_BYTES, STAGE_BYTES>(pb, base, &map, tg, nmine);
+    }
+    if (NORM) {
+        // calcnorm: block partial -> last block writes the deferred factor (reading S13)
+        const double part = block_sum_t<NT>(acc, red);
+        const unsigned int nb = gridDim.x;
+        if (tid == 0) {
+            partial[blockIdx.x] = part;
+            __threadfence();
+            last = (atomicAdd(ticket, 1u) == nb - 1);
+        }
+        __syncthreads();
+        if (last) {
+            __threadfence();
+            double a = 0.0;
+            for (unsigned int i = tid; i < nb; i += NT) a += __ldcg(partial + i);
+            const double tot = block_sum_t<NT>(a, red);
+            if (tid == 0) {
+                const double sfac = 1.0 / sqrt(tot * dV);
+                scal[SC_S] = sfac;
+                scal[SC_S2] = sfac * sfac;
+                *ticket = 0u;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// FFT along y or z on the half spectrum (calcpsidd2); MODE 2 = forward * V_dd(k)/P * inverse
+// ------------------------------------------------------------------------------------------------
+template <class P, int S>
+__device__ __forceinline__ void fft_line_nb(cd (&v)[16], int m, cd* sm, const cd* __restrict__ twA,
+                                            const cd* __restrict__ twN, int bar, int nthreads) {
+    fft_stage1<P, S>(v, m, twA);
+    if (P::T > 1) {
+        fft_x1_write<P>(v, m, sm, TCOLS);            // every thread overwrites only rows it owns
+        named_bar_sync(bar, nthreads);
+        fft_stage2<P, S>(v, m, sm, TCOLS, twN);
+        if (P::R3 > 1) {
+            named_bar_sync(bar, nthreads);
+            fft_x2_write<P>(v, m, sm, TCOLS);
+            named_bar_sync(bar, nthreads);
+            fft_stage3<P, S>(v, m, sm, TCOLS);
+        }
+    }
+}
+
+template <class P, int MODE, int NG, int NST>
+__global__ void __launch_bounds__(NG* P::T* TCOLS + 64, 1)
+k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap map_vdd,
+          const cd* twA, const cd* twN, TileGeom tg) {
+    constexpr int T = P::T, N = P::N, GT = T * TCOLS;
+    constexpr int MAIN_BYTES = N * TCOLS * (int)sizeof(cd);
+    constexpr int EXTRA_BYTES = (MODE == 2) ? N * TCOLS * (int)sizeof(double) : 0;
+    constexpr int STAGE_BYTES = MAIN_BYTES + EXTRA_BYTES;
+    extern __shared__ unsigned char smraw[];
+    unsigned char* base = (unsigned char*)(((uintptr_t)smraw + 127) & ~(uintptr_t)127);
+    uint64_t* bars = (uint64_t*)(base + (size_t)NST * STAGE_BYTES);
+    // twiddle tables staged once per CTA (2 x N entries)
+    cd* tw = (cd*)(bars + ((3 * NST + 1) & ~1));
+    const int tid = threadIdx.x;
+    for (int k = tid; k < N; k += NG * GT + 64) { tw[k] = twA[k]; tw[N + k] = twN[k]; }
+    twA = tw; twN = tw + N;
+    const PipeBars pb = pipe_init<NST>(bars, GT / 32);
+    const int nmine = (tg.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    if (tid < NG * GT) {
+        const int g = tid / GT, r = tid % GT, col = r % TCOLS, m = r / TCOLS;
+        for (int i = g; i < nmine; i += NG) {
+            const int s = i % NST;
+            mbar_wait(pb.full + s, (i / NST) & 1);
+            cd* sm = (cd*)(base + (size_t)s * STAGE_BYTES) + col;
+            cd v[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = sm[(j * T + m) * TCOLS];
+            if (MODE == 0 || MODE == 2) fft_line_nb<P, -1>(v, m, sm, twA, twN, 1 + g, GT);
+            if (MODE == 2) {
+                const double* w = (const double*)(base + (size_t)s * STAGE_BYTES + MAIN_BYTES) + col;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) v[j] = cmul(w[(j * T + m) * TCOLS], v[j]);
+            }
+            if (MODE == 2 && T > 1) named_bar_sync(1 + g, GT);      // stage-2/3 reads of the forward pass are over
+            if (MODE == 1 || MODE == 2) fft_line_nb<P, +1>(v, m, sm, twA, twN, 1 + g, GT);
+            if (T > 1) named_bar_sync(1 + g, GT);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) sm[(j * T + m) * TCOLS] = v[j];
+            fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(pb.done + s);
+        }
+    } else if (tid == NG * GT) {
+        pipe_loader<NST, STAGE_BYTES, MAIN_BYTES, EXTRA_BYTES>(pb, base, &map, &map_vdd, tg, nmine);
+    } else if (tid == NG * GT + 32) {
+        pipe_storer<NST, STAGE_BYTES, MAIN_BYTES>(pb, base, &map, tg, nmine);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// tensor maps
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// A field of doubles [n2][n1][n0] (n0 fastest) and a box of (b0, b1, b2) elements.
+static int make_map(CUtensorMap* m, void* ptr, long long n0, long long n1, long long n2, int b0, int b1, int b2) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return (int)cudaErrorNotSupported;
+    cuuint64_t dims[3] = {(cuuint64_t)n0, (cuuint64_t)n1, (cuuint64_t)n2};
+    cuuint64_t strides[2] = {(cuuint64_t)n0 * 8, (cuuint64_t)n0 * n1 * 8};
+    cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, ptr, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
+}
+
+static int box_rows_of(int n) { return n < 256 ? n : 256; }
+
+// Maps of the handle: psi / spec / vdd, boxes along y and along z.  Called once by dbec_create.
+int dbec_make_tensor_maps(dbec_handle_s* h) {
+    static_assert(sizeof(CUtensorMap) == DBEC_TMAP_BYTES, "tensor map size");
+    const int by = box_rows_of(h->ny), bz = box_rows_of(h->nz);
+    int rc = 0;
+    rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Y], h->psi, 2LL * h->nx, h->ny, h->nz, 2 * TCOLS, by, 1);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Z], h->psi, 2LL * h->nx, h->ny, h->nz, 2 * TCOLS, 1, bz);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Y], h->spec, 2LL * h->nxhp, h->ny, h->nz, 2 * TCOLS, by, 1);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Z], h->spec, 2LL * h->nxhp, h->ny, h->nz, 2 * TCOLS, 1, bz);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Y], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, by, 1);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Z], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, 1, bz);
+    return rc ? (int)cudaErrorInvalidValue : 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+static TileGeom geom_of(const dbec_handle_s* h, int axis, int row_elems, int z0, int nzs) {
+    TileGeom tg;
+    tg.axis = axis;
+    tg.ntiles_x = row_elems / TCOLS;
+    const int n = axis == 1 ? h->ny : h->nz;
+    tg.box_rows = box_rows_of(n);
+    tg.nbox = n / tg.box_rows;
+    if (axis == 1) { tg.ntiles = tg.ntiles_x * nzs; tg.outer0 = z0; }
+    else { tg.ntiles = tg.ntiles_x * h->ny; tg.outer0 = 0; }
+    return tg;
+}
+
+static int grid_of(const dbec_handle_s* h, int ntiles) { return ntiles < h->num_sms ? ntiles : h->num_sms; }
+
+template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
+    constexpr int GT = NCH * TCOLS, STAGE = NCH * CN_L * TCOLS * (int)sizeof(cd);
+    const TileGeom tg = geom_of(h, axis, h->nx, z0, nzs);
+    const int grid = grid_of(h, tg.ntiles);
+    if (NORM && grid > h->npartial) return (int)cudaErrorInvalidValue;
+    const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 1) * sizeof(uint64_t) +
+                      (3 * cn_tab_elems(NCH * CN_L) + 2 * NCH) * sizeof(typename CnCoef<RT>::type);
+    auto k = k_cn_tma<RT, NCH, NG, NST, NORM>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_PSI_Y : TM_PSI_Z];
+    k<<<grid, NG * GT + 64, sm, h->stream>>>(*map, make_cntab<RT>(h->ax[axis]), tg, h->partial, h->ticket, h->scal, h->dV);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <bool RT, bool NORM> static int launch_cn_tma_n(dbec_handle_s* h, int axis, int z0, int nzs) {
+    switch (h->ax[axis].n) {
+        case 128: return launch_cn_tma<RT, 8, 4, 12, NORM>(h, axis, z0, nzs);     // 16 KiB tiles
+        case 256: return launch_cn_tma<RT, 16, 3, 6, NORM>(h, axis, z0, nzs);     // 32 KiB tiles
+        case 512: return launch_cn_tma<RT, 32, 1, 3, NORM>(h, axis, z0, nzs);     // 64 KiB tiles
+        default: return (int)cudaErrorInvalidValue;
+    }
+}
+
+int dbec_tma_supported(const dbec_handle_s* h, int axis) {
+    const int n = h->ax[axis].n;
+    return h->use_tma && (n == 128 || n == 256 || n == 512);
+}
+
+int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nzs) {
+    if (h->p.time_mode == 1)
+        return with_norm ? launch_cn_tma_n<true, true>(h, axis, z0, nzs) : launch_cn_tma_n<true, false>(h, axis, z0, nzs);
+    return with_norm ? launch_cn_tma_n<false, true>(h, axis, z0, nzs) : launch_cn_tma_n<false, false>(h, axis, z0, nzs);
+}
+
+template <int N> struct PlanS;
+template <> struct PlanS<128> { typedef FftPlan<8, 1, false> P; };
+template <> struct PlanS<256> { typedef FftPlan<16, 1, false> P; };
+template <> struct PlanS<512> { typedef FftPlan<16, 2, false> P; };
+
+template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
+    typedef typename PlanS<N>::P P;
+    constexpr int GT = P::T * TCOLS;
+    constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? N * TCOLS * (int)sizeof(double) : 0);
+    const TileGeom tg = geom_of(h, axis, h->nxhp, z0, nzs);
+    const int grid = grid_of(h, tg.ntiles);
+    const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 2) * sizeof(uint64_t) + 2 * N * sizeof(cd);
+    auto k = k_fft_tma<P, MODE, NG, NST>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_SPEC_Y : TM_SPEC_Z];
+    const CUtensorMap* mv = (const CUtensorMap*)h->tmap[axis == 1 ? TM_VDD_Y : TM_VDD_Z];
+    k<<<grid, NG * GT + 64, sm, h->stream>>>(*map, *mv, h->ax[axis].twA, h->ax[axis].twN, tg);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <int MODE> static int launch_fft_tma_n(dbec_handle_s* h, int axis, int z0, int nzs) {
+    switch (h->ax[axis].n) {
+        case 128: return launch_fft_tma<128, MODE, 4, (MODE == 2 ? 8 : 12)>(h, axis, z0, nzs);
+        case 256: return launch_fft_tma<256, MODE, 2, (MODE == 2 ? 4 : 6)>(h, axis, z0, nzs);
+        case 512: return launch_fft_tma<512, MODE, 1, (MODE == 2 ? 2 : 3)>(h, axis, z0, nzs);
+        default: return (int)cudaErrorInvalidValue;
+    }
+}
+
+int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs) {
+    if (mode == 0) return launch_fft_tma_n<0>(h, axis, z0, nzs);
+    if (mode == 1) return launch_fft_tma_n<1>(h, axis, z0, nzs);
+    return launch_fft_tma_n<2>(h, axis, z0, nzs);
+}
