@@ -186,7 +186,8 @@ static int enqueue_step(dbec_handle h) {
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
     int rc = enqueue_dipolar_spectrum(h);
     if (rc) return rc;
-    KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
+    if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nz));
+    else KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
     if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, launch_cn_pass(h, 0, 0));
     for (int ax = 1; ax <= last_axis; ++ax)
         KLAUNCH(h, ax == 1 ? KS_CN_Y : KS_CN_Z, launch_cn_pass(h, ax, imag && ax == last_axis));

@@ -88,3 +88,6 @@ int dbec_make_tensor_maps(dbec_handle_s* h);
 int dbec_tma_supported(const dbec_handle_s* h, int axis);
 int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs);
 int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nzs);
+// persistent bulk-copy-fed versions of the x passes (kernels_xline.cu)
+int dbec_xline_supported(const dbec_handle_s* h);
+int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs);          // a3 (x) + a4 + a5

@@ -159,3 +159,24 @@ template <class P, int S> DBEC_HD void fft_stage3(cd (&v)[16], int m, const cd* 
         for (int k3 = 0; k3 < P::R3; ++k3) v[i + P::I3 * k3] = w[k3];
     }
 }
+
+#if defined(__CUDACC__)
+// One line FFT in registers with its shared-memory exchanges.  SYNC = 0: the T threads of a line sit
+// in one warp (__syncwarp); SYNC = 1: block-wide barrier (tile kernels).
+template <class P, int S, int SYNC>
+__device__ __forceinline__ void fft_line(cd (&v)[16], int m, cd* sm, int es, const cd* __restrict__ twA,
+                                         const cd* __restrict__ twN) {
+    fft_stage1<P, S>(v, m, twA);
+    if (P::T > 1) {
+        fft_x1_write<P>(v, m, sm, es);
+        if (SYNC) __syncthreads(); else __syncwarp();
+        fft_stage2<P, S>(v, m, sm, es, twN);
+        if (P::R3 > 1) {
+            if (SYNC) __syncthreads(); else __syncwarp();
+            fft_x2_write<P>(v, m, sm, es);
+            if (SYNC) __syncthreads(); else __syncwarp();
+            fft_stage3<P, S>(v, m, sm, es);
+        }
+    }
+}
+#endif

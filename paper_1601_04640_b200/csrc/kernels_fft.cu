@@ -16,25 +16,6 @@
 #include "cn_chunk.cuh"
 #include "cn_line_smem.cuh"
 
-// One line FFT in registers with its shared-memory exchanges.  SYNC = 0: the T threads of a line sit
-// in one warp (__syncwarp); SYNC = 1: block-wide barrier (tile kernels).
-template <class P, int S, int SYNC>
-__device__ __forceinline__ void fft_line(cd (&v)[16], int m, cd* sm, int es, const cd* __restrict__ twA,
-                                         const cd* __restrict__ twN) {
-    fft_stage1<P, S>(v, m, twA);
-    if (P::T > 1) {
-        fft_x1_write<P>(v, m, sm, es);
-        if (SYNC) __syncthreads(); else __syncwarp();
-        fft_stage2<P, S>(v, m, sm, es, twN);
-        if (P::R3 > 1) {
-            if (SYNC) __syncthreads(); else __syncwarp();
-            fft_x2_write<P>(v, m, sm, es);
-            if (SYNC) __syncthreads(); else __syncwarp();
-            fft_stage3<P, S>(v, m, sm, es);
-        }
-    }
-}
-
 template <class P> struct XLine {
     // shared elements per line pair of the contiguous-x kernels: FFT exchange or one padded line
     static constexpr int PADN = P::N + 3 * P::T;   // padded line + two rows of chunk ends (cn_line_smem.cuh)

@@ -118,10 +118,10 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
     typedef typename CnCoef<RT>::type CT;
     constexpr int N = NCH * CN_L, GT = NCH * TCOLS, TILE = N * TCOLS, STAGE_BYTES = TILE * (int)sizeof(cd);
     constexpr int NT = NG * GT + 64;
-    extern __shared__ unsigned char smraw[];
+    extern __shared__ __align__(1024) unsigned char smraw[];
     __shared__ double red[32];
     __shared__ bool last;
-    unsigned char* base = (unsigned char*)(((uintptr_t)smraw + 127) & ~(uintptr_t)127);
+    unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
     cd* ends = (cd*)(base + (size_t)NST * STAGE_BYTES);
     uint64_t* bars = (uint64_t*)(ends + NG * 2 * GT);
     // h / PF / PB (entry k at k + k/16, so that the four chunks a warp works on hit different banks) and
@@ -225,8 +225,8 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
     constexpr int MAIN_BYTES = N * TCOLS * (int)sizeof(cd);
     constexpr int EXTRA_BYTES = (MODE == 2) ? N * TCOLS * (int)sizeof(double) : 0;
     constexpr int STAGE_BYTES = MAIN_BYTES + EXTRA_BYTES;
-    extern __shared__ unsigned char smraw[];
-    unsigned char* base = (unsigned char*)(((uintptr_t)smraw + 127) & ~(uintptr_t)127);
+    extern __shared__ __align__(1024) unsigned char smraw[];
+    unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
     uint64_t* bars = (uint64_t*)(base + (size_t)NST * STAGE_BYTES);
     // twiddle tables staged once per CTA (2 x N entries)
     cd* tw = (cd*)(bars + ((3 * NST + 1) & ~1));

@@ -1,0 +1,218 @@
+// kernels_xline.cu — the passes along x (contiguous grid lines) as persistent, warp-specialised
+// sm_100a kernels fed by bulk asynchronous copies (cp.async.bulk + mbarrier, tma_pipe.cuh):
+//
+//   k_xline_nonlin   a3 along x (complex-to-real inverse FFT, two real lines per complex transform,
+//                    PAPER.md:71) + a4 psi <- s psi exp(-c dt (V + G n + D Phi)) (calcnu)
+//                    + a5 the Crank-Nicolson sweep along x (calclux), one tile of
+//                    8 grid lines at a time, all in shared memory.
+//   k_xline_density  a1 along x: n = |s psi|^2 fused into the forward real-to-complex transform.
+//
+// Same arithmetic as k_ifftx_nonlin / k_density_fftx (kernels_fft.cu); what changes is that the next
+// tiles' loads and the previous tiles' stores are in flight while a tile is being worked on.
+#include "dbec_internal.hpp"
+#include "fft_line.cuh"
+#include "cn_chunk.cuh"
+#include "cn_line_smem.cuh"
+#include "tma_pipe.cuh"
+
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
+
+constexpr int XP = 4;            // line pairs per tile
+constexpr int XR = 2 * XP;       // grid lines per tile
+
+template <int N> struct XPlan;
+template <> struct XPlan<128> { typedef FftPlan<8, 1, true> P; };
+template <> struct XPlan<256> { typedef FftPlan<16, 1, true> P; };
+
+__host__ __device__ constexpr int nxhp_of(int n) { return ((n / 2 + 1) + DBEC_SPEC_COLS - 1) / DBEC_SPEC_COLS * DBEC_SPEC_COLS; }
+
+// ------------------------------------------------------------------------------------------------
+// a3 (x) + a4 + a5
+// ------------------------------------------------------------------------------------------------
+// Stage layout: 8 psi lines with a pitch of N+1 elements (so that the 8 lines of a tile sit in 8
+// different 16-byte bank groups and the chunked Thomas pass reads them without conflicts), then the
+// 8 half-spectrum rows.  A pair's two spectrum rows (2*NXHP elements) double as its FFT exchange
+// buffer once they are in registers; after the transform the spectrum area holds the chunk ends of
+// the Thomas carries.
+template <class P, bool RT, int NG, int NST>
+__global__ void __launch_bounds__(NG* XR* P::T + 64, 1)
+k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __restrict__ twA_g,
+               const cd* __restrict__ twN_g, const double* __restrict__ scal, const double* __restrict__ vx_g,
+               const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny,
+               long long row0, CnTab<RT> cn) {
+    typedef typename CnCoef<RT>::type CT;
+    // A group of GT = 8*T threads owns one tile: its first half runs the four pair transforms (T threads
+    // per pair), then all of it runs calcnu (T threads per line) and calclux (one 16-point chunk each).
+    constexpr int T = P::T, N = P::N, NCH = N / CN_L, GT = XR * T, NT = NG * GT + 64;
+    constexpr int NXHP = nxhp_of(N), PITCH = N + 1;
+    constexpr int PSI_BYTES = XR * PITCH * (int)sizeof(cd), SPEC_BYTES = XR * NXHP * (int)sizeof(cd);
+    constexpr int STAGE_BYTES = PSI_BYTES + SPEC_BYTES;
+    constexpr int E = cn_tab_elems(N);
+    static_assert(NCH == T, "one chunk per thread of a line");
+    static_assert(P::SMEM <= 2 * NXHP, "a pair's spectrum rows must hold its FFT exchange");
+    static_assert(2 * NCH * XR <= XR * NXHP, "chunk ends must fit the spectrum area");
+    extern __shared__ __align__(1024) unsigned char smraw[];
+    unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
+    cd* tw = (cd*)(base + (size_t)NST * STAGE_BYTES);            // twA [N], twN [N]
+    CT* tab = (CT*)(tw + 2 * N);                                 // h, PF, PB (padded), PFE, PBS
+    double* vxs = (double*)(tab + 3 * E + 2 * NCH);              // trap table along x
+    uint64_t* bars = (uint64_t*)(vxs + N);
+    uint64_t* full = bars; uint64_t* empty = bars + NST; uint64_t* done = bars + 2 * NST;
+    const int tid = threadIdx.x;
+    for (int k = tid; k < N; k += NT) { tw[k] = twA_g[k]; tw[N + k] = twN_g[k]; vxs[k] = vx_g[k]; }
+    CnTab<RT> cs = cn_stage_tables<RT, N>(cn, tab);
+    for (int k = tid; k < NCH; k += NT) { tab[3 * E + k] = cn.pfe[k]; tab[3 * E + NCH + k] = cn.pbs[k]; }
+    cs.pfe = tab + 3 * E; cs.pbs = tab + 3 * E + NCH;
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); mbar_init(done + s, GT / 32); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    const int nmine = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    if (tid < NG * GT) {
+        const int g = tid / GT, t = tid % GT;
+        const int lp = t / T, m = t % T;                 // transform: pair lp (t < GT/2); calcnu: line lp, x = j*T + m
+        const int r = t % XR, c = t / XR;                // calclux: line r, chunk c
+        const cd* twA = tw; const cd* twN = tw + N;
+        const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
+        for (int i = g; i < nmine; i += NG) {
+            const int st = i % NST;
+            mbar_wait(full + st, (i / NST) & 1);
+            cd* ps = (cd*)(base + (size_t)st * STAGE_BYTES);
+            cd* ss = (cd*)(base + (size_t)st * STAGE_BYTES + PSI_BYTES);
+            const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            // ---- inverse transform of a pair's spectrum: v[j] = (Phi on line a, Phi on line b) at x = j*T + m;
+            //      Phi goes back to the pair's spectrum rows as two real lines [2][N]
+            if (t < GT / 2) {
+                cd* sa = ss + (2 * lp) * NXHP;
+                const cd* sb = sa + NXHP;
+                cd v[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int k = j * T + m;
+                    if (k <= N / 2) {
+                        cd a = sa[k], b = sb[k];
+                        v[j] = cmake(a.x - b.y, a.y + b.x);          // X_a + i X_b
+                    } else {
+                        cd a = sa[N - k], b = sb[N - k];
+                        v[j] = cmake(a.x + b.y, b.x - a.y);          // conj X_a + i conj X_b
+                    }
+                }
+                __syncwarp();                                        // the pair's rows are in registers: reuse them
+                fft_line<P, +1, 0>(v, m, sa, 1, twA, twN);
+                __syncwarp();
+                double* ph = (double*)sa;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) { ph[j * T + m] = v[j].x; ph[N + j * T + m] = v[j].y; }
+            }
+            named_bar_sync(1 + g, GT);
+            // ---- calcnu on line lp
+            {
+                const long long row = row0 + tile * XR + lp;
+                const int y = (int)(row % ny), z = (int)(row / ny);
+                const double vrow = vy[y] + vz[z];
+                cd* p = ps + lp * PITCH;
+                const double* ph = (const double*)(ss + (lp >> 1) * 2 * NXHP) + (lp & 1) * N;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const cd q = p[j * T + m];
+                    const double u = dt * (vxs[j * T + m] + vrow + G * (s2 * cnorm2(q)) + D * ph[j * T + m]);
+                    if (RT) {
+                        double sn, cs_;
+                        sincos(u, &sn, &cs_);
+                        p[j * T + m] = cmul(s, cmul(q, cmake(cs_, -sn)));
+                    } else {
+                        p[j * T + m] = cmul(s * exp(-u), q);
+                    }
+                }
+            }
+            named_bar_sync(1 + g, GT);
+            // ---- calclux: line r, chunk c
+            cd* line = ps + r * PITCH + c * CN_L;
+            cd* e0 = ss;                    // [NCH][XR] forward chunk ends
+            cd* e1 = ss + NCH * XR;         // [NCH][XR] backward chunk starts
+            cd u[CN_L];
+#pragma unroll
+            for (int k = 0; k < CN_L; ++k) u[k] = line[k];
+            const cd lo = (c > 0) ? line[-1] : cmake(0.0, 0.0);
+            const cd hi = (c < NCH - 1) ? line[CN_L] : cmake(0.0, 0.0);
+            cn_chunk_forward<CT>(u, lo, hi, cs.kap, cs.h + 17 * c);
+            e0[c * XR + r] = u[CN_L - 1];
+            named_bar_sync(1 + g, GT);
+            const cd din = cn_carry_forward<CT>(c, e0 + r, XR, cs.pfe);
+            cn_chunk_backward<CT>(u, din, cs.h + 17 * c, cs.pf + 17 * c);
+            e1[c * XR + r] = u[0];
+            named_bar_sync(1 + g, GT);
+            const cd uin = cn_carry_backward<CT>(c, NCH, e1 + r, XR, cs.pbs);
+            cn_chunk_fix<CT>(u, uin, cs.pb + 17 * c);
+#pragma unroll
+            for (int k = 0; k < CN_L; ++k) line[k] = u[k];
+            fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(done + st);
+        }
+    } else if (tid == NG * GT) {
+        for (int i = 0; i < nmine; ++i) {
+            const int st = i % NST;
+            if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            mbar_expect_tx(full + st, XR * N * (int)sizeof(cd) + SPEC_BYTES);
+            const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            unsigned char* dst = base + (size_t)st * STAGE_BYTES;
+            const cd* src = psi + tile * XR * N;
+#pragma unroll
+            for (int rr = 0; rr < XR; ++rr)
+                bulk_load(dst + (size_t)rr * PITCH * sizeof(cd), src + (size_t)rr * N, N * (int)sizeof(cd), full + st);
+            bulk_load(dst + PSI_BYTES, spec + tile * XR * NXHP, SPEC_BYTES, full + st);
+        }
+    } else if (tid == NG * GT + 32) {
+        for (int i = 0; i < nmine; ++i) {
+            const int st = i % NST;
+            mbar_wait(done + st, (i / NST) & 1);
+            const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            const unsigned char* src = base + (size_t)st * STAGE_BYTES;
+            cd* dstg = psi + tile * XR * N;
+#pragma unroll
+            for (int rr = 0; rr < XR; ++rr)
+                bulk_store(dstg + (size_t)rr * N, src + (size_t)rr * PITCH * sizeof(cd), N * (int)sizeof(cd));
+            bulk_commit();
+            if (i > 0) { bulk_wait_read<1>(); mbar_arrive(empty + (i - 1) % NST); }
+        }
+        bulk_wait<0>();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+int dbec_xline_supported(const dbec_handle_s* h) {
+    return h->use_tma && (h->nx == 128 || h->nx == 256) && ((h->ny * h->nz) % XR == 0);
+}
+
+template <int N, bool RT, int NG, int NST> static int launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
+    typedef typename XPlan<N>::P P;
+    typedef typename CnCoef<RT>::type CT;
+    constexpr int GT = XR * P::T, NXHP = nxhp_of(N);
+    constexpr int STAGE = XR * (N + 1) * (int)sizeof(cd) + XR * NXHP * (int)sizeof(cd);
+    if (h->nxhp != NXHP) return (int)cudaErrorInvalidValue;
+    const int ntiles = (int)((long long)h->ny * nzs / XR);
+    const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
+    const size_t sm = 128 + (size_t)NST * STAGE + 2 * N * sizeof(cd) + (3 * cn_tab_elems(N) + 2 * (N / CN_L)) * sizeof(CT) +
+                      N * sizeof(double) + 3 * NST * sizeof(uint64_t);
+    auto k = k_xline_nonlin<P, RT, NG, NST>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const long long row0 = (long long)z0 * h->ny;
+    k<<<grid, NG * GT + 64, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
+                                             h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, row0,
+                                             make_cntab<RT>(h->ax[0]));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
+    const bool rt = h->p.time_mode == 1;
+    switch (h->nx) {
+        case 128: return rt ? launch_xline_nonlin<128, true, 4, 8>(h, z0, nzs) : launch_xline_nonlin<128, false, 4, 8>(h, z0, nzs);
+        case 256: return rt ? launch_xline_nonlin<256, true, 3, 4>(h, z0, nzs) : launch_xline_nonlin<256, false, 3, 4>(h, z0, nzs);
+        default: return (int)cudaErrorInvalidValue;
+    }
+}
