@@ -72,10 +72,12 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
     }
 }
 
+// Two storers take alternate tiles (first = 0 / 1): while one sits in wait_group.read (which lasts about
+// as long as the global write), the other already drains the next finished stage.
 template <int NST, int STAGE_BYTES, int MAIN_BYTES>
 __device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
-                                            const TileGeom& tg, int nmine) {
-    for (int i = 0; i < nmine; ++i) {
+                                            const TileGeom& tg, int nmine, int first) {
+    for (int i = first; i < nmine; i += 2) {
         const int s = i % NST;
         mbar_wait(pb.done + s, (i / NST) & 1);
         const int t = blockIdx.x + i * gridDim.x;
@@ -86,7 +88,8 @@ __device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* s
             tma_store_3d(map, c0, c1, c2, src + (size_t)b * (MAIN_BYTES / tg.nbox));
         }
         bulk_commit();
-        if (i > 0) { bulk_wait_read<1>(); mbar_arrive(pb.empty + (i - 1) % NST); }
+        bulk_wait_read<0>();              // the copy engine has read the stage (fast; not the global write)
+        mbar_arrive(pb.empty + s);
     }
     bulk_wait<0>();
 }
@@ -112,12 +115,12 @@ template <int NT> __device__ __forceinline__ double block_sum_t(double x, double
 // Crank-Nicolson sweep along y or z (calcluy / calcluz)
 // ------------------------------------------------------------------------------------------------
 template <bool RT, int NCH, int NG, int NST, bool NORM>
-__global__ void __launch_bounds__(NG* NCH* TCOLS + 64, 1)
+__global__ void __launch_bounds__(NG* NCH* TCOLS + 96, 1)
 k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, double* __restrict__ partial,
          unsigned int* ticket, double* __restrict__ scal, double dV) {
     typedef typename CnCoef<RT>::type CT;
     constexpr int N = NCH * CN_L, GT = NCH * TCOLS, TILE = N * TCOLS, STAGE_BYTES = TILE * (int)sizeof(cd);
-    constexpr int NT = NG * GT + 64;
+    constexpr int NT = NG * GT + 96;
     extern __shared__ __align__(1024) unsigned char smraw[];
     __shared__ double red[32];
     __shared__ bool last;
@@ -169,8 +172,8 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
         }
     } else if (tid == NG * GT) {
         pipe_loader<NST, STAGE_BYTES, STAGE_BYTES, 0>(pb, base, &map, nullptr, tg, nmine);
-    } else if (tid == NG * GT + 32) {
-        pipe_storer<NST, STAGE_BYTES, STAGE_BYTES>(pb, base, &map, tg, nmine);
+    } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
+        pipe_storer<NST, STAGE_BYTES, STAGE_BYTES>(pb, base, &map, tg, nmine, (tid - NG * GT) / 32 - 1);
     }
     if (NORM) {
         // calcnorm: block partial -> last block writes the deferred factor (reading S13)
@@ -218,7 +221,7 @@ __device__ __forceinline__ void fft_line_nb(cd (&v)[16], int m, cd* sm, const cd
 }
 
 template <class P, int MODE, int NG, int NST>
-__global__ void __launch_bounds__(NG* P::T* TCOLS + 64, 1)
+__global__ void __launch_bounds__(NG* P::T* TCOLS + 96, 1)
 k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap map_vdd,
           const cd* twA, const cd* twN, TileGeom tg) {
     constexpr int T = P::T, N = P::N, GT = T * TCOLS;
@@ -231,7 +234,7 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
     // twiddle tables staged once per CTA (2 x N entries)
     cd* tw = (cd*)(bars + ((3 * NST + 1) & ~1));
     const int tid = threadIdx.x;
-    for (int k = tid; k < N; k += NG * GT + 64) { tw[k] = twA[k]; tw[N + k] = twN[k]; }
+    for (int k = tid; k < N; k += NG * GT + 96) { tw[k] = twA[k]; tw[N + k] = twN[k]; }
     twA = tw; twN = tw + N;
     const PipeBars pb = pipe_init<NST>(bars, GT / 32);
     const int nmine = (tg.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
@@ -261,8 +264,8 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
         }
     } else if (tid == NG * GT) {
         pipe_loader<NST, STAGE_BYTES, MAIN_BYTES, EXTRA_BYTES>(pb, base, &map, &map_vdd, tg, nmine);
-    } else if (tid == NG * GT + 32) {
-        pipe_storer<NST, STAGE_BYTES, MAIN_BYTES>(pb, base, &map, tg, nmine);
+    } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
+        pipe_storer<NST, STAGE_BYTES, MAIN_BYTES>(pb, base, &map, tg, nmine, (tid - NG * GT) / 32 - 1);
     }
 }
 
@@ -341,7 +344,7 @@ template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma
     auto k = k_cn_tma<RT, NCH, NG, NST, NORM>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_PSI_Y : TM_PSI_Z];
-    k<<<grid, NG * GT + 64, sm, h->stream>>>(*map, make_cntab<RT>(h->ax[axis]), tg, h->partial, h->ticket, h->scal, h->dV);
+    k<<<grid, NG * GT + 96, sm, h->stream>>>(*map, make_cntab<RT>(h->ax[axis]), tg, h->partial, h->ticket, h->scal, h->dV);
     h->launches++;
     return (int)cudaGetLastError();
 }
@@ -382,7 +385,7 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_SPEC_Y : TM_SPEC_Z];
     const CUtensorMap* mv = (const CUtensorMap*)h->tmap[axis == 1 ? TM_VDD_Y : TM_VDD_Z];
-    k<<<grid, NG * GT + 64, sm, h->stream>>>(*map, *mv, h->ax[axis].twA, h->ax[axis].twN, tg);
+    k<<<grid, NG * GT + 96, sm, h->stream>>>(*map, *mv, h->ax[axis].twA, h->ax[axis].twN, tg);
     h->launches++;
     return (int)cudaGetLastError();
 }

@@ -14,6 +14,7 @@
 #include "cn_chunk.cuh"
 #include "cn_line_smem.cuh"
 #include "tma_pipe.cuh"
+#include "trig.cuh"
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
@@ -35,7 +36,7 @@ __host__ __device__ constexpr int nxhp_of(int n) { return ((n / 2 + 1) + DBEC_SP
 // buffer once they are in registers; after the transform the spectrum area holds the chunk ends of
 // the Thomas carries.
 template <class P, bool RT, int NG, int NST>
-__global__ void __launch_bounds__(NG* XR* P::T + 64, 1)
+__global__ void __launch_bounds__(NG* XR* P::T + 96, 1)
 k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __restrict__ twA_g,
                const cd* __restrict__ twN_g, const double* __restrict__ scal, const double* __restrict__ vx_g,
                const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny,
@@ -43,7 +44,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
     typedef typename CnCoef<RT>::type CT;
     // A group of GT = 8*T threads owns one tile: its first half runs the four pair transforms (T threads
     // per pair), then all of it runs calcnu (T threads per line) and calclux (one 16-point chunk each).
-    constexpr int T = P::T, N = P::N, NCH = N / CN_L, GT = XR * T, NT = NG * GT + 64;
+    constexpr int T = P::T, N = P::N, NCH = N / CN_L, GT = XR * T, NT = NG * GT + 96;
     constexpr int NXHP = nxhp_of(N), PITCH = N + 1;
     constexpr int PSI_BYTES = XR * PITCH * (int)sizeof(cd), SPEC_BYTES = XR * NXHP * (int)sizeof(cd);
     constexpr int STAGE_BYTES = PSI_BYTES + SPEC_BYTES;
@@ -75,12 +76,18 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         const int r = t % XR, c = t / XR;                // calclux: line r, chunk c
         const cd* twA = tw; const cd* twN = tw + N;
         const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
+        // trap potential of this thread's line, V_y + V_z, fetched one tile ahead (global tables)
+        auto vrow_of = [&](int i) {
+            const int row = (int)(row0 + ((long long)blockIdx.x + (long long)i * gridDim.x) * XR) + lp;
+            return vy[row % ny] + vz[row / ny];
+        };
+        double vrow = (g < nmine) ? vrow_of(g) : 0.0;
         for (int i = g; i < nmine; i += NG) {
             const int st = i % NST;
+            const double vrow_next = (i + NG < nmine) ? vrow_of(i + NG) : 0.0;
             mbar_wait(full + st, (i / NST) & 1);
             cd* ps = (cd*)(base + (size_t)st * STAGE_BYTES);
             cd* ss = (cd*)(base + (size_t)st * STAGE_BYTES + PSI_BYTES);
-            const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             // ---- inverse transform of a pair's spectrum: v[j] = (Phi on line a, Phi on line b) at x = j*T + m;
             //      Phi goes back to the pair's spectrum rows as two real lines [2][N]
             if (t < GT / 2) {
@@ -108,18 +115,17 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             named_bar_sync(1 + g, GT);
             // ---- calcnu on line lp
             {
-                const long long row = row0 + tile * XR + lp;
-                const int y = (int)(row % ny), z = (int)(row / ny);
-                const double vrow = vy[y] + vz[z];
                 cd* p = ps + lp * PITCH;
                 const double* ph = (const double*)(ss + (lp >> 1) * 2 * NXHP) + (lp & 1) * N;
-#pragma unroll
+                // four points at a time: enough independent work to cover the fp64 latency, and a quarter of
+                // the code (the kernel must stay inside the instruction cache: the groups run out of phase)
+#pragma unroll 4
                 for (int j = 0; j < 16; ++j) {
                     const cd q = p[j * T + m];
                     const double u = dt * (vxs[j * T + m] + vrow + G * (s2 * cnorm2(q)) + D * ph[j * T + m]);
                     if (RT) {
                         double sn, cs_;
-                        sincos(u, &sn, &cs_);
+                        sincos_cw(u, &sn, &cs_);              // branch-free: the 16 evaluations interleave
                         p[j * T + m] = cmul(s, cmul(q, cmake(cs_, -sn)));
                     } else {
                         p[j * T + m] = cmul(s * exp(-u), q);
@@ -150,6 +156,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             fence_proxy_async();
             __syncwarp();
             if ((tid & 31) == 0) mbar_arrive(done + st);
+            vrow = vrow_next;
         }
     } else if (tid == NG * GT) {
         for (int i = 0; i < nmine; ++i) {
@@ -159,23 +166,26 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             unsigned char* dst = base + (size_t)st * STAGE_BYTES;
             const cd* src = psi + tile * XR * N;
-#pragma unroll
+#pragma unroll 1
             for (int rr = 0; rr < XR; ++rr)
                 bulk_load(dst + (size_t)rr * PITCH * sizeof(cd), src + (size_t)rr * N, N * (int)sizeof(cd), full + st);
             bulk_load(dst + PSI_BYTES, spec + tile * XR * NXHP, SPEC_BYTES, full + st);
         }
-    } else if (tid == NG * GT + 32) {
-        for (int i = 0; i < nmine; ++i) {
+    } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
+        // two storers take alternate tiles: while one sits in wait_group.read (which lasts about as long
+        // as the global write), the other already drains the next finished stage
+        for (int i = (tid - NG * GT) / 32 - 1; i < nmine; i += 2) {
             const int st = i % NST;
             mbar_wait(done + st, (i / NST) & 1);
             const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             const unsigned char* src = base + (size_t)st * STAGE_BYTES;
             cd* dstg = psi + tile * XR * N;
-#pragma unroll
+#pragma unroll 1
             for (int rr = 0; rr < XR; ++rr)
                 bulk_store(dstg + (size_t)rr * N, src + (size_t)rr * PITCH * sizeof(cd), N * (int)sizeof(cd));
             bulk_commit();
-            if (i > 0) { bulk_wait_read<1>(); mbar_arrive(empty + (i - 1) % NST); }
+            bulk_wait_read<0>();
+            mbar_arrive(empty + st);
         }
         bulk_wait<0>();
     }
@@ -201,7 +211,7 @@ template <int N, bool RT, int NG, int NST> static int launch_xline_nonlin(dbec_h
     auto k = k_xline_nonlin<P, RT, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
-    k<<<grid, NG * GT + 64, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
+    k<<<grid, NG * GT + 96, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
                                              h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, row0,
                                              make_cntab<RT>(h->ax[0]));
     h->launches++;
