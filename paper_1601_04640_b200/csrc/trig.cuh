@@ -17,10 +17,30 @@
 
 #define SINCOS_CW_MAX 1.0e14
 
+// Coefficients: on the device they sit in constant memory, so that every DFMA takes its coefficient
+// as a constant-bank operand (as 64-bit immediates they cost two uniform-register moves per use).
+#define SINCOS_CW_COEFS                                                                                   \
+    { 0.63661977236758134 /* 2/pi */, 1.5707963267948966, 6.123233995736766e-17, -1.4973849048591698e-33, \
+      /* sin: -1/15!, 1/13!, -1/11!, 1/9!, -1/7!, 1/5!, -1/3! */                                          \
+      -1.0 / 1307674368000.0, 1.0 / 6227020800.0, -1.0 / 39916800.0, 1.0 / 362880.0, -1.0 / 5040.0,       \
+      1.0 / 120.0, -1.0 / 6.0,                                                                            \
+      /* cos: 1/16!, -1/14!, 1/12!, -1/10!, 1/8!, -1/6!, 1/4!, -1/2! */                                   \
+      1.0 / 20922789888000.0, -1.0 / 87178291200.0, 1.0 / 479001600.0, -1.0 / 3628800.0, 1.0 / 40320.0,   \
+      -1.0 / 720.0, 1.0 / 24.0, -0.5 }
+#if defined(__CUDACC__)
+static __constant__ double sincos_cw_dev[19] = SINCOS_CW_COEFS;
+#endif
+static const double sincos_cw_host[19] = SINCOS_CW_COEFS;
+
 DBEC_HD void sincos_cw(double u, double* sn, double* cs) {
+#if defined(__CUDA_ARCH__)
+    const double* K = sincos_cw_dev;
+#else
+    const double* K = sincos_cw_host;
+#endif
     u = (fabs(u) <= SINCOS_CW_MAX) ? u : (u - u) / (u - u);   // out of range or not finite -> NaN
     const double MAGIC = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to nearest integer
-    const double kb = u * 0.63661977236758134 + MAGIC;
+    const double kb = fma(u, K[0], MAGIC);
     const double kd = kb - MAGIC;
 #if defined(__CUDA_ARCH__)
     const int q = __double2loint(kb);
@@ -28,26 +48,17 @@ DBEC_HD void sincos_cw(double u, double* sn, double* cs) {
     union { double d; unsigned long long u; } cv; cv.d = kb;
     const int q = (int)(unsigned)(cv.u & 0xffffffffull);
 #endif
-    double r = fma(-kd, 1.5707963267948966, u);
-    r = fma(-kd, 6.123233995736766e-17, r);
-    r = fma(-kd, -1.4973849048591698e-33, r);
+    double r = fma(-kd, K[1], u);
+    r = fma(-kd, K[2], r);
+    r = fma(-kd, K[3], r);
     const double r2 = r * r;
-    double ps = -1.0 / 1307674368000.0;                      // -1/15!
-    ps = fma(ps, r2, 1.0 / 6227020800.0);                    //  1/13!
-    ps = fma(ps, r2, -1.0 / 39916800.0);                     // -1/11!
-    ps = fma(ps, r2, 1.0 / 362880.0);                        //  1/9!
-    ps = fma(ps, r2, -1.0 / 5040.0);                         // -1/7!
-    ps = fma(ps, r2, 1.0 / 120.0);                           //  1/5!
-    ps = fma(ps, r2, -1.0 / 6.0);                            // -1/3!
+    double ps = K[4];
+#pragma unroll
+    for (int i = 5; i <= 10; ++i) ps = fma(ps, r2, K[i]);
     const double sr = fma(ps * r2, r, r);
-    double pc = 1.0 / 20922789888000.0;                      //  1/16!
-    pc = fma(pc, r2, -1.0 / 87178291200.0);                  // -1/14!
-    pc = fma(pc, r2, 1.0 / 479001600.0);                     //  1/12!
-    pc = fma(pc, r2, -1.0 / 3628800.0);                      // -1/10!
-    pc = fma(pc, r2, 1.0 / 40320.0);                         //  1/8!
-    pc = fma(pc, r2, -1.0 / 720.0);                          // -1/6!
-    pc = fma(pc, r2, 1.0 / 24.0);                            //  1/4!
-    pc = fma(pc, r2, -0.5);                                  // -1/2!
+    double pc = K[11];
+#pragma unroll
+    for (int i = 12; i <= 18; ++i) pc = fma(pc, r2, K[i]);
     const double cr = fma(pc, r2, 1.0);
     const double a = (q & 1) ? cr : sr;                      // sin u up to sign
     const double b = (q & 1) ? sr : cr;                      // cos u up to sign
