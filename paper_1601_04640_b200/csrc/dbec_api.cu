@@ -159,10 +159,14 @@ static const char* const kernel_names[DBEC_MAX_KERNELS] = {
         }                                                                                        \
     } while (0)
 
-static int launch_fft_pass(dbec_handle h, int axis, int mode) {
+// rev: walk the tiles of a plane-ordered pass last to first, so that it starts on the planes the
+// previous pass has just left (dirty) in the 126 MB L2.
+static int launch_fft_pass(dbec_handle h, int axis, int mode, int rev = 0) {
+    h->rev_next = rev && h->use_rev;
     return dbec_tma_supported(h, axis) ? dbec_launch_fft_tma(h, axis, mode, 0, h->nz) : dbec_launch_fft_strided(h, axis, mode);
 }
-static int launch_cn_pass(dbec_handle h, int axis, int with_norm) {
+static int launch_cn_pass(dbec_handle h, int axis, int with_norm, int rev = 0) {
+    h->rev_next = rev && h->use_rev;
     return (axis > 0 && dbec_tma_supported(h, axis)) ? dbec_launch_cn_tma(h, axis, with_norm, 0, h->nz)
                                                      : dbec_launch_cn(h, axis, with_norm);
 }
@@ -171,7 +175,7 @@ static int launch_cn_pass(dbec_handle h, int axis, int with_norm) {
 static int enqueue_dipolar_spectrum(dbec_handle h) {
     KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
     if (h->p.ndim == 3) {
-        KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0));
+        KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
         KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 2, 2));
         KLAUNCH(h, KS_FFT_Y_INV, launch_fft_pass(h, 1, 1));
     } else {
@@ -186,6 +190,7 @@ static int enqueue_step(dbec_handle h) {
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
     int rc = enqueue_dipolar_spectrum(h);
     if (rc) return rc;
+    h->rev_next = h->use_rev;                                       // inverse y pass went up: come back down
     if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nz));
     else KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
     if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, launch_cn_pass(h, 0, 0));
@@ -259,6 +264,8 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->fuse_cnx = fe ? atoi(fe) : 1;
     const char* ge = getenv("DBEC_GRAPH");
     h->use_graph = ge ? atoi(ge) : 1;
+    const char* re = getenv("DBEC_REV");
+    h->use_rev = re ? atoi(re) : 1;
     const char* te = getenv("DBEC_TMA");
     h->use_tma = te ? atoi(te) : 1;
     // the legacy default stream cannot be captured: plain launches there

@@ -69,6 +69,8 @@ struct dbec_handle_s {
     int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
     int use_tma;                    // env DBEC_TMA (default 1): persistent TMA-fed kernels for lines of 128..512 points
     int num_sms;
+    int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
+    int use_rev;                    // env DBEC_REV (default 1)
     alignas(64) unsigned char tmap[TM_COUNT][DBEC_TMAP_BYTES];
 };
 

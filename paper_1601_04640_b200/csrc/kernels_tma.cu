@@ -26,6 +26,7 @@ struct TileGeom {
     int box_rows;    // rows of one TMA box (<= 256)
     int nbox;        // boxes per tile (N / box_rows)
     int outer0;      // first outer coordinate (slab offset; axis 1 only)
+    int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
 };
 
 struct PipeBars {
@@ -43,6 +44,7 @@ template <int NST> __device__ __forceinline__ PipeBars pipe_init(uint64_t* bars,
 }
 
 __device__ __forceinline__ void tile_coords(const TileGeom& tg, int t, int b, int inner, int& c0, int& c1, int& c2) {
+    if (tg.rev) t = tg.ntiles - 1 - t;
     const int tx = t % tg.ntiles_x, o = t / tg.ntiles_x + tg.outer0;
     c0 = tx * inner;
     c1 = tg.axis == 1 ? b * tg.box_rows : o;
@@ -322,6 +324,7 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
 // ------------------------------------------------------------------------------------------------
 static TileGeom geom_of(const dbec_handle_s* h, int axis, int row_elems, int z0, int nzs) {
     TileGeom tg;
+    tg.rev = h->rev_next;
     tg.axis = axis;
     tg.ntiles_x = row_elems / TCOLS;
     const int n = axis == 1 ? h->ny : h->nz;

@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(NG* XR* P::T + 96, 1)
 k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __restrict__ twA_g,
                const cd* __restrict__ twN_g, const double* __restrict__ scal, const double* __restrict__ vx_g,
                const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny,
-               long long row0, CnTab<RT> cn) {
+               long long row0, CnTab<RT> cn, int rev) {
     typedef typename CnCoef<RT>::type CT;
     // A group of GT = 8*T threads owns one tile: its first half runs the four pair transforms (T threads
     // per pair), then all of it runs calcnu (T threads per line) and calclux (one 16-point chunk each).
@@ -78,7 +78,9 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
         // trap potential of this thread's line, V_y + V_z, fetched one tile ahead (global tables)
         auto vrow_of = [&](int i) {
-            const int row = (int)(row0 + ((long long)blockIdx.x + (long long)i * gridDim.x) * XR) + lp;
+            long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            if (rev) tile = ntiles - 1 - tile;
+            const int row = (int)(row0 + tile * XR) + lp;
             return vy[row % ny] + vz[row / ny];
         };
         double vrow = (g < nmine) ? vrow_of(g) : 0.0;
@@ -163,7 +165,8 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
             mbar_expect_tx(full + st, XR * N * (int)sizeof(cd) + SPEC_BYTES);
-            const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            if (rev) tile = ntiles - 1 - tile;
             unsigned char* dst = base + (size_t)st * STAGE_BYTES;
             const cd* src = psi + tile * XR * N;
 #pragma unroll 1
@@ -177,7 +180,8 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         for (int i = (tid - NG * GT) / 32 - 1; i < nmine; i += 2) {
             const int st = i % NST;
             mbar_wait(done + st, (i / NST) & 1);
-            const long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
+            if (rev) tile = ntiles - 1 - tile;
             const unsigned char* src = base + (size_t)st * STAGE_BYTES;
             cd* dstg = psi + tile * XR * N;
 #pragma unroll 1
@@ -213,7 +217,7 @@ template <int N, bool RT, int NG, int NST> static int launch_xline_nonlin(dbec_h
     const long long row0 = (long long)z0 * h->ny;
     k<<<grid, NG * GT + 96, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
                                              h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, row0,
-                                             make_cntab<RT>(h->ax[0]));
+                                             make_cntab<RT>(h->ax[0]), h->rev_next);
     h->launches++;
     return (int)cudaGetLastError();
 }
