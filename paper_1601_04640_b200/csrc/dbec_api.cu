@@ -152,7 +152,11 @@ static const char* const kernel_names[DBEC_MAX_KERNELS] = {
     do {                                                                                         \
         if ((h)->prof_on) cudaEventRecord((h)->prof_ev[2 * (h)->prof_n], (h)->stream);           \
         int rc_ = (x);                                                                           \
-        if (rc_) return cuda_fail(h, (cudaError_t)rc_);                                          \
+        if (!rc_ && getenv("DBEC_SYNC")) rc_ = (int)cudaStreamSynchronize((h)->stream);          \
+        if (rc_) {                                                                               \
+            if (getenv("DBEC_DEBUG")) fprintf(stderr, "dbec: launch in slot %d (%s) failed: %d\n", (slot), kernel_names[slot], rc_); \
+            return cuda_fail(h, (cudaError_t)rc_);                                               \
+        }                                                                                        \
         if ((h)->prof_on) {                                                                      \
             cudaEventRecord((h)->prof_ev[2 * (h)->prof_n + 1], (h)->stream);                     \
             (h)->prof_slot[(h)->prof_n++] = (slot);                                              \
@@ -173,7 +177,9 @@ static int launch_cn_pass(dbec_handle h, int axis, int with_norm, int rev = 0) {
 
 // calcpsidd2 up to the x-inverse: density -> half spectrum -> x V_dd -> back along z, y.
 static int enqueue_dipolar_spectrum(dbec_handle h) {
-    KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
+    h->rev_next = 0;
+    if (dbec_xline_supported(h) && !getenv("DBEC_NO_XDENS")) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nz));
+    else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
     if (h->p.ndim == 3) {
         KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
         KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 2, 2));

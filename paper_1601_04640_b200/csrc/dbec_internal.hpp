@@ -93,3 +93,4 @@ int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nz
 // persistent bulk-copy-fed versions of the x passes (kernels_xline.cu)
 int dbec_xline_supported(const dbec_handle_s* h);
 int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs);          // a3 (x) + a4 + a5
+int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs);         // a1 (x)

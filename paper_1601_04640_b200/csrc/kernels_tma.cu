@@ -31,11 +31,13 @@ struct TileGeom {
 
 struct PipeBars {
     uint64_t* full; uint64_t* empty; uint64_t* done;
+    int* issued;     // tiles whose loads the loader has issued (tma_pipe.cuh: wait_issued)
 };
 
 template <int NST> __device__ __forceinline__ PipeBars pipe_init(uint64_t* bars, int done_count) {
-    PipeBars b; b.full = bars; b.empty = bars + NST; b.done = bars + 2 * NST;
+    PipeBars b; b.full = bars; b.empty = bars + NST; b.done = bars + 2 * NST; b.issued = (int*)(bars + 3 * NST);
     if (threadIdx.x == 0) {
+        *b.issued = 0;
         for (int s = 0; s < NST; ++s) { mbar_init(b.full + s, 1); mbar_init(b.empty + s, 1); mbar_init(b.done + s, done_count); }
         fence_mbar_init();
     }
@@ -59,6 +61,7 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
     for (int i = 0; i < nmine; ++i) {
         const int s = i % NST;
         if (i >= NST) mbar_wait(pb.empty + s, ((i / NST) - 1) & 1);
+        st_release_shared(pb.issued, i + 1);
         mbar_expect_tx(pb.full + s, MAIN_BYTES + EXTRA_BYTES);
         const int t = blockIdx.x + i * gridDim.x;
         unsigned char* dst = stages + (size_t)s * STAGE_BYTES;
@@ -74,13 +77,15 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
     }
 }
 
-// Two storers take alternate tiles (first = 0 / 1): while one sits in wait_group.read (which lasts about
-// as long as the global write), the other already drains the next finished stage.
+// Two storers, one for the even and one for the odd stages (which = 0 / 1): while one sits in
+// wait_group.read (which lasts about as long as the global write), the other already drains the next
+// finished stage.  A stage always belongs to the same storer, so its done[] phases are seen in order.
 template <int NST, int STAGE_BYTES, int MAIN_BYTES>
 __device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
-                                            const TileGeom& tg, int nmine, int first) {
-    for (int i = first; i < nmine; i += 2) {
+                                            const TileGeom& tg, int nmine, int which) {
+    for (int i = 0; i < nmine; ++i) {
         const int s = i % NST;
+        if ((s & 1) != which) continue;
         mbar_wait(pb.done + s, (i / NST) & 1);
         const int t = blockIdx.x + i * gridDim.x;
         unsigned char* src = stages + (size_t)s * STAGE_BYTES;
@@ -132,7 +137,7 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
     // h / PF / PB (entry k at k + k/16, so that the four chunks a warp works on hit different banks) and
     // the chunk-end products, staged once per CTA: read straight from global memory inside the
     // recurrences every table value costs an exposed L1/L2 round trip
-    CT* tab = (CT*)(bars + ((3 * NST + 1) & ~1));
+    CT* tab = (CT*)(bars + ((3 * NST + 3) & ~1));
     constexpr int E = cn_tab_elems(N);
     const int tid = threadIdx.x;
     CnTab<RT> cs = cn_stage_tables<RT, N>(cn, tab);
@@ -147,6 +152,7 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
         cd* myends = ends + g * 2 * GT;
         for (int i = g; i < nmine; i += NG) {
             const int s = i % NST;
+            wait_issued(pb.issued, i);
             mbar_wait(pb.full + s, (i / NST) & 1);
             cd* t = (cd*)(base + (size_t)s * STAGE_BYTES) + col;
             cd u[CN_L];
@@ -234,7 +240,7 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
     unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
     uint64_t* bars = (uint64_t*)(base + (size_t)NST * STAGE_BYTES);
     // twiddle tables staged once per CTA (2 x N entries)
-    cd* tw = (cd*)(bars + ((3 * NST + 1) & ~1));
+    cd* tw = (cd*)(bars + ((3 * NST + 3) & ~1));
     const int tid = threadIdx.x;
     for (int k = tid; k < N; k += NG * GT + 96) { tw[k] = twA[k]; tw[N + k] = twN[k]; }
     twA = tw; twN = tw + N;
@@ -244,6 +250,7 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
         const int g = tid / GT, r = tid % GT, col = r % TCOLS, m = r / TCOLS;
         for (int i = g; i < nmine; i += NG) {
             const int s = i % NST;
+            wait_issued(pb.issued, i);
             mbar_wait(pb.full + s, (i / NST) & 1);
             cd* sm = (cd*)(base + (size_t)s * STAGE_BYTES) + col;
             cd v[16];
@@ -342,7 +349,7 @@ template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma
     const TileGeom tg = geom_of(h, axis, h->nx, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
     if (NORM && grid > h->npartial) return (int)cudaErrorInvalidValue;
-    const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 1) * sizeof(uint64_t) +
+    const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 4) * sizeof(uint64_t) +
                       (3 * cn_tab_elems(NCH * CN_L) + 2 * NCH) * sizeof(typename CnCoef<RT>::type);
     auto k = k_cn_tma<RT, NCH, NG, NST, NORM>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
@@ -383,7 +390,7 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
     constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? N * TCOLS * (int)sizeof(double) : 0);
     const TileGeom tg = geom_of(h, axis, h->nxhp, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
-    const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 2) * sizeof(uint64_t) + 2 * N * sizeof(cd);
+    const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 4) * sizeof(uint64_t) + 2 * N * sizeof(cd);
     auto k = k_fft_tma<P, MODE, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_SPEC_Y : TM_SPEC_Z];

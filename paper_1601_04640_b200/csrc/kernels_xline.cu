@@ -59,12 +59,14 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
     double* vxs = (double*)(tab + 3 * E + 2 * NCH);              // trap table along x
     uint64_t* bars = (uint64_t*)(vxs + N);
     uint64_t* full = bars; uint64_t* empty = bars + NST; uint64_t* done = bars + 2 * NST;
+    int* issued = (int*)(bars + 3 * NST);
     const int tid = threadIdx.x;
     for (int k = tid; k < N; k += NT) { tw[k] = twA_g[k]; tw[N + k] = twN_g[k]; vxs[k] = vx_g[k]; }
     CnTab<RT> cs = cn_stage_tables<RT, N>(cn, tab);
     for (int k = tid; k < NCH; k += NT) { tab[3 * E + k] = cn.pfe[k]; tab[3 * E + NCH + k] = cn.pbs[k]; }
     cs.pfe = tab + 3 * E; cs.pbs = tab + 3 * E + NCH;
     if (tid == 0) {
+        *issued = 0;
         for (int s = 0; s < NST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); mbar_init(done + s, GT / 32); }
         fence_mbar_init();
     }
@@ -87,6 +89,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         for (int i = g; i < nmine; i += NG) {
             const int st = i % NST;
             const double vrow_next = (i + NG < nmine) ? vrow_of(i + NG) : 0.0;
+            wait_issued(issued, i);
             mbar_wait(full + st, (i / NST) & 1);
             cd* ps = (cd*)(base + (size_t)st * STAGE_BYTES);
             cd* ss = (cd*)(base + (size_t)st * STAGE_BYTES + PSI_BYTES);
@@ -164,6 +167,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            st_release_shared(issued, i + 1);
             mbar_expect_tx(full + st, XR * N * (int)sizeof(cd) + SPEC_BYTES);
             long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             if (rev) tile = ntiles - 1 - tile;
@@ -175,10 +179,12 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             bulk_load(dst + PSI_BYTES, spec + tile * XR * NXHP, SPEC_BYTES, full + st);
         }
     } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
-        // two storers take alternate tiles: while one sits in wait_group.read (which lasts about as long
+        // two storers (even / odd stages): while one sits in wait_group.read (which lasts about as long
         // as the global write), the other already drains the next finished stage
-        for (int i = (tid - NG * GT) / 32 - 1; i < nmine; i += 2) {
+        const int which = (tid - NG * GT) / 32 - 1;      // storer 0: even stages, storer 1: odd stages
+        for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
+            if ((st & 1) != which) continue;
             mbar_wait(done + st, (i / NST) & 1);
             long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             if (rev) tile = ntiles - 1 - tile;
@@ -187,6 +193,106 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
 #pragma unroll 1
             for (int rr = 0; rr < XR; ++rr)
                 bulk_store(dstg + (size_t)rr * N, src + (size_t)rr * PITCH * sizeof(cd), N * (int)sizeof(cd));
+            bulk_commit();
+            bulk_wait_read<0>();
+            mbar_arrive(empty + st);
+        }
+        bulk_wait<0>();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 (x): n = |s psi|^2 -> half spectrum along x
+// ------------------------------------------------------------------------------------------------
+// A stage holds the 8 psi lines of a tile (contiguous, one bulk load).  The T threads of a pair read
+// its two lines into registers, then reuse the pair's 2N-element area: [0, 2*NXHP) FFT exchange, later
+// the pair's two output rows; [N, 2N) the transform Z, of which other threads read only the upper half
+// (the mirror Z[N-k], k = 1..N/2).  One bulk store per pair.
+template <class P, int NG, int NST>
+__global__ void __launch_bounds__(NG* XP* P::T + 96, 1)
+k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA_g,
+                const cd* __restrict__ twN_g, const double* __restrict__ scal, int ntiles, int rev) {
+    constexpr int T = P::T, N = P::N, GT = XP * T, NT = NG * GT + 96;
+    constexpr int NXHP = nxhp_of(N);
+    constexpr int STAGE_BYTES = XR * N * (int)sizeof(cd), PAIR_BYTES = 2 * NXHP * (int)sizeof(cd);
+    static_assert(P::SMEM <= 2 * NXHP && 2 * NXHP <= N + N / 2, "exchange / output rows must stay below Z's upper half");
+    extern __shared__ __align__(1024) unsigned char smraw[];
+    unsigned char* base = smraw;
+    cd* tw = (cd*)(base + (size_t)NST * STAGE_BYTES);
+    uint64_t* bars = (uint64_t*)(tw + 2 * N);
+    uint64_t* full = bars; uint64_t* empty = bars + NST; uint64_t* done = bars + 2 * NST;
+    int* issued = (int*)(bars + 3 * NST);
+    const int tid = threadIdx.x;
+    for (int k = tid; k < N; k += NT) { tw[k] = twA_g[k]; tw[N + k] = twN_g[k]; }
+    if (tid == 0) {
+        *issued = 0;
+        for (int s = 0; s < NST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); mbar_init(done + s, GT / 32); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    const int nmine = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto tile_of = [&](int i) {
+        const long long t = (long long)blockIdx.x + (long long)i * gridDim.x;
+        return rev ? (long long)ntiles - 1 - t : t;
+    };
+    if (tid < NG * GT) {
+        const int g = tid / GT, t = tid % GT, lp = t / T, m = t % T;
+        const cd* twA = tw; const cd* twN = tw + N;
+        const double s2 = scal[SC_S2];
+        for (int i = g; i < nmine; i += NG) {
+            const int st = i % NST;
+            wait_issued(issued, i);
+            mbar_wait(full + st, (i / NST) & 1);
+            cd* pr = (cd*)(base + (size_t)st * STAGE_BYTES) + lp * 2 * N;     // the pair's area
+            cd v[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const cd a = pr[j * T + m], b = pr[N + j * T + m];
+                v[j] = cmake(s2 * cnorm2(a), s2 * cnorm2(b));
+            }
+            __syncwarp();
+            fft_line<P, -1, 0>(v, m, pr, 1, twA, twN);
+            __syncwarp();
+#pragma unroll
+            for (int j = 8; j < 16; ++j) pr[N + j * T + m] = v[j];            // Z[N/2 .. N-1]
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const int k = j * T + m;
+                if (k <= N / 2) {
+                    const cd z = v[j];
+                    const cd zp = (k == 0) ? z : pr[2 * N - k];               // Z[N-k]
+                    // X_a = (Z[k] + conj Z[N-k])/2,  X_b = (Z[k] - conj Z[N-k])/(2i)
+                    pr[k] = cmake(0.5 * (z.x + zp.x), 0.5 * (z.y - zp.y));
+                    pr[NXHP + k] = cmake(0.5 * (z.y + zp.y), -0.5 * (z.x - zp.x));
+                } else if (k < NXHP) {
+                    pr[k] = cmake(0.0, 0.0);
+                    pr[NXHP + k] = cmake(0.0, 0.0);
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(done + st);
+        }
+    } else if (tid == NG * GT) {
+        for (int i = 0; i < nmine; ++i) {
+            const int st = i % NST;
+            if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            st_release_shared(issued, i + 1);
+            mbar_expect_tx(full + st, STAGE_BYTES);
+            bulk_load(base + (size_t)st * STAGE_BYTES, psi + tile_of(i) * XR * N, STAGE_BYTES, full + st);
+        }
+    } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
+        const int which = (tid - NG * GT) / 32 - 1;      // storer 0: even stages, storer 1: odd stages
+        for (int i = 0; i < nmine; ++i) {
+            const int st = i % NST;
+            if ((st & 1) != which) continue;
+            mbar_wait(done + st, (i / NST) & 1);
+            const unsigned char* src = base + (size_t)st * STAGE_BYTES;
+            cd* dstg = spec + tile_of(i) * XR * NXHP;
+#pragma unroll 1
+            for (int pp = 0; pp < XP; ++pp)
+                bulk_store(dstg + (size_t)pp * 2 * NXHP, src + (size_t)pp * 2 * N * sizeof(cd), PAIR_BYTES);
             bulk_commit();
             bulk_wait_read<0>();
             mbar_arrive(empty + st);
@@ -211,7 +317,7 @@ template <int N, bool RT, int NG, int NST> static int launch_xline_nonlin(dbec_h
     const int ntiles = (int)((long long)h->ny * nzs / XR);
     const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
     const size_t sm = 128 + (size_t)NST * STAGE + 2 * N * sizeof(cd) + (3 * cn_tab_elems(N) + 2 * (N / CN_L)) * sizeof(CT) +
-                      N * sizeof(double) + 3 * NST * sizeof(uint64_t);
+                      N * sizeof(double) + (3 * NST + 1) * sizeof(uint64_t);
     auto k = k_xline_nonlin<P, RT, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
@@ -227,6 +333,30 @@ int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
     switch (h->nx) {
         case 128: return rt ? launch_xline_nonlin<128, true, 4, 8>(h, z0, nzs) : launch_xline_nonlin<128, false, 4, 8>(h, z0, nzs);
         case 256: return rt ? launch_xline_nonlin<256, true, 3, 4>(h, z0, nzs) : launch_xline_nonlin<256, false, 3, 4>(h, z0, nzs);
+        default: return (int)cudaErrorInvalidValue;
+    }
+}
+
+template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s* h, int z0, int nzs) {
+    typedef typename XPlan<N>::P P;
+    constexpr int GT = XP * P::T, NXHP = nxhp_of(N);
+    if (h->nxhp != NXHP) return (int)cudaErrorInvalidValue;
+    const int ntiles = (int)((long long)h->ny * nzs / XR);
+    const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
+    const size_t sm = (size_t)NST * XR * N * sizeof(cd) + 2 * N * sizeof(cd) + (3 * NST + 1) * sizeof(uint64_t);
+    auto k = k_xline_density<P, NG, NST>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const long long row0 = (long long)z0 * h->ny;
+    k<<<grid, NG * GT + 96, sm, h->stream>>>(h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
+                                             ntiles, h->rev_next);
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs) {
+    switch (h->nx) {
+        case 128: return launch_xline_density<128, 4, 12>(h, z0, nzs);
+        case 256: return launch_xline_density<256, 4, 6>(h, z0, nzs);
         default: return (int)cudaErrorInvalidValue;
     }
 }

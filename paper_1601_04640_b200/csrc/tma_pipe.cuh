@@ -5,8 +5,9 @@
 // Pattern (every persistent kernel in kernels_tma.cu / kernels_xline.cu):
 //   loader thread   waits empty[s], arms full[s] with the tile's byte count, issues the TMA loads
 //   worker groups   wait full[s], transform the tile in shared memory, fence.proxy.async, arrive done[s]
-//   storer thread   waits done[s], issues the TMA store, and frees the stage (arrive empty[s]) once
-//                   the store has finished READING shared memory (cp.async.bulk.wait_group.read)
+//   storer threads  (two: even / odd stages) wait done[s], issue the TMA store, and free the stage
+//                   (arrive empty[s]) once the store has finished READING shared memory
+//                   (cp.async.bulk.wait_group.read); a stage always belongs to the same storer
 // so that global loads, arithmetic and global stores of different tiles overlap inside one CTA.
 #pragma once
 #include <cuda.h>
@@ -37,6 +38,23 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {}
+}
+
+// ---- loader -> workers: number of tiles whose loads have been issued ----
+// A worker may only wait on full[s] for the k-th use of stage s once the (k-1)-th use has landed:
+// mbarrier waits test a phase PARITY, so a worker that runs a whole ring ahead of its stage would
+// otherwise see the parity of an older, completed phase and walk into a stage that is still in use.
+// The loader publishes its tile counter after it has passed empty[s]; workers check it first.
+__device__ __forceinline__ int ld_acquire_shared(const int* p) {
+    int v;
+    asm volatile("ld.acquire.cta.shared::cta.b32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_shared(int* p, int v) {
+    asm volatile("st.release.cta.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void wait_issued(const int* issued, int i) {
+    while (ld_acquire_shared(issued) <= i) __nanosleep(64);
 }
 
 // generic-proxy writes to shared memory become visible to the async proxy (TMA store reads them)
