@@ -38,17 +38,17 @@ from paper_1601_04640_b200.inputs import initial_psi, workload  # noqa: E402
 METRIC = "grid_point_updates_per_s"
 UNIT = "updates/s"
 
-# Algorithmic bytes per grid point per launch of each kernel (
-# SURVEY.md §8(d)).  The half spectrum is half a complex value per grid point.
+# Algorithmic bytes per grid point per launch of each pass (
+# SURVEY.md §8(d)).  The half spectrum is half a complex value per grid point.  Keys = dbec_kernel_name.
 ALG_BYTES_PER_POINT = {
-    "k_density_fftx": 16 + 8,
-    "k_fft_strided<y,fwd>": 8 + 8,
-    "k_fft_strided<last,fwd*Vdd*inv>": 8 + 8,
-    "k_fft_strided<y,inv>": 8 + 8,
-    "k_ifftx_nonlin": 8 + 16 + 16,
-    "k_cn_x": 32,
-    "k_cn_strided<y>": 32,
-    "k_cn_strided<z>": 32,
+    "density+fft_x": 16 + 8,
+    "fft_y<fwd>": 8 + 8,
+    "fft_last<fwd*Vdd*inv>": 8 + 8,          # the V_dd table (4 B/pt) is not counted as useful traffic
+    "fft_y<inv>": 8 + 8,
+    "ifft_x+calcnu+cn_x": 8 + 16 + 16,
+    "cn_x": 32,
+    "cn_y": 32,
+    "cn_z": 32,
 }
 MODEL_BYTES_PER_POINT = {3: 208, 2: 144}    # SURVEY.md §8(d) "Model M": fixed reference accounting
 
@@ -270,24 +270,29 @@ def run_ours(args, w):
         prof = sim.step_profile(prof_steps)
         peak, peak_src = measured_peaks()
         per_kernel = {}
+        kernels = sim.pass_kernels()
         for name, (tot_ms, cnt) in prof.items():
             avg_ms = tot_ms / cnt
             gbs = ALG_BYTES_PER_POINT[name] * w.npoints / (avg_ms * 1e-3) / 1e9
-            per_kernel[name] = {"ms": avg_ms, "alg_GBps": gbs, "frac": gbs / peak}
+            per_kernel[name] = {"kernel": kernels.get(name, ""), "ms": avg_ms, "alg_GBps": gbs, "frac": gbs / peak}
         top = max(per_kernel, key=lambda k: per_kernel[k]["ms"])
         step_ms_prof = sum(v["ms"] for v in per_kernel.values())
         model = MODEL_BYTES_PER_POINT[w.ndim]
         model_gbs = model * w.npoints / (ms / args.steps * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": top, "achieved": per_kernel[top]["alg_GBps"], "peak": peak,
+        roofline = {"bound": "hbm", "kernel": kernels.get(top, top), "pass": top, "achieved": per_kernel[top]["alg_GBps"], "peak": peak,
                     "unit": "GB/s", "frac": per_kernel[top]["frac"], "traffic": None, "peak_source": peak_src,
                     "kernel_ms": per_kernel[top]["ms"], "kernel_share_of_step": per_kernel[top]["ms"] / step_ms_prof,
                     "alg_bytes_per_launch": ALG_BYTES_PER_POINT[top] * w.npoints,
                     "per_kernel": per_kernel,
                     "step_model": {"bytes_per_point": model, "achieved_GBps": model_gbs, "frac": model_gbs / peak}}
-        tr = os.path.join(ROOT, "profiles", "traffic.json")
+        tr = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram__bytes_{read,write}.sum per launch
         if os.path.exists(tr):
+            import csv
             with open(tr) as f:
-                roofline["traffic"] = json.load(f).get(w.name, {}).get(top)
+                for row in csv.DictReader(f):
+                    if row["workload"] == w.name and row["pass"] == top:
+                        roofline["traffic"] = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+                        roofline["traffic_source"] = row["source"]
 
         # ---- CPU baseline: the oracle on this box's cores, bounded sample ----
         cpu = None

@@ -122,6 +122,10 @@ int dbec_launch_count(dbec_handle h, long long* launches);
 #define DBEC_KERNEL_SLOTS 8
 int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long* launches_per_slot);
 const char* dbec_kernel_name(int slot);
+/* Name of the __global__ function that serves pass `slot` on this handle ("" if the pass is not part
+ * of this handle's step): grid lines of 128..512 points run in the persistent TMA-fed kernels,
+ * shorter ones in the one-tile-per-block kernels. */
+const char* dbec_pass_kernel(dbec_handle h, int slot);
 
 int dbec_version(void);
 

@@ -145,8 +145,8 @@ static int write_scalars(dbec_handle h, bool reset_scale) {
 // Kernel slots of one step (dbec_step_profile / dbec_kernel_name).
 enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z };
 static const char* const kernel_names[DBEC_MAX_KERNELS] = {
-    "k_density_fftx", "k_fft_strided<y,fwd>", "k_fft_strided<last,fwd*Vdd*inv>", "k_fft_strided<y,inv>",
-    "k_ifftx_nonlin", "k_cn_x", "k_cn_strided<y>", "k_cn_strided<z>"};
+    "density+fft_x", "fft_y<fwd>", "fft_last<fwd*Vdd*inv>", "fft_y<inv>",
+    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z"};
 
 #define KLAUNCH(h, slot, x)                                                                      \
     do {                                                                                         \
@@ -178,7 +178,7 @@ static int launch_cn_pass(dbec_handle h, int axis, int with_norm, int rev = 0) {
 // calcpsidd2 up to the x-inverse: density -> half spectrum -> x V_dd -> back along z, y.
 static int enqueue_dipolar_spectrum(dbec_handle h) {
     h->rev_next = 0;
-    if (dbec_xline_supported(h) && !getenv("DBEC_NO_XDENS")) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nz));
+    if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nz));
     else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
     if (h->p.ndim == 3) {
         KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
@@ -435,6 +435,24 @@ int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long*
 
 const char* dbec_kernel_name(int slot) {
     return (slot >= 0 && slot < DBEC_MAX_KERNELS) ? kernel_names[slot] : "";
+}
+
+// Which __global__ function serves a pass on this handle (lines of 128..512 points go to the
+// persistent TMA / bulk-copy kernels, shorter ones to the one-tile-per-block kernels).
+const char* dbec_pass_kernel(dbec_handle h, int slot) {
+    if (!h || slot < 0 || slot >= DBEC_MAX_KERNELS) return "";
+    const int last_axis = h->p.ndim == 3 ? 2 : 1;
+    switch (slot) {
+        case KS_DENS_FFTX: return dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
+        case KS_FFT_Y_FWD: case KS_FFT_Y_INV:
+            return h->p.ndim == 3 ? (dbec_tma_supported(h, 1) ? "k_fft_tma" : "k_fft_strided") : "";
+        case KS_FFT_LAST_FMI: return dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
+        case KS_IFFTX_NONLIN: return (h->fuse_cnx && dbec_xline_supported(h)) ? "k_xline_nonlin" : "k_ifftx_nonlin";
+        case KS_CN_X: return h->fuse_cnx ? "" : "k_cn_x";
+        case KS_CN_Y: return dbec_tma_supported(h, 1) ? "k_cn_tma" : "k_cn_strided";
+        case KS_CN_Z: return h->p.ndim == 3 ? (dbec_tma_supported(h, 2) ? "k_cn_tma" : "k_cn_strided") : "";
+    }
+    return "";
 }
 
 int dbec_launch_count(dbec_handle h, long long* launches) {

@@ -21,7 +21,7 @@ DBEC_OK, DBEC_EINVAL, DBEC_ESIZE, DBEC_EWORKSPACE, DBEC_ECUDA, DBEC_ENODEVICE = 
 EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi", "dbec_set_coupling",
            "dbec_step", "dbec_observables", "dbec_destroy", "dbec_strerror", "dbec_last_cuda_error",
            "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
-           "dbec_version", "dbec_step_profile", "dbec_kernel_name"]
+           "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel"]
 KERNEL_SLOTS = 8
 
 
@@ -83,6 +83,8 @@ def lib():
         L.dbec_step_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.dbec_kernel_name.argtypes = [C.c_int]
         L.dbec_kernel_name.restype = C.c_char_p
+        L.dbec_pass_kernel.argtypes = [vp, C.c_int]
+        L.dbec_pass_kernel.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -216,6 +218,15 @@ class Dbec:
         cnt = (C.c_longlong * KERNEL_SLOTS)()
         self._ck(lib().dbec_step_profile(self._h, int(n), ms, cnt), "dbec_step_profile")
         return {lib().dbec_kernel_name(i).decode(): (ms[i], cnt[i]) for i in range(KERNEL_SLOTS) if cnt[i]}
+
+    def pass_kernels(self) -> dict:
+        """{pass name: __global__ function serving it on this handle}."""
+        out = {}
+        for i in range(KERNEL_SLOTS):
+            k = lib().dbec_pass_kernel(self._h, i).decode()
+            if k:
+                out[lib().dbec_kernel_name(i).decode()] = k
+        return out
 
     def synchronize(self):
         self.stream.synchronize()
