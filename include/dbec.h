@@ -119,7 +119,7 @@ int dbec_launch_count(dbec_handle h, long long* launches);
  * around every kernel.  ms_per_slot: HOST pointer to DBEC_KERNEL_SLOTS doubles receiving the total
  * milliseconds spent in each kernel slot over the nsteps steps; launches_per_slot: HOST pointer to
  * DBEC_KERNEL_SLOTS counts.  Synchronises the stream.  Slot names from dbec_kernel_name. */
-#define DBEC_KERNEL_SLOTS 8
+#define DBEC_KERNEL_SLOTS 9
 int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long* launches_per_slot);
 const char* dbec_kernel_name(int slot);
 /* Name of the __global__ function that serves pass `slot` on this handle ("" if the pass is not part

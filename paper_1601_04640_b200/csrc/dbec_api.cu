@@ -33,7 +33,7 @@ static int check_params(const dbec_params* p) {
 
 // ---- workspace layout: one pass computes the offsets, used by both sizing and create ----
 struct Layout {
-    size_t psi, spec, vdd, phi, scal, partial, ticket, obs, tables, total;
+    size_t psi, spec, vdd, phi, scal, partial, ticket, sync, obs, tables, total;
     size_t tab_bytes;
 };
 static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -61,6 +61,7 @@ static void make_layout(const dbec_params* p, Layout* L) {
     L->scal = o;    o += up256(SC_COUNT * sizeof(double));
     L->partial = o; o += up256(NPARTIAL * sizeof(double));
     L->ticket = o;  o += 256;
+    L->sync = o;    o += 1024;
     L->obs = o;     o += 256;
     L->tables = o;
     L->tab_bytes = axis_table_bytes(p->nx) + axis_table_bytes(p->ny) + axis_table_bytes(p->nz);
@@ -143,10 +144,10 @@ static int write_scalars(dbec_handle h, bool reset_scale) {
 }
 
 // Kernel slots of one step (dbec_step_profile / dbec_kernel_name).
-enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z };
+enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z, KS_FFT_SPECTRAL };
 static const char* const kernel_names[DBEC_MAX_KERNELS] = {
     "density+fft_x", "fft_y<fwd>", "fft_last<fwd*Vdd*inv>", "fft_y<inv>",
-    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z"};
+    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z", "fft_y<fwd>+fft_z<fwd*Vdd*inv>+fft_y<inv>"};
 
 #define KLAUNCH(h, slot, x)                                                                      \
     do {                                                                                         \
@@ -180,7 +181,9 @@ static int enqueue_dipolar_spectrum(dbec_handle h) {
     h->rev_next = 0;
     if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nz));
     else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
-    if (h->p.ndim == 3) {
+    if (dbec_spectral_supported(h)) {
+        KLAUNCH(h, KS_FFT_SPECTRAL, dbec_launch_fft_spectral(h));
+    } else if (h->p.ndim == 3) {
         KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
         KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 2, 2));
         KLAUNCH(h, KS_FFT_Y_INV, launch_fft_pass(h, 1, 1));
@@ -264,6 +267,7 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->scal = (double*)(w + L.scal);
     h->partial = (double*)(w + L.partial);
     h->ticket = (unsigned int*)(w + L.ticket);
+    h->sync = (int*)(w + L.sync);
     h->obs_dev = (double*)(w + L.obs);
     h->npartial = NPARTIAL;
     const char* fe = getenv("DBEC_FUSE_CNX");
@@ -272,6 +276,14 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->use_graph = ge ? atoi(ge) : 1;
     const char* re = getenv("DBEC_REV");
     h->use_rev = re ? atoi(re) : 1;
+    const char* se = getenv("DBEC_SPECTRAL");
+    h->use_spectral = se ? atoi(se) : 0;
+    const char* xe = getenv("DBEC_SPEC_XG");
+    h->spec_xg = xe ? atoi(xe) : 1;
+    if (h->spec_xg < 1) h->spec_xg = 1;
+    const char* le = getenv("DBEC_SPEC_LAG");
+    h->spec_lag = le ? atoi(le) : 2;
+    if (h->spec_lag < 1) h->spec_lag = 1;
     const char* te = getenv("DBEC_TMA");
     h->use_tma = te ? atoi(te) : 1;
     // the legacy default stream cannot be captured: plain launches there
@@ -444,9 +456,12 @@ const char* dbec_pass_kernel(dbec_handle h, int slot) {
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
     switch (slot) {
         case KS_DENS_FFTX: return dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
+        case KS_FFT_SPECTRAL: return dbec_spectral_supported(h) ? "k_fft_spectral" : "";
         case KS_FFT_Y_FWD: case KS_FFT_Y_INV:
+            if (dbec_spectral_supported(h)) return "";
             return h->p.ndim == 3 ? (dbec_tma_supported(h, 1) ? "k_fft_tma" : "k_fft_strided") : "";
-        case KS_FFT_LAST_FMI: return dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
+        case KS_FFT_LAST_FMI: if (dbec_spectral_supported(h)) return "";
+            return dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
         case KS_IFFTX_NONLIN: return (h->fuse_cnx && dbec_xline_supported(h)) ? "k_xline_nonlin" : "k_ifftx_nonlin";
         case KS_CN_X: return h->fuse_cnx ? "" : "k_cn_x";
         case KS_CN_Y: return dbec_tma_supported(h, 1) ? "k_cn_tma" : "k_cn_strided";

@@ -22,7 +22,7 @@ EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi"
            "dbec_step", "dbec_observables", "dbec_destroy", "dbec_strerror", "dbec_last_cuda_error",
            "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
            "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel"]
-KERNEL_SLOTS = 8
+KERNEL_SLOTS = 9
 
 
 class DbecParams(C.Structure):

@@ -204,6 +204,28 @@ def test_persistent_kernels_are_bit_reproducible(gp, shape, mode):
     sim.close()
 
 
+@pytest.mark.parametrize("n", [128, 256])
+def test_single_kernel_spectral_passes_agree(gp, monkeypatch, n):
+    """DBEC_SPECTRAL=1 runs forward-y, forward-z * V_dd * inverse-z and inverse-y as ONE persistent kernel
+    whose CTAs hand blocks of tiles to one another through global counters (k_fft_spectral); the
+    arithmetic per line is the same up to the compiler's choice of FMA contraction: Phi_dd and psi must
+    agree with the three-kernel result to round-off, and two runs of the single kernel bit for bit."""
+    w = grid3(n, n, n, REAL, dx=0.1)
+    psi0 = random_psi(w, seed=9)
+    outs = []
+    for flag in ("0", "1", "1"):
+        monkeypatch.setenv("DBEC_SPECTRAL", flag)
+        sim = gp.Dbec(gp.params_of(w))
+        assert ("k_fft_spectral" in sim.pass_kernels().values()) == (flag == "1")
+        sim.set_psi(psi0)
+        outs.append(sim.phi_dd().cpu().numpy().copy())
+        sim.step(2)
+        outs.append(sim.get_psi().copy())
+        sim.close()
+    assert relerr(outs[2], outs[0]) < 1e-14 and relerr(outs[3], outs[1]) < 1e-14
+    assert np.array_equal(outs[2], outs[4]) and np.array_equal(outs[3], outs[5])
+
+
 def test_full_run_C1_observables(gp, ob):
     w = workload("C1")
     psi0 = initial_psi(w)
