@@ -18,12 +18,11 @@
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
-constexpr int XP = 4;            // line pairs per tile
-constexpr int XR = 2 * XP;       // grid lines per tile
-
+// XP line pairs (XR = 2 XP grid lines) per tile: 4 pairs up to 256 points, 2 pairs of 512 points
 template <int N> struct XPlan;
-template <> struct XPlan<128> { typedef FftPlan<8, 1, true> P; };
-template <> struct XPlan<256> { typedef FftPlan<16, 1, true> P; };
+template <> struct XPlan<128> { typedef FftPlan<8, 1, true> P;  static constexpr int XP = 4; };
+template <> struct XPlan<256> { typedef FftPlan<16, 1, true> P; static constexpr int XP = 4; };
+template <> struct XPlan<512> { typedef FftPlan<16, 2, true> P; static constexpr int XP = 2; };
 
 __host__ __device__ constexpr int nxhp_of(int n) { return ((n / 2 + 1) + DBEC_SPEC_COLS - 1) / DBEC_SPEC_COLS * DBEC_SPEC_COLS; }
 
@@ -35,8 +34,8 @@ __host__ __device__ constexpr int nxhp_of(int n) { return ((n / 2 + 1) + DBEC_SP
 // 8 half-spectrum rows.  A pair's two spectrum rows (2*NXHP elements) double as its FFT exchange
 // buffer once they are in registers; after the transform the spectrum area holds the chunk ends of
 // the Thomas carries.
-template <class P, bool RT, int NG, int NST>
-__global__ void __launch_bounds__(NG* XR* P::T + 96, 1)
+template <class P, int XP, bool RT, int NG, int NST>
+__global__ void __launch_bounds__(NG * 2 * XP * P::T + 96, 1)
 k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __restrict__ twA_g,
                const cd* __restrict__ twN_g, const double* __restrict__ scal, const double* __restrict__ vx_g,
                const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny,
@@ -44,14 +43,16 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
     typedef typename CnCoef<RT>::type CT;
     // A group of GT = 8*T threads owns one tile: its first half runs the four pair transforms (T threads
     // per pair), then all of it runs calcnu (T threads per line) and calclux (one 16-point chunk each).
+    constexpr int XR = 2 * XP;
     constexpr int T = P::T, N = P::N, NCH = N / CN_L, GT = XR * T, NT = NG * GT + 96;
     constexpr int NXHP = nxhp_of(N), PITCH = N + 1;
-    constexpr int PSI_BYTES = XR * PITCH * (int)sizeof(cd), SPEC_BYTES = XR * NXHP * (int)sizeof(cd);
+    // a pair's area: its two spectrum rows, later its FFT exchange, later Phi as two real lines
+    constexpr int SPP = (P::SMEM > 2 * NXHP) ? P::SMEM : 2 * NXHP;
+    constexpr int PSI_BYTES = XR * PITCH * (int)sizeof(cd), SPEC_BYTES = XP * SPP * (int)sizeof(cd);
     constexpr int STAGE_BYTES = PSI_BYTES + SPEC_BYTES;
     constexpr int E = cn_tab_elems(N);
     static_assert(NCH == T, "one chunk per thread of a line");
-    static_assert(P::SMEM <= 2 * NXHP, "a pair's spectrum rows must hold its FFT exchange");
-    static_assert(2 * NCH * XR <= XR * NXHP, "chunk ends must fit the spectrum area");
+    static_assert(2 * NCH * XR <= XP * SPP, "chunk ends must fit the spectrum area");
     extern __shared__ __align__(1024) unsigned char smraw[];
     unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
     cd* tw = (cd*)(base + (size_t)NST * STAGE_BYTES);            // twA [N], twN [N]
@@ -96,7 +97,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             // ---- inverse transform of a pair's spectrum: v[j] = (Phi on line a, Phi on line b) at x = j*T + m;
             //      Phi goes back to the pair's spectrum rows as two real lines [2][N]
             if (t < GT / 2) {
-                cd* sa = ss + (2 * lp) * NXHP;
+                cd* sa = ss + lp * SPP;
                 const cd* sb = sa + NXHP;
                 cd v[16];
 #pragma unroll
@@ -121,7 +122,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             // ---- calcnu on line lp
             {
                 cd* p = ps + lp * PITCH;
-                const double* ph = (const double*)(ss + (lp >> 1) * 2 * NXHP) + (lp & 1) * N;
+                const double* ph = (const double*)(ss + (lp >> 1) * SPP) + (lp & 1) * N;
                 // four points at a time: enough independent work to cover the fp64 latency, and a quarter of
                 // the code (the kernel must stay inside the instruction cache: the groups run out of phase)
 #pragma unroll 4
@@ -168,7 +169,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
             st_release_shared(issued, i + 1);
-            mbar_expect_tx(full + st, XR * N * (int)sizeof(cd) + SPEC_BYTES);
+            mbar_expect_tx(full + st, XR * N * (int)sizeof(cd) + XR * NXHP * (int)sizeof(cd));
             long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             if (rev) tile = ntiles - 1 - tile;
             unsigned char* dst = base + (size_t)st * STAGE_BYTES;
@@ -176,7 +177,10 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
 #pragma unroll 1
             for (int rr = 0; rr < XR; ++rr)
                 bulk_load(dst + (size_t)rr * PITCH * sizeof(cd), src + (size_t)rr * N, N * (int)sizeof(cd), full + st);
-            bulk_load(dst + PSI_BYTES, spec + tile * XR * NXHP, SPEC_BYTES, full + st);
+#pragma unroll 1
+            for (int pp = 0; pp < XP; ++pp)
+                bulk_load(dst + PSI_BYTES + (size_t)pp * SPP * sizeof(cd), spec + (tile * XP + pp) * 2 * NXHP,
+                          2 * NXHP * (int)sizeof(cd), full + st);
         }
     } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
         // two storers (even / odd stages): while one sits in wait_group.read (which lasts about as long
@@ -208,14 +212,15 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
 // its two lines into registers, then reuse the pair's 2N-element area: [0, 2*NXHP) FFT exchange, later
 // the pair's two output rows; [N, 2N) the transform Z, of which other threads read only the upper half
 // (the mirror Z[N-k], k = 1..N/2).  One bulk store per pair.
-template <class P, int NG, int NST>
+template <class P, int XP, int NG, int NST>
 __global__ void __launch_bounds__(NG* XP* P::T + 96, 1)
 k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA_g,
                 const cd* __restrict__ twN_g, const double* __restrict__ scal, int ntiles, int rev) {
+    constexpr int XR = 2 * XP;
     constexpr int T = P::T, N = P::N, GT = XP * T, NT = NG * GT + 96;
     constexpr int NXHP = nxhp_of(N);
     constexpr int STAGE_BYTES = XR * N * (int)sizeof(cd), PAIR_BYTES = 2 * NXHP * (int)sizeof(cd);
-    static_assert(P::SMEM <= 2 * NXHP && 2 * NXHP <= N + N / 2, "exchange / output rows must stay below Z's upper half");
+    static_assert(P::SMEM <= N + N / 2 && 2 * NXHP <= N + N / 2, "exchange / output rows must stay below Z's upper half");
     extern __shared__ __align__(1024) unsigned char smraw[];
     unsigned char* base = smraw;
     cd* tw = (cd*)(base + (size_t)NST * STAGE_BYTES);
@@ -305,20 +310,22 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
 // launchers
 // ------------------------------------------------------------------------------------------------
 int dbec_xline_supported(const dbec_handle_s* h) {
-    return h->use_tma && (h->nx == 128 || h->nx == 256) && ((h->ny * h->nz) % XR == 0);
+    return h->use_tma && (h->nx == 128 || h->nx == 256 || h->nx == 512) && ((h->ny * h->nz) % 8 == 0);
 }
 
 template <int N, bool RT, int NG, int NST> static int launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
     typedef typename XPlan<N>::P P;
     typedef typename CnCoef<RT>::type CT;
+    constexpr int XP = XPlan<N>::XP, XR = 2 * XP;
     constexpr int GT = XR * P::T, NXHP = nxhp_of(N);
-    constexpr int STAGE = XR * (N + 1) * (int)sizeof(cd) + XR * NXHP * (int)sizeof(cd);
+    constexpr int SPP = (P::SMEM > 2 * NXHP) ? P::SMEM : 2 * NXHP;
+    constexpr int STAGE = XR * (N + 1) * (int)sizeof(cd) + XP * SPP * (int)sizeof(cd);
     if (h->nxhp != NXHP) return (int)cudaErrorInvalidValue;
     const int ntiles = (int)((long long)h->ny * nzs / XR);
     const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
-    const size_t sm = 128 + (size_t)NST * STAGE + 2 * N * sizeof(cd) + (3 * cn_tab_elems(N) + 2 * (N / CN_L)) * sizeof(CT) +
+    const size_t sm = (size_t)NST * STAGE + 2 * N * sizeof(cd) + (3 * cn_tab_elems(N) + 2 * (N / CN_L)) * sizeof(CT) +
                       N * sizeof(double) + (3 * NST + 1) * sizeof(uint64_t);
-    auto k = k_xline_nonlin<P, RT, NG, NST>;
+    auto k = k_xline_nonlin<P, XP, RT, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
     k<<<grid, NG * GT + 96, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
@@ -333,18 +340,20 @@ int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
     switch (h->nx) {
         case 128: return rt ? launch_xline_nonlin<128, true, 4, 8>(h, z0, nzs) : launch_xline_nonlin<128, false, 4, 8>(h, z0, nzs);
         case 256: return rt ? launch_xline_nonlin<256, true, 3, 4>(h, z0, nzs) : launch_xline_nonlin<256, false, 3, 4>(h, z0, nzs);
+        case 512: return rt ? launch_xline_nonlin<512, true, 2, 3>(h, z0, nzs) : launch_xline_nonlin<512, false, 2, 3>(h, z0, nzs);
         default: return (int)cudaErrorInvalidValue;
     }
 }
 
 template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s* h, int z0, int nzs) {
     typedef typename XPlan<N>::P P;
+    constexpr int XP = XPlan<N>::XP, XR = 2 * XP;
     constexpr int GT = XP * P::T, NXHP = nxhp_of(N);
     if (h->nxhp != NXHP) return (int)cudaErrorInvalidValue;
     const int ntiles = (int)((long long)h->ny * nzs / XR);
     const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
     const size_t sm = (size_t)NST * XR * N * sizeof(cd) + 2 * N * sizeof(cd) + (3 * NST + 1) * sizeof(uint64_t);
-    auto k = k_xline_density<P, NG, NST>;
+    auto k = k_xline_density<P, XP, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
     k<<<grid, NG * GT + 96, sm, h->stream>>>(h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
@@ -357,6 +366,7 @@ int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs) {
     switch (h->nx) {
         case 128: return launch_xline_density<128, 4, 12>(h, z0, nzs);
         case 256: return launch_xline_density<256, 4, 6>(h, z0, nzs);
+        case 512: return launch_xline_density<512, 4, 6>(h, z0, nzs);
         default: return (int)cudaErrorInvalidValue;
     }
 }
