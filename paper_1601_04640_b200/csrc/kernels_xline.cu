@@ -62,7 +62,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
     uint64_t* full = bars; uint64_t* empty = bars + NST; uint64_t* done = bars + 2 * NST;
     int* issued = (int*)(bars + 3 * NST);
     const int tid = threadIdx.x;
-    for (int k = tid; k < N; k += NT) { tw[k] = twA_g[k]; tw[N + k] = twN_g[k]; vxs[k] = vx_g[k]; }
+    for (int k = tid; k < N; k += NT) { tw[k] = twA_g[k]; tw[N + k] = twN_g[k]; vxs[k] = dt * vx_g[k]; }
     CnTab<RT> cs = cn_stage_tables<RT, N>(cn, tab);
     for (int k = tid; k < NCH; k += NT) { tab[3 * E + k] = cn.pfe[k]; tab[3 * E + NCH + k] = cn.pbs[k]; }
     cs.pfe = tab + 3 * E; cs.pbs = tab + 3 * E + NCH;
@@ -78,13 +78,14 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         const int lp = t / T, m = t % T;                 // transform: pair lp (t < GT/2); calcnu: line lp, x = j*T + m
         const int r = t % XR, c = t / XR;                // calclux: line r, chunk c
         const cd* twA = tw; const cd* twN = tw + N;
-        const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
+        const double s = scal[SC_S];
+        const double dtG = dt * (scal[SC_G] * scal[SC_S2]), dtD = dt * scal[SC_D];   // u = dt V + dtG |q|^2 + dtD Phi
         // trap potential of this thread's line, V_y + V_z, fetched one tile ahead (global tables)
         auto vrow_of = [&](int i) {
             long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             if (rev) tile = ntiles - 1 - tile;
             const int row = (int)(row0 + tile * XR) + lp;
-            return vy[row % ny] + vz[row / ny];
+            return dt * (vy[row % ny] + vz[row / ny]);
         };
         double vrow = (g < nmine) ? vrow_of(g) : 0.0;
         for (int i = g; i < nmine; i += NG) {
@@ -128,7 +129,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
 #pragma unroll 4
                 for (int j = 0; j < 16; ++j) {
                     const cd q = p[j * T + m];
-                    const double u = dt * (vxs[j * T + m] + vrow + G * (s2 * cnorm2(q)) + D * ph[j * T + m]);
+                    const double u = fma(dtG, cnorm2(q), fma(dtD, ph[j * T + m], vxs[j * T + m] + vrow));
                     if (RT) {
                         double sn, cs_;
                         sincos_cw(u, &sn, &cs_);              // branch-free: the 16 evaluations interleave
