@@ -16,6 +16,8 @@
 #include "tma_pipe.cuh"
 #include "trig.cuh"
 
+// calcnu: points evaluated side by side (2, 4 and 8 measure the same; 4 keeps the code small)
+constexpr int NLU_C = 4;
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
 // XP line pairs (XR = 2 XP grid lines) per tile: 4 pairs up to 256 points, 2 pairs of 512 points
@@ -126,7 +128,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
                 const double* ph = (const double*)(ss + (lp >> 1) * SPP) + (lp & 1) * N;
                 // four points at a time: enough independent work to cover the fp64 latency, and a quarter of
                 // the code (the kernel must stay inside the instruction cache: the groups run out of phase)
-#pragma unroll 4
+#pragma unroll NLU_C
                 for (int j = 0; j < 16; ++j) {
                     const cd q = p[j * T + m];
                     const double u = fma(dtG, cnorm2(q), fma(dtD, ph[j * T + m], vxs[j * T + m] + vrow));
@@ -314,10 +316,10 @@ int dbec_xline_supported(const dbec_handle_s* h) {
     return h->use_tma && (h->nx == 128 || h->nx == 256 || h->nx == 512) && ((h->ny * h->nz) % 8 == 0);
 }
 
-template <int N, bool RT, int NG, int NST> static int launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
+template <int N, bool RT, int NG, int NST, int XP = XPlan<N>::XP> static int launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
     typedef typename XPlan<N>::P P;
     typedef typename CnCoef<RT>::type CT;
-    constexpr int XP = XPlan<N>::XP, XR = 2 * XP;
+    constexpr int XR = 2 * XP;
     constexpr int GT = XR * P::T, NXHP = nxhp_of(N);
     constexpr int SPP = (P::SMEM > 2 * NXHP) ? P::SMEM : 2 * NXHP;
     constexpr int STAGE = XR * (N + 1) * (int)sizeof(cd) + XP * SPP * (int)sizeof(cd);
