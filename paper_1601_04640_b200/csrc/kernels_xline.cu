@@ -16,7 +16,7 @@
 #include "tma_pipe.cuh"
 #include "trig.cuh"
 
-// calcnu: points evaluated side by side (2, 4 and 8 measure the same; 4 keeps the code small)
+// calcnu: points evaluated side by side (8 measures slower than 4)
 constexpr int NLU_C = 4;
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
@@ -126,19 +126,32 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             {
                 cd* p = ps + lp * PITCH;
                 const double* ph = (const double*)(ss + (lp >> 1) * SPP) + (lp & 1) * N;
-                // four points at a time: enough independent work to cover the fp64 latency, and a quarter of
-                // the code (the kernel must stay inside the instruction cache: the groups run out of phase)
-#pragma unroll NLU_C
-                for (int j = 0; j < 16; ++j) {
-                    const cd q = p[j * T + m];
-                    const double u = fma(dtG, cnorm2(q), fma(dtD, ph[j * T + m], vxs[j * T + m] + vrow));
-                    if (RT) {
-                        double sn, cs_;
-                        sincos_cw(u, &sn, &cs_);              // branch-free: the 16 evaluations interleave
-                        p[j * T + m] = cmul(s, cmul(q, cmake(cs_, -sn)));
-                    } else {
-                        p[j * T + m] = cmul(s * exp(-u), q);
+                // NLU_C points at a time, all their loads first and all their stores last: p, ph and vxs point
+                // into the same shared array, so a store in between would pin every later load behind it and
+                // the evaluations would run one after the other (8-cycle fp64 latency, ~30 dependent steps each)
+#pragma unroll 1
+                for (int j0 = 0; j0 < 16; j0 += NLU_C) {
+                    cd q[NLU_C];
+                    double u[NLU_C];
+#pragma unroll
+                    for (int jj = 0; jj < NLU_C; ++jj) {
+                        const int x = (j0 + jj) * T + m;
+                        q[jj] = p[x];
+                        u[jj] = fma(dtD, ph[x], vxs[x] + vrow);
                     }
+#pragma unroll
+                    for (int jj = 0; jj < NLU_C; ++jj) {
+                        u[jj] = fma(dtG, cnorm2(q[jj]), u[jj]);
+                        if (RT) {
+                            double sn, cs_;
+                            sincos_cw(u[jj], &sn, &cs_);          // branch-free: the evaluations interleave
+                            q[jj] = cmul(s, cmul(q[jj], cmake(cs_, -sn)));
+                        } else {
+                            q[jj] = cmul(s * exp(-u[jj]), q[jj]);
+                        }
+                    }
+#pragma unroll
+                    for (int jj = 0; jj < NLU_C; ++jj) p[(j0 + jj) * T + m] = q[jj];
                 }
             }
             named_bar_sync(1 + g, GT);
