@@ -277,12 +277,18 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
 #pragma unroll
             for (int j = 8; j < 16; ++j) pr[N + j * T + m] = v[j];            // Z[N/2 .. N-1]
             __syncwarp();
+            // mirrors first, stores afterwards (a store in between would pin the later loads behind it)
+            cd zm[9];
+#pragma unroll
+            for (int j = 0; j <= 8; ++j) {
+                const int k = j * T + m;
+                zm[j] = (k == 0 || k > N / 2) ? v[j] : pr[2 * N - k];         // Z[N-k]
+            }
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
                 const int k = j * T + m;
                 if (k <= N / 2) {
-                    const cd z = v[j];
-                    const cd zp = (k == 0) ? z : pr[2 * N - k];               // Z[N-k]
+                    const cd z = v[j], zp = zm[j < 9 ? j : 8];
                     // X_a = (Z[k] + conj Z[N-k])/2,  X_b = (Z[k] - conj Z[N-k])/(2i)
                     pr[k] = cmake(0.5 * (z.x + zp.x), 0.5 * (z.y - zp.y));
                     pr[NXHP + k] = cmake(0.5 * (z.y + zp.y), -0.5 * (z.x - zp.x));
