@@ -71,7 +71,8 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
             tma_load_3d(dst + (size_t)b * (MAIN_BYTES / tg.nbox), map, c0, c1, c2, pb.full + s);
             if (EXTRA_BYTES) {
                 tile_coords(tg, t, b, TCOLS, c0, c1, c2);
-                tma_load_3d(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.nbox), extra, c0, c1, c2, pb.full + s);
+                tma_load_3d_hint(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.nbox), extra, c0, c1, c2, pb.full + s,
+                                 l2_policy_evict_first());      // the V_dd table is read once per step
             }
         }
     }

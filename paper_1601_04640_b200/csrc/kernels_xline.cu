@@ -181,6 +181,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             vrow = vrow_next;
         }
     } else if (tid == NG * GT) {
+        const uint64_t pol = l2_policy_evict_first();            // the spectrum is dead once it is on chip
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
@@ -195,8 +196,8 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
                 bulk_load(dst + (size_t)rr * PITCH * sizeof(cd), src + (size_t)rr * N, N * (int)sizeof(cd), full + st);
 #pragma unroll 1
             for (int pp = 0; pp < XP; ++pp)
-                bulk_load(dst + PSI_BYTES + (size_t)pp * SPP * sizeof(cd), spec + (tile * XP + pp) * 2 * NXHP,
-                          2 * NXHP * (int)sizeof(cd), full + st);
+                bulk_load_hint(dst + PSI_BYTES + (size_t)pp * SPP * sizeof(cd), spec + (tile * XP + pp) * 2 * NXHP,
+                               2 * NXHP * (int)sizeof(cd), full + st, pol);
         }
     } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
         // two storers (even / odd stages): while one sits in wait_group.read (which lasts about as long
@@ -302,12 +303,13 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
             if ((tid & 31) == 0) mbar_arrive(done + st);
         }
     } else if (tid == NG * GT) {
+        const uint64_t pol = l2_policy_evict_first();            // psi is not read again before four more passes
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
             st_release_shared(issued, i + 1);
             mbar_expect_tx(full + st, STAGE_BYTES);
-            bulk_load(base + (size_t)st * STAGE_BYTES, psi + tile_of(i) * XR * N, STAGE_BYTES, full + st);
+            bulk_load_hint(base + (size_t)st * STAGE_BYTES, psi + tile_of(i) * XR * N, STAGE_BYTES, full + st, pol);
         }
     } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
         const int which = (tid - NG * GT) / 32 - 1;      // storer 0: even stages, storer 1: odd stages
