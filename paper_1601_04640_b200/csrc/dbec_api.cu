@@ -284,6 +284,14 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     const char* le = getenv("DBEC_SPEC_LAG");
     h->spec_lag = le ? atoi(le) : 2;
     if (h->spec_lag < 1) h->spec_lag = 1;
+    {   // defaults: the outputs of the two x-line kernels are kept evict-last (the passes after them find part
+        // of the spectrum / of psi in L2), their dead inputs evict-first, everything else a neutral hint
+        const float def[POL_COUNT] = {0.f, 0.f, 0.f, 1.f, 2.f, 2.f, 1.f, 0.f, 0.f};
+        for (int i = 0; i < POL_COUNT; ++i) h->pol[i] = def[i];
+        const char* e = getenv("DBEC_POL");
+        if (e) sscanf(e, "%f,%f,%f,%f,%f,%f,%f,%f,%f", &h->pol[0], &h->pol[1], &h->pol[2], &h->pol[3], &h->pol[4],
+                      &h->pol[5], &h->pol[6], &h->pol[7], &h->pol[8]);
+    }
     const char* te = getenv("DBEC_TMA");
     h->use_tma = te ? atoi(te) : 1;
     // the legacy default stream cannot be captured: plain launches there

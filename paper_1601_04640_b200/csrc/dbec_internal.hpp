@@ -12,6 +12,10 @@
 #define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
 #define DBEC_TMAP_BYTES 128     // sizeof(CUtensorMap)
 
+// Access sites with an L2 eviction hint: loads / stores of psi in k_cn_tma, of psi and of the spectrum in
+// k_xline_nonlin, of psi and the spectrum in k_xline_density, of the spectrum in k_fft_tma.
+enum { POL_CN_LD = 0, POL_CN_ST, POL_NL_LD, POL_NL_ST, POL_NL_SPEC, POL_D_PSI, POL_D_SPEC, POL_FFT_LD, POL_FFT_ST, POL_COUNT };
+
 // Tensor maps of the handle (kernels_tma.cu): field x direction of the box rows.
 enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD_Y, TM_VDD_Z, TM_COUNT };
 
@@ -72,6 +76,8 @@ struct dbec_handle_s {
     int num_sms;
     int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
     int use_rev;                    // env DBEC_REV (default 1)
+    // L2 eviction policy code of every bulk / TMA access site (tma_pipe.cuh: l2_policy_code); env DBEC_POL
+    float pol[POL_COUNT];
     int use_spectral;               // env DBEC_SPECTRAL (default 0): y/z transforms of a step in one kernel (k_fft_spectral)
     int spec_xg, spec_lag;          // its tile list: column tiles per group (env DBEC_SPEC_XG, 1), lag in groups (DBEC_SPEC_LAG, 2)
     alignas(64) unsigned char tmap[TM_COUNT][DBEC_TMAP_BYTES];

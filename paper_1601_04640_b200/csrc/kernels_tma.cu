@@ -27,6 +27,7 @@ struct TileGeom {
     int nbox;        // boxes per tile (N / box_rows)
     int outer0;      // first outer coordinate (slab offset; axis 1 only)
     int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
+    float pol_ld, pol_st;   // L2 eviction policy codes of the tile loads / stores (tma_pipe.cuh: l2_policy_code)
 };
 
 struct PipeBars {
@@ -58,6 +59,7 @@ __device__ __forceinline__ void tile_coords(const TileGeom& tg, int t, int b, in
 template <int NST, int STAGE_BYTES, int MAIN_BYTES, int EXTRA_BYTES>
 __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
                                             const CUtensorMap* extra, const TileGeom& tg, int nmine) {
+    const uint64_t pol = l2_policy_code(tg.pol_ld);
     for (int i = 0; i < nmine; ++i) {
         const int s = i % NST;
         if (i >= NST) mbar_wait(pb.empty + s, ((i / NST) - 1) & 1);
@@ -68,7 +70,7 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
         for (int b = 0; b < tg.nbox; ++b) {
             int c0, c1, c2;
             tile_coords(tg, t, b, 2 * TCOLS, c0, c1, c2);
-            tma_load_3d(dst + (size_t)b * (MAIN_BYTES / tg.nbox), map, c0, c1, c2, pb.full + s);
+            tma_load_3d_hint(dst + (size_t)b * (MAIN_BYTES / tg.nbox), map, c0, c1, c2, pb.full + s, pol);
             if (EXTRA_BYTES) {
                 tile_coords(tg, t, b, TCOLS, c0, c1, c2);
                 tma_load_3d_hint(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.nbox), extra, c0, c1, c2, pb.full + s,
@@ -84,6 +86,7 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
 template <int NST, int STAGE_BYTES, int MAIN_BYTES>
 __device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
                                             const TileGeom& tg, int nmine, int which) {
+    const uint64_t pol = l2_policy_code(tg.pol_st);
     for (int i = 0; i < nmine; ++i) {
         const int s = i % NST;
         if ((s & 1) != which) continue;
@@ -93,7 +96,7 @@ __device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* s
         for (int b = 0; b < tg.nbox; ++b) {
             int c0, c1, c2;
             tile_coords(tg, t, b, 2 * TCOLS, c0, c1, c2);
-            tma_store_3d(map, c0, c1, c2, src + (size_t)b * (MAIN_BYTES / tg.nbox));
+            tma_store_3d_hint(map, c0, c1, c2, src + (size_t)b * (MAIN_BYTES / tg.nbox), pol);
         }
         bulk_commit();
         bulk_wait_read<0>();              // the copy engine has read the stage (fast; not the global write)
@@ -473,6 +476,9 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
 static TileGeom geom_of(const dbec_handle_s* h, int axis, int row_elems, int z0, int nzs) {
     TileGeom tg;
     tg.rev = h->rev_next;
+    const bool sp = row_elems == h->nxhp;
+    tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
+    tg.pol_st = h->pol[sp ? POL_FFT_ST : POL_CN_ST];
     tg.axis = axis;
     tg.ntiles_x = row_elems / TCOLS;
     const int n = axis == 1 ? h->ny : h->nz;

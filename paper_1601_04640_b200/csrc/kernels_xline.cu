@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(NG * 2 * XP * P::T + 96, 1)
 k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __restrict__ twA_g,
                const cd* __restrict__ twN_g, const double* __restrict__ scal, const double* __restrict__ vx_g,
                const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny,
-               long long row0, CnTab<RT> cn, int rev) {
+               long long row0, CnTab<RT> cn, int rev, float pol_ld, float pol_st, float pol_spec) {
     typedef typename CnCoef<RT>::type CT;
     // A group of GT = 8*T threads owns one tile: its first half runs the four pair transforms (T threads
     // per pair), then all of it runs calcnu (T threads per line) and calclux (one 16-point chunk each).
@@ -181,7 +181,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             vrow = vrow_next;
         }
     } else if (tid == NG * GT) {
-        const uint64_t pol = l2_policy_evict_first();            // the spectrum is dead once it is on chip
+        const uint64_t pol = l2_policy_code(pol_spec), polp = l2_policy_code(pol_ld);
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
@@ -193,7 +193,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             const cd* src = psi + tile * XR * N;
 #pragma unroll 1
             for (int rr = 0; rr < XR; ++rr)
-                bulk_load(dst + (size_t)rr * PITCH * sizeof(cd), src + (size_t)rr * N, N * (int)sizeof(cd), full + st);
+                bulk_load_hint(dst + (size_t)rr * PITCH * sizeof(cd), src + (size_t)rr * N, N * (int)sizeof(cd), full + st, polp);
 #pragma unroll 1
             for (int pp = 0; pp < XP; ++pp)
                 bulk_load_hint(dst + PSI_BYTES + (size_t)pp * SPP * sizeof(cd), spec + (tile * XP + pp) * 2 * NXHP,
@@ -203,6 +203,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         // two storers (even / odd stages): while one sits in wait_group.read (which lasts about as long
         // as the global write), the other already drains the next finished stage
         const int which = (tid - NG * GT) / 32 - 1;      // storer 0: even stages, storer 1: odd stages
+        const uint64_t polp = l2_policy_code(pol_st);
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if ((st & 1) != which) continue;
@@ -213,7 +214,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             cd* dstg = psi + tile * XR * N;
 #pragma unroll 1
             for (int rr = 0; rr < XR; ++rr)
-                bulk_store(dstg + (size_t)rr * N, src + (size_t)rr * PITCH * sizeof(cd), N * (int)sizeof(cd));
+                bulk_store_hint(dstg + (size_t)rr * N, src + (size_t)rr * PITCH * sizeof(cd), N * (int)sizeof(cd), polp);
             bulk_commit();
             bulk_wait_read<0>();
             mbar_arrive(empty + st);
@@ -232,7 +233,8 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
 template <class P, int XP, int NG, int NST>
 __global__ void __launch_bounds__(NG* XP* P::T + 96, 1)
 k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA_g,
-                const cd* __restrict__ twN_g, const double* __restrict__ scal, int ntiles, int rev) {
+                const cd* __restrict__ twN_g, const double* __restrict__ scal, int ntiles, int rev, float pol_psi,
+                float pol_spec) {
     constexpr int XR = 2 * XP;
     constexpr int T = P::T, N = P::N, GT = XP * T, NT = NG * GT + 96;
     constexpr int NXHP = nxhp_of(N);
@@ -303,7 +305,7 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
             if ((tid & 31) == 0) mbar_arrive(done + st);
         }
     } else if (tid == NG * GT) {
-        const uint64_t pol = l2_policy_evict_first();            // psi is not read again before four more passes
+        const uint64_t pol = l2_policy_code(pol_psi);
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
@@ -318,10 +320,11 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
             if ((st & 1) != which) continue;
             mbar_wait(done + st, (i / NST) & 1);
             const unsigned char* src = base + (size_t)st * STAGE_BYTES;
+            const uint64_t pols = l2_policy_code(pol_spec);
             cd* dstg = spec + tile_of(i) * XR * NXHP;
 #pragma unroll 1
             for (int pp = 0; pp < XP; ++pp)
-                bulk_store(dstg + (size_t)pp * 2 * NXHP, src + (size_t)pp * 2 * N * sizeof(cd), PAIR_BYTES);
+                bulk_store_hint(dstg + (size_t)pp * 2 * NXHP, src + (size_t)pp * 2 * N * sizeof(cd), PAIR_BYTES, pols);
             bulk_commit();
             bulk_wait_read<0>();
             mbar_arrive(empty + st);
@@ -354,7 +357,7 @@ template <int N, bool RT, int NG, int NST, int XP = XPlan<N>::XP> static int lau
     const long long row0 = (long long)z0 * h->ny;
     k<<<grid, NG * GT + 96, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
                                              h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, row0,
-                                             make_cntab<RT>(h->ax[0]), h->rev_next);
+                                             make_cntab<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]);
     h->launches++;
     return (int)cudaGetLastError();
 }
@@ -381,7 +384,7 @@ template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s*
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
     k<<<grid, NG * GT + 96, sm, h->stream>>>(h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
-                                             ntiles, h->rev_next);
+                                             ntiles, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC]);
     h->launches++;
     return (int)cudaGetLastError();
 }

@@ -109,6 +109,31 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
+// A fraction f of the lines (chosen by the hardware from the address, the same lines every time) is kept
+// evict-last, the rest left alone: with f * field size well below the L2 size that part of a field that
+// is streamed several times per step stays in L2 from pass to pass and from step to step.
+// Policy from a code: c >= 2 evict-first; otherwise a fraction c (0..1) of the lines evict-last, the rest
+// left alone (c = 0: a neutral hint).
+__device__ __forceinline__ uint64_t l2_policy_pin(float f);
+__device__ __forceinline__ uint64_t l2_policy_code(float c) {
+    uint64_t pol;
+    if (c >= 2.f) { asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol)); return pol; }
+    return l2_policy_pin(c);
+}
+__device__ __forceinline__ uint64_t l2_policy_pin(float f) {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.L2::evict_unchanged.b64 %0, %1;" : "=l"(pol) : "f"(f));
+    return pol;
+}
+__device__ __forceinline__ void tma_store_3d_hint(const CUtensorMap* map, int c0, int c1, int c2, const void* src, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;"
+                 ::"l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_store_hint(void* dst, const void* src, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes), "l"(pol)
+                 : "memory");
+}
 __device__ __forceinline__ void tma_load_3d_hint(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar,
                                                  uint64_t pol) {
     asm volatile(
