@@ -292,6 +292,8 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
         if (e) sscanf(e, "%f,%f,%f,%f,%f,%f,%f,%f,%f", &h->pol[0], &h->pol[1], &h->pol[2], &h->pol[3], &h->pol[4],
                       &h->pol[5], &h->pol[6], &h->pol[7], &h->pol[8]);
     }
+    const char* pe = getenv("DBEC_PDL");
+    h->use_pdl = pe ? atoi(pe) : 1;
     const char* te = getenv("DBEC_TMA");
     h->use_tma = te ? atoi(te) : 1;
     // the legacy default stream cannot be captured: plain launches there

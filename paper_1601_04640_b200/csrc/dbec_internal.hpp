@@ -74,6 +74,7 @@ struct dbec_handle_s {
     int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
     int use_tma;                    // env DBEC_TMA (default 1): persistent TMA-fed kernels for lines of 128..512 points
     int num_sms;
+    int use_pdl;                    // env DBEC_PDL (default 1): programmatic dependent launch of the persistent kernels
     int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
     int use_rev;                    // env DBEC_REV (default 1)
     // L2 eviction policy code of every bulk / TMA access site (tma_pipe.cuh: l2_policy_code); env DBEC_POL

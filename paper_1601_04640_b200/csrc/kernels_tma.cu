@@ -43,6 +43,8 @@ template <int NST> __device__ __forceinline__ PipeBars pipe_init(uint64_t* bars,
         fence_mbar_init();
     }
     __syncthreads();
+    pdl_launch_dependents();        // the next kernel of the stream may start its own prologue
+    pdl_wait();                     // tables are staged, barriers set up: now wait for the previous kernel's data
     return b;
 }
 
@@ -501,7 +503,8 @@ template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma
     auto k = k_cn_tma<RT, NCH, NG, NST, NORM>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_PSI_Y : TM_PSI_Z];
-    k<<<grid, NG * GT + 96, sm, h->stream>>>(*map, make_cntab<RT>(h->ax[axis]), tg, h->partial, h->ticket, h->scal, h->dV);
+    CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, *map, make_cntab<RT>(h->ax[axis]), tg, h->partial,
+                  h->ticket, h->scal, h->dV));
     h->launches++;
     return (int)cudaGetLastError();
 }
@@ -542,7 +545,7 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_SPEC_Y : TM_SPEC_Z];
     const CUtensorMap* mv = (const CUtensorMap*)h->tmap[axis == 1 ? TM_VDD_Y : TM_VDD_Z];
-    k<<<grid, NG * GT + 96, sm, h->stream>>>(*map, *mv, h->ax[axis].twA, h->ax[axis].twN, tg);
+    CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, *map, *mv, h->ax[axis].twA, h->ax[axis].twN, tg));
     h->launches++;
     return (int)cudaGetLastError();
 }

@@ -74,6 +74,8 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         fence_mbar_init();
     }
     __syncthreads();
+    pdl_launch_dependents();        // the next kernel of the stream may start its own prologue
+    pdl_wait();                     // tables are staged, barriers set up: now wait for the previous kernel's data
     const int nmine = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     if (tid < NG * GT) {
         const int g = tid / GT, t = tid % GT;
@@ -254,6 +256,8 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
         fence_mbar_init();
     }
     __syncthreads();
+    pdl_launch_dependents();        // the next kernel of the stream may start its own prologue
+    pdl_wait();                     // tables are staged, barriers set up: now wait for the previous kernel's data
     const int nmine = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     auto tile_of = [&](int i) {
         const long long t = (long long)blockIdx.x + (long long)i * gridDim.x;
@@ -355,9 +359,9 @@ template <int N, bool RT, int NG, int NST, int XP = XPlan<N>::XP> static int lau
     auto k = k_xline_nonlin<P, XP, RT, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
-    k<<<grid, NG * GT + 96, sm, h->stream>>>(h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
+    CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
                                              h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, row0,
-                                             make_cntab<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]);
+                                             make_cntab<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]));
     h->launches++;
     return (int)cudaGetLastError();
 }
@@ -383,8 +387,8 @@ template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s*
     auto k = k_xline_density<P, XP, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
-    k<<<grid, NG * GT + 96, sm, h->stream>>>(h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
-                                             ntiles, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC]);
+    CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
+                                             ntiles, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC]));
     h->launches++;
     return (int)cudaGetLastError();
 }

@@ -12,6 +12,7 @@
 #pragma once
 #include <cuda.h>
 #include <stdint.h>
+#include <utility>
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -165,7 +166,28 @@ template <int N> __device__ __forceinline__ void bulk_wait() {
     asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
 }
 
+// ---- programmatic dependent launch: a kernel launched with launch_pdl() may become resident while the
+// kernel before it in the stream is still draining; everything it does before pdl_wait() (staging constant
+// tables, initialising barriers) overlaps that tail, everything after sees the predecessor's memory ----
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // barrier over `nthreads` threads (a multiple of 32) with hardware barrier `id` (1..15; 0 is __syncthreads)
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+
+#if defined(__CUDACC__)
+// Host: launch with programmatic stream serialisation (the kernel MUST call pdl_wait() before it touches
+// anything an earlier kernel of the stream writes).
+template <class K, class... Args>
+static inline cudaError_t launch_pdl(K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t stream, int enable, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = enable ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+#endif
