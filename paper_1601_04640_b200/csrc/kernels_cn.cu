@@ -14,6 +14,7 @@
 #include "dbec_internal.hpp"
 #include "cn_chunk.cuh"
 #include "cn_line_smem.cuh"
+#include "tma_pipe.cuh"
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
@@ -98,6 +99,7 @@ k_cn_strided(cd* __restrict__ psi, CnTab<RT> cn, long long line_stride, long lon
     __shared__ cd edge[2][NCH][COLS];     // first and last point of every chunk (halo of the neighbours)
     __shared__ cd ends[2][NCH][COLS];     // zero-start chunk results for the carries
     __shared__ double red[32];
+    pdl_launch_dependents(); pdl_wait();       // (tma_pipe.cuh) launch latency overlaps the previous kernel
     const int col = threadIdx.x % COLS, c = threadIdx.x / COLS;
     long long gcol = (long long)blockIdx.x * COLS + col;
     const bool active = gcol < ncols;          // narrow grids: a tile may be wider than the grid
@@ -152,6 +154,7 @@ k_cn_x(cd* __restrict__ psi, CnTab<RT> cn, int nlines, double* __restrict__ part
     extern __shared__ cd smem[];
     __shared__ double red[32];
     typedef typename CnCoef<RT>::type CT;
+    pdl_launch_dependents(); pdl_wait();
     constexpr int N = 16 * T;
     const int lp = threadIdx.x / T, m = threadIdx.x % T;
     long long line = (long long)blockIdx.x * LPB + lp;
@@ -280,10 +283,10 @@ template <bool RT, int NCH, bool NORM> static int launch_cn_strided(dbec_handle_
     else { line_stride = (long long)h->nx * h->ny; outer_stride = 0; ncols = line_stride; nouter = 1; }
     dim3 grid((unsigned)((ncols + COLS - 1) / COLS), (unsigned)nouter);
     if (NORM && (long long)grid.x * grid.y > h->npartial) return (int)cudaErrorInvalidValue;
-    k_cn_strided<RT, NCH, COLS, NORM><<<grid, NCH * COLS, 0, h->stream>>>(
-        h->psi, make_cntab<RT>(h->ax[axis]), line_stride, outer_stride, ncols, h->partial, h->ticket, h->scal, h->dV);
+    cudaError_t e = launch_pdl(k_cn_strided<RT, NCH, COLS, NORM>, grid, dim3(NCH * COLS), 0, h->stream, h->use_pdl, h->psi,
+                               make_cntab<RT>(h->ax[axis]), line_stride, outer_stride, ncols, h->partial, h->ticket, h->scal, h->dV);
     h->launches++;
-    return (int)cudaGetLastError();
+    return (int)e;
 }
 
 template <bool RT, int NCH, bool NORM> static int launch_cn_x(dbec_handle_s* h) {
@@ -295,9 +298,10 @@ template <bool RT, int NCH, bool NORM> static int launch_cn_x(dbec_handle_s* h) 
     if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const int nb = (nlines + LPB - 1) / LPB;
     if (NORM && nb > h->npartial) return (int)cudaErrorInvalidValue;
-    k<<<nb, T * LPB, sm, h->stream>>>(h->psi, make_cntab<RT>(h->ax[0]), nlines, h->partial, h->ticket, h->scal, h->dV);
+    cudaError_t e = launch_pdl(k, dim3(nb), dim3(T * LPB), sm, h->stream, h->use_pdl, h->psi, make_cntab<RT>(h->ax[0]), nlines,
+                               h->partial, h->ticket, h->scal, h->dV);
     h->launches++;
-    return (int)cudaGetLastError();
+    return (int)e;
 }
 
 template <bool RT, bool NORM> static int launch_cn_rt(dbec_handle_s* h, int axis) {

@@ -15,6 +15,7 @@
 #include "fft_line.cuh"
 #include "cn_chunk.cuh"
 #include "cn_line_smem.cuh"
+#include "tma_pipe.cuh"
 
 template <class P> struct XLine {
     // shared elements per line pair of the contiguous-x kernels: FFT exchange or one padded line
@@ -31,6 +32,7 @@ __global__ void __launch_bounds__(P::T* LP)
 k_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA,
                const cd* __restrict__ twN, const double* __restrict__ scal, int npairs, int nxhp) {
     extern __shared__ cd smem[];
+    pdl_launch_dependents(); pdl_wait();       // (tma_pipe.cuh) launch latency overlaps the previous kernel
     constexpr int T = P::T, N = P::N;
     const int lp = threadIdx.x / T, m = threadIdx.x % T;
     const long long pair = (long long)blockIdx.x * LP + lp;
@@ -81,6 +83,7 @@ k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* _
               const cd* __restrict__ twN, long long line_stride, long long outer_stride, int ntiles_x,
               long long ntiles) {
     extern __shared__ cd smem[];
+    pdl_launch_dependents(); pdl_wait();
     constexpr int T = P::T, C = DBEC_SPEC_COLS;
     const int tl = threadIdx.x / (T * C), r = threadIdx.x % (T * C);
     const int col = r % C, m = r / C;
@@ -123,6 +126,7 @@ k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __rest
                const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
                double dt, int npairs, int nxhp, int ny, CnTab<RT> cn) {
     extern __shared__ cd smem[];
+    pdl_launch_dependents(); pdl_wait();
     typedef typename CnCoef<RT>::type CT;
     constexpr int T = P::T, N = P::N;
     const int lp = threadIdx.x / T, m = threadIdx.x % T;
@@ -278,10 +282,10 @@ template <int N> static int launch_density_fftx(dbec_handle_s* h) {
     auto k = k_density_fftx<P, LP>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
-    k<<<(npairs + LP - 1) / LP, P::T * LP, sm, h->stream>>>(h->psi, h->spec, h->ax[0].twA, h->ax[0].twN, h->scal,
-                                                            npairs, h->nxhp);
+    cudaError_t e = launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(P::T * LP), sm, h->stream, h->use_pdl, h->psi, h->spec,
+                               h->ax[0].twA, h->ax[0].twN, h->scal, npairs, h->nxhp);
     h->launches++;
-    return (int)cudaGetLastError();
+    return (int)e;
 }
 
 template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int axis) {
@@ -301,10 +305,10 @@ template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int a
     auto k = k_fft_strided<P, MODE, TILES>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
-    k<<<(unsigned)((ntiles + TILES - 1) / TILES), P::T * C * TILES, sm, h->stream>>>(
-        h->spec, h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles);
+    cudaError_t e = launch_pdl(k, dim3((unsigned)((ntiles + TILES - 1) / TILES)), dim3(P::T * C * TILES), sm, h->stream, h->use_pdl,
+                               h->spec, (const double*)h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles);
     h->launches++;
-    return (int)cudaGetLastError();
+    return (int)e;
 }
 
 template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, double* phi) {
@@ -316,11 +320,11 @@ template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, do
     auto k = k_ifftx_nonlin<P, LP, RT, MODE>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
-    k<<<(npairs + LP - 1) / LP, P::T * LP, sm, h->stream>>>(
-        h->spec, h->psi, phi, h->ax[0].twA, h->ax[0].twN, h->scal, h->ax[0].vtrap, h->ax[1].vtrap,
-        h->ax[2].vtrap, h->p.dt, npairs, h->nxhp, h->ny, make_cntab<RT>(h->ax[0]));
+    cudaError_t e = launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(P::T * LP), sm, h->stream, h->use_pdl,
+                               (const cd*)h->spec, h->psi, phi, h->ax[0].twA, h->ax[0].twN, (const double*)h->scal, h->ax[0].vtrap,
+                               h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, npairs, h->nxhp, h->ny, make_cntab<RT>(h->ax[0]));
     h->launches++;
-    return (int)cudaGetLastError();
+    return (int)e;
 }
 
 int dbec_launch_density_fftx(dbec_handle_s* h) {
