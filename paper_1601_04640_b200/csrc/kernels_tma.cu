@@ -101,7 +101,7 @@ __device__ __forceinline__ void pipe_storer(const PipeBars& pb, unsigned char* s
             tma_store_3d_hint(map, c0, c1, c2, src + (size_t)b * (MAIN_BYTES / tg.nbox), pol);
         }
         bulk_commit();
-        bulk_wait_read<0>();              // the copy engine has read the stage (fast; not the global write)
+        bulk_wait_read<0>();              // the copy engine has read the stage (takes about as long as the global write)
         mbar_arrive(pb.empty + s);
     }
     bulk_wait<0>();

@@ -98,32 +98,23 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, int c0, int
                  ::"l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2)
                  : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
-    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
-}
 
-// ---- L2 eviction hints: inputs that nobody reads again soon (the spectrum in the x-line kernel, psi in the
-// density kernel, the V_dd table) are loaded evict-first, so that what stays in the 126 MB L2 at the end
-// of a pass is its dirty OUTPUT, which the next pass walks first (TileGeom::rev) ----
+// ---- L2 eviction policies (createpolicy + .L2::cache_hint on every bulk / TMA access) ----
+// What stays in the 126 MB L2 at the end of a pass should be its OUTPUT, which the next pass walks first
+// (TileGeom::rev): outputs of the x-line kernels are stored evict-last, inputs that nobody reads again soon
+// (the spectrum in the x-line kernel, psi in the density kernel, the V_dd tiles) are loaded evict-first,
+// every other access carries a neutral hint.  Measured alternatives: profiles/r1d_step_ncu_full.md.
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
-// A fraction f of the lines (chosen by the hardware from the address, the same lines every time) is kept
-// evict-last, the rest left alone: with f * field size well below the L2 size that part of a field that
-// is streamed several times per step stays in L2 from pass to pass and from step to step.
-// Policy from a code: c >= 2 evict-first; otherwise a fraction c (0..1) of the lines evict-last, the rest
-// left alone (c = 0: a neutral hint).
-__device__ __forceinline__ uint64_t l2_policy_pin(float f);
+// Policy from a code (dbec_handle_s::pol): c >= 2 evict-first; otherwise a fraction c (0..1) of the lines
+// evict-last and the rest left alone (c = 0: neutral, c = 1: all evict-last).
 __device__ __forceinline__ uint64_t l2_policy_code(float c) {
+    if (c >= 2.f) return l2_policy_evict_first();
     uint64_t pol;
-    if (c >= 2.f) { asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol)); return pol; }
-    return l2_policy_pin(c);
-}
-__device__ __forceinline__ uint64_t l2_policy_pin(float f) {
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.L2::evict_unchanged.b64 %0, %1;" : "=l"(pol) : "f"(f));
+    asm volatile("createpolicy.fractional.L2::evict_last.L2::evict_unchanged.b64 %0, %1;" : "=l"(pol) : "f"(c));
     return pol;
 }
 __device__ __forceinline__ void tma_store_3d_hint(const CUtensorMap* map, int c0, int c1, int c2, const void* src, uint64_t pol) {
@@ -149,15 +140,6 @@ __device__ __forceinline__ void bulk_load_hint(void* dst, const void* src, uint3
 }
 
 // ---- 1-D bulk copies (contiguous runs, multiples of 16 bytes, 16-byte aligned on both sides) ----
-__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_store(void* dst, const void* src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes)
-                 : "memory");
-}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void bulk_wait_read() {
     asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
