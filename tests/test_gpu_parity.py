@@ -140,7 +140,7 @@ def test_one_step_small_grids(gp, ob, w):
     o.close()
 
 
-@pytest.mark.parametrize("key", ["C1", "C2", "C3", "C4"])
+@pytest.mark.parametrize("key", ["C1", "C2", "C3", "C4", "C5"])
 def test_one_step_baseline_configs(gp, ob, key):
     """Full-size BASELINE.json configs, one step, every grid point compared."""
     w = workload(key)
