@@ -38,7 +38,13 @@ DBEC_HD void sincos_cw(double u, double* sn, double* cs) {
 #else
     const double* K = sincos_cw_host;
 #endif
-    u = (fabs(u) <= SINCOS_CW_MAX) ? u : (u - u) / (u - u);   // out of range or not finite -> NaN
+    // out of range or not finite -> NaN, by a select of a constant (a division here would put a branch with a
+    // slow-path call around every evaluation and keep the compiler from interleaving them)
+#if defined(__CUDA_ARCH__)
+    u = (fabs(u) <= SINCOS_CW_MAX) ? u : __longlong_as_double(0x7ff8000000000000LL);
+#else
+    { union { unsigned long long i; double d; } qn; qn.i = 0x7ff8000000000000ULL; u = (fabs(u) <= SINCOS_CW_MAX) ? u : qn.d; }
+#endif
     const double MAGIC = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to nearest integer
     const double kb = fma(u, K[0], MAGIC);
     const double kd = kb - MAGIC;
