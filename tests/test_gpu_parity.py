@@ -36,14 +36,18 @@ def grid3(nx, ny, nz, mode, G=30.0, D=20.0, dx=0.4, dt=None, trap=(1.0, 1.2, 0.7
     return Workload("t3", 3, nx, ny, nz, d[0], d[1], d[2], dt, *trap, G, D, G, D, mode, 1, 21, 1, cutoff=cutoff)
 
 
-def grid2(nx, ny, mode, G=20.0, D=15.0, dx=0.2, dt=None, trap=(1.0, 1.5, 0.0)):
+def grid2(nx, ny, mode, G=20.0, D=15.0, dx=0.2, dt=None, trap=(1.0, 1.5, 0.0), dy=None):
     dt = dt if dt is not None else (0.1 if mode == IMAG else 0.5) * dx ** 2
-    return Workload("t2", 2, nx, ny, 1, dx, dx, 1.0, dt, *trap, G, D, G, D, mode, 1, 22, 1)
+    return Workload("t2", 2, nx, ny, 1, dx, dy or dx, 1.0, dt, *trap, G, D, G, D, mode, 1, 22, 1)
 
 
 SHAPES3 = [(16, 16, 16), (32, 32, 32), (64, 16, 32), (16, 64, 128), (128, 32, 16), (256, 16, 16), (16, 256, 32),
            (32, 16, 512), (512, 32, 16)]
 SHAPES2 = [(16, 16), (32, 64), (128, 32), (512, 16), (16, 512), (256, 256)]
+# dx != dy != dz (C5 is the only BASELINE.json config with two spacings): the V_dd wavenumbers, dV, the
+# Crank-Nicolson coefficient of every axis and the kinetic / rms sums each take their own spacing
+ANISO3 = [(32, 16, 64), (128, 32, 16), (16, 128, 128)]
+ANISO2 = [(64, 32), (128, 256)]
 
 
 def all_small_workloads():
@@ -53,11 +57,16 @@ def all_small_workloads():
             out.append(grid3(*s, mode))
         for s in SHAPES2:
             out.append(grid2(*s, mode))
+        for s in ANISO3:
+            out.append(grid3(*s, mode, d=(0.4, 0.3, 0.6)))
+        for s in ANISO2:
+            out.append(grid2(*s, mode, dx=0.2, dy=0.3))
     return out
 
 
 def wid(w):
-    return f"{w.ndim}d-{w.nx}x{w.ny}x{w.nz}-{'imag' if w.time_mode == IMAG else 'real'}"
+    aniso = "" if (w.dx == w.dy and (w.ndim == 2 or w.dx == w.dz)) else "-aniso"
+    return f"{w.ndim}d-{w.nx}x{w.ny}x{w.nz}-{'imag' if w.time_mode == IMAG else 'real'}{aniso}"
 
 
 @pytest.mark.parametrize("w", all_small_workloads(), ids=wid)
