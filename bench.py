@@ -49,7 +49,6 @@ ALG_BYTES_PER_POINT = {
     "cn_x": 32,
     "cn_y": 32,
     "cn_z": 32,
-    "fft_y<fwd>+fft_z<fwd*Vdd*inv>+fft_y<inv>": 3 * (8 + 8),     # the three passes it replaces
 }
 MODEL_BYTES_PER_POINT = {3: 208, 2: 144}    # SURVEY.md §8(d) "Model M": fixed reference accounting
 

@@ -92,7 +92,9 @@ int dbec_observables(dbec_handle h, dbec_obs* host_out);
 int dbec_destroy(dbec_handle h);
 
 const char* dbec_strerror(int code);
-int dbec_last_cuda_error(dbec_handle h);     /* CUDA error code of the last DBEC_ECUDA, else 0 */
+/* CUDA error code behind this handle's last DBEC_ECUDA (0 if none).  h == NULL: the CUDA error behind the
+ * calling thread's last failed dbec_create, which leaves no handle to ask. */
+int dbec_last_cuda_error(dbec_handle h);
 
 /* ---- single parts of the step, exported so that each can be checked on its own ---- */
 
@@ -108,8 +110,9 @@ int dbec_cn_sweep(dbec_handle h, int axis);
  * current psi, no Crank-Nicolson sweep, asynchronous. */
 int dbec_nonlinear(dbec_handle h);
 
-/* calcnorm alone: psi <- psi / sqrt(dV sum |psi|^2); the factor is kept deferred
- * (applied by every consumer), asynchronous. */
+/* calcnorm alone: psi <- psi / sqrt(dV sum |psi|^2), asynchronous.  In imaginary time the
+ * factor is kept deferred (applied by every consumer); in real time, where no step ever renormalises, it is
+ * applied to the stored field at once. */
 int dbec_normalize(dbec_handle h);
 
 /* Number of kernel launches the library has enqueued on this handle since creation. */
@@ -119,7 +122,7 @@ int dbec_launch_count(dbec_handle h, long long* launches);
  * around every kernel.  ms_per_slot: HOST pointer to DBEC_KERNEL_SLOTS doubles receiving the total
  * milliseconds spent in each kernel slot over the nsteps steps; launches_per_slot: HOST pointer to
  * DBEC_KERNEL_SLOTS counts.  Synchronises the stream.  Slot names from dbec_kernel_name. */
-#define DBEC_KERNEL_SLOTS 9
+#define DBEC_KERNEL_SLOTS 8
 int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long* launches_per_slot);
 const char* dbec_kernel_name(int slot);
 /* Name of the __global__ function that serves pass `slot` on this handle ("" if the pass is not part
@@ -128,6 +131,8 @@ const char* dbec_kernel_name(int slot);
 const char* dbec_pass_kernel(dbec_handle h, int slot);
 
 int dbec_version(void);
+/* "DBEC_BUILD_ID=<hash of the sources this library was built from>" (paper_1601_04640_b200/build.py). */
+const char* dbec_build_id(void);
 
 #ifdef __cplusplus
 }

@@ -3,10 +3,12 @@
     python -m paper_1601_04640_b200.build [--force]
 
 nvcc cross-compiles without a GPU.  The object files land in paper_1601_04640_b200/build/, the
-library beside this file so that it travels with the source tree.
+library beside this file so that it travels with the source tree.  The library carries a hash of its
+sources (dbec_build_id); build() is a no-op when that hash matches the tree, whatever the file times say.
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -24,22 +26,39 @@ FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=s
 
 def _deps():
     out = [os.path.join(HERE, "..", "include", "dbec.h")]
-    for f in os.listdir(CSRC):
+    for f in sorted(os.listdir(CSRC)):
         out.append(os.path.join(CSRC, f))
     return out
 
 
-def _stale(target, deps):
-    if not os.path.exists(target):
-        return True
-    t = os.path.getmtime(target)
-    return any(os.path.getmtime(d) > t for d in deps)
+_MARK = b"DBEC_BUILD_ID="
 
 
-def _compile(src):
+def source_id() -> str:
+    """Hash of every source file the library is built from (and of the compiler flags)."""
+    h = hashlib.sha256(" ".join(FLAGS).encode())
+    for d in _deps():
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:32]
+
+
+def built_id(lib=LIB):
+    """The source hash compiled into an existing libdbec.so (dbec_build_id), read from the file's bytes so
+    that a stale library never has to be loaded; None if the file is missing or carries no id."""
+    if not os.path.exists(lib):
+        return None
+    with open(lib, "rb") as f:
+        blob = f.read()
+    i = blob.find(_MARK)
+    return blob[i + len(_MARK): i + len(_MARK) + 32].decode("ascii", "replace") if i >= 0 else None
+
+
+def _compile(src, sid):
     obj = os.path.join(OBJ, src.replace(".cu", ".o"))
     log = obj + ".log"
-    cmd = [NVCC, *FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+    cmd = [NVCC, *FLAGS, f'-DDBEC_BUILD_ID_STR="{sid}"', "-c", os.path.join(CSRC, src), "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     with open(log, "w") as f:
         f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
@@ -49,12 +68,12 @@ def _compile(src):
 
 
 def build(force: bool = False) -> str:
-    deps = _deps()
-    if not force and not _stale(LIB, deps):
+    sid = source_id()
+    if not force and built_id() == sid:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(_compile, SOURCES))
+        objs = list(ex.map(lambda s: _compile(s, sid), SOURCES))
     cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:

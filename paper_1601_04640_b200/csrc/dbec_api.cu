@@ -33,7 +33,7 @@ static int check_params(const dbec_params* p) {
 
 // ---- workspace layout: one pass computes the offsets, used by both sizing and create ----
 struct Layout {
-    size_t psi, spec, vdd, phi, scal, partial, ticket, sync, obs, tables, total;
+    size_t psi, spec, vdd, phi, scal, partial, ticket, obs, tables, total;
     size_t tab_bytes;
 };
 static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -61,13 +61,14 @@ static void make_layout(const dbec_params* p, Layout* L) {
     L->scal = o;    o += up256(SC_COUNT * sizeof(double));
     L->partial = o; o += up256(NPARTIAL * sizeof(double));
     L->ticket = o;  o += 256;
-    L->sync = o;    o += 1024;
     L->obs = o;     o += 256;
     L->tables = o;
     L->tab_bytes = axis_table_bytes(p->nx) + axis_table_bytes(p->ny) + axis_table_bytes(p->nz);
     o += L->tab_bytes;
     L->total = o;
 }
+
+static thread_local int create_cuda_error = 0;     // CUDA error of this thread's last failed dbec_create
 
 static int cuda_fail(dbec_handle h, cudaError_t e) {
     if (h) h->last_cuda = (int)e;
@@ -144,20 +145,16 @@ static int write_scalars(dbec_handle h, bool reset_scale) {
 }
 
 // Kernel slots of one step (dbec_step_profile / dbec_kernel_name).
-enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z, KS_FFT_SPECTRAL };
+enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z };
 static const char* const kernel_names[DBEC_MAX_KERNELS] = {
     "density+fft_x", "fft_y<fwd>", "fft_last<fwd*Vdd*inv>", "fft_y<inv>",
-    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z", "fft_y<fwd>+fft_z<fwd*Vdd*inv>+fft_y<inv>"};
+    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z"};
 
 #define KLAUNCH(h, slot, x)                                                                      \
     do {                                                                                         \
         if ((h)->prof_on) cudaEventRecord((h)->prof_ev[2 * (h)->prof_n], (h)->stream);           \
         int rc_ = (x);                                                                           \
-        if (!rc_ && getenv("DBEC_SYNC")) rc_ = (int)cudaStreamSynchronize((h)->stream);          \
-        if (rc_) {                                                                               \
-            if (getenv("DBEC_DEBUG")) fprintf(stderr, "dbec: launch in slot %d (%s) failed: %d\n", (slot), kernel_names[slot], rc_); \
-            return cuda_fail(h, (cudaError_t)rc_);                                               \
-        }                                                                                        \
+        if (rc_) return cuda_fail(h, (cudaError_t)rc_);                                          \
         if ((h)->prof_on) {                                                                      \
             cudaEventRecord((h)->prof_ev[2 * (h)->prof_n + 1], (h)->stream);                     \
             (h)->prof_slot[(h)->prof_n++] = (slot);                                              \
@@ -181,9 +178,7 @@ static int enqueue_dipolar_spectrum(dbec_handle h) {
     h->rev_next = 0;
     if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nz));
     else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
-    if (dbec_spectral_supported(h)) {
-        KLAUNCH(h, KS_FFT_SPECTRAL, dbec_launch_fft_spectral(h));
-    } else if (h->p.ndim == 3) {
+    if (h->p.ndim == 3) {
         KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
         KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 2, 2));
         KLAUNCH(h, KS_FFT_Y_INV, launch_fft_pass(h, 1, 1));
@@ -267,42 +262,31 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->scal = (double*)(w + L.scal);
     h->partial = (double*)(w + L.partial);
     h->ticket = (unsigned int*)(w + L.ticket);
-    h->sync = (int*)(w + L.sync);
     h->obs_dev = (double*)(w + L.obs);
     h->npartial = NPARTIAL;
+    // the only two switches (both exercised by tests/test_gpu_parity.py): the CUDA graph of a step and the
+    // x sweep fused into the nonlinear kernel
     const char* fe = getenv("DBEC_FUSE_CNX");
     h->fuse_cnx = fe ? atoi(fe) : 1;
     const char* ge = getenv("DBEC_GRAPH");
     h->use_graph = ge ? atoi(ge) : 1;
-    const char* re = getenv("DBEC_REV");
-    h->use_rev = re ? atoi(re) : 1;
-    const char* se = getenv("DBEC_SPECTRAL");
-    h->use_spectral = se ? atoi(se) : 0;
-    const char* xe = getenv("DBEC_SPEC_XG");
-    h->spec_xg = xe ? atoi(xe) : 1;
-    if (h->spec_xg < 1) h->spec_xg = 1;
-    const char* le = getenv("DBEC_SPEC_LAG");
-    h->spec_lag = le ? atoi(le) : 2;
-    if (h->spec_lag < 1) h->spec_lag = 1;
-    {   // defaults: the outputs of the two x-line kernels are kept evict-last (the passes after them find part
-        // of the spectrum / of psi in L2), their dead inputs evict-first, everything else a neutral hint
+    h->use_rev = 1; h->use_pdl = 1; h->use_tma = 1;
+    {   // L2 eviction policy per access site: the outputs of the two x-line kernels are kept evict-last (the
+        // passes after them find part of the spectrum / of psi in L2), their dead inputs evict-first,
+        // everything else a neutral hint (measured alternatives: profiles/r1d_step_ncu_full.md)
         const float def[POL_COUNT] = {0.f, 0.f, 0.f, 1.f, 2.f, 2.f, 1.f, 0.f, 0.f};
         for (int i = 0; i < POL_COUNT; ++i) h->pol[i] = def[i];
-        const char* e = getenv("DBEC_POL");
-        if (e) sscanf(e, "%f,%f,%f,%f,%f,%f,%f,%f,%f", &h->pol[0], &h->pol[1], &h->pol[2], &h->pol[3], &h->pol[4],
-                      &h->pol[5], &h->pol[6], &h->pol[7], &h->pol[8]);
     }
-    const char* pe = getenv("DBEC_PDL");
-    h->use_pdl = pe ? atoi(pe) : 1;
-    const char* te = getenv("DBEC_TMA");
-    h->use_tma = te ? atoi(te) : 1;
     // the legacy default stream cannot be captured: plain launches there
     if (h->stream == nullptr || h->stream == cudaStreamLegacy) h->use_graph = 0;
 
-#define FAIL(code) do { delete h; return (code); } while (0)
-    if (cudaMemsetAsync(h->psi, 0, sizeof(cd) * h->P, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
-    if (cudaMemsetAsync(h->ticket, 0, 256, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
-    if (cudaMemsetAsync(h->spec, 0, sizeof(cd) * h->SP, h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
+    // a failed create has no handle to ask: its CUDA error is kept per thread (dbec_last_cuda_error(NULL))
+#define FAIL(code) do { create_cuda_error = h->last_cuda ? h->last_cuda : (int)cudaGetLastError(); delete h; return (code); } while (0)
+#define TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { h->last_cuda = (int)e_; FAIL(DBEC_ECUDA); } } while (0)
+    create_cuda_error = 0;
+    TRY(cudaMemsetAsync(h->psi, 0, sizeof(cd) * h->P, h->stream));
+    TRY(cudaMemsetAsync(h->ticket, 0, 256, h->stream));
+    TRY(cudaMemsetAsync(h->spec, 0, sizeof(cd) * h->SP, h->stream));
     char* t = w + L.tables;
     const double om[3] = {p->nu, p->lambda, p->kappa};
     const double dd[3] = {p->dx, p->dy, p->ndim == 3 ? p->dz : 1.0};
@@ -313,10 +297,11 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
         if (rc) FAIL(rc);
         t += used;
     }
-    if (h->use_tma && dbec_make_tensor_maps(h)) FAIL(DBEC_ECUDA);
+    if (h->use_tma) TRY((cudaError_t)dbec_make_tensor_maps(h));
     if (write_scalars(h, true)) FAIL(DBEC_ECUDA);
-    if (dbec_launch_build_vdd(h)) FAIL(DBEC_ECUDA);
-    if (cudaStreamSynchronize(h->stream) != cudaSuccess) FAIL(DBEC_ECUDA);
+    TRY((cudaError_t)dbec_launch_build_vdd(h));
+    TRY(cudaStreamSynchronize(h->stream));
+#undef TRY
 #undef FAIL
     *out = h;
     return DBEC_OK;
@@ -330,7 +315,14 @@ int dbec_destroy(dbec_handle h) {
     return DBEC_OK;
 }
 
-int dbec_last_cuda_error(dbec_handle h) { return h ? h->last_cuda : 0; }
+int dbec_last_cuda_error(dbec_handle h) { return h ? h->last_cuda : create_cuda_error; }
+
+const char* dbec_build_id(void) {
+#ifndef DBEC_BUILD_ID_STR
+#define DBEC_BUILD_ID_STR "unknown"
+#endif
+    return "DBEC_BUILD_ID=" DBEC_BUILD_ID_STR;
+}
 
 int dbec_set_psi(dbec_handle h, const void* psi, int on_device) {
     if (!h || !psi) return DBEC_EINVAL;
@@ -405,6 +397,9 @@ int dbec_cn_sweep(dbec_handle h, int axis) {
 
 int dbec_nonlinear(dbec_handle h) {
     if (!h) return DBEC_EINVAL;
+    // the nonlinear kernel multiplies by the deferred norm factor s but leaves it in place (inside a step the
+    // last sweep rewrites it): bring the stored field to s = 1 first, or every later consumer applies s again
+    LAUNCH(h, dbec_launch_apply_scale(h));
     { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
     LAUNCH(h, dbec_launch_nonlinear(h, 0));
     return DBEC_OK;
@@ -413,6 +408,9 @@ int dbec_nonlinear(dbec_handle h) {
 int dbec_normalize(dbec_handle h) {
     if (!h) return DBEC_EINVAL;
     LAUNCH(h, dbec_launch_normalize(h));
+    // real time never rewrites the factor (no calcnorm inside its step) and dbec_get_psi does not apply it:
+    // apply it now, so that s is 1 again and the field stays normalised instead of being rescaled every step
+    if (h->p.time_mode == 1) LAUNCH(h, dbec_launch_apply_scale(h));
     return DBEC_OK;
 }
 
@@ -466,11 +464,9 @@ const char* dbec_pass_kernel(dbec_handle h, int slot) {
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
     switch (slot) {
         case KS_DENS_FFTX: return dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
-        case KS_FFT_SPECTRAL: return dbec_spectral_supported(h) ? "k_fft_spectral" : "";
         case KS_FFT_Y_FWD: case KS_FFT_Y_INV:
-            if (dbec_spectral_supported(h)) return "";
             return h->p.ndim == 3 ? (dbec_tma_supported(h, 1) ? "k_fft_tma" : "k_fft_strided") : "";
-        case KS_FFT_LAST_FMI: if (dbec_spectral_supported(h)) return "";
+        case KS_FFT_LAST_FMI:
             return dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
         case KS_IFFTX_NONLIN: return (h->fuse_cnx && dbec_xline_supported(h)) ? "k_xline_nonlin" : "k_ifftx_nonlin";
         case KS_CN_X: return h->fuse_cnx ? "" : "k_cn_x";

@@ -8,7 +8,7 @@
 #include "cplx.cuh"
 
 #define DBEC_MAX_N 512          // longest supported grid line (16 values per thread x 32 lanes)
-#define DBEC_MAX_KERNELS 9      // kernel slots of one step (dbec_step_profile)
+#define DBEC_MAX_KERNELS 8      // kernel slots of one step (dbec_step_profile)
 #define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
 #define DBEC_TMAP_BYTES 128     // sizeof(CUtensorMap)
 
@@ -59,7 +59,6 @@ struct dbec_handle_s {
     double* scal;                   // SC_COUNT doubles
     double* partial;                // reduction partials
     unsigned int* ticket;           // last-block tickets
-    int* sync;                      // k_fft_spectral: finished-tile counters per block of tiles (256 ints)
     double* obs_dev;                // 16 doubles
     AxisTables ax[3];
     int npartial;
@@ -72,15 +71,13 @@ struct dbec_handle_s {
     int prof_slot[DBEC_MAX_KERNELS];
     int use_graph;                  // env DBEC_GRAPH (default 1): replay one captured step per dbec_step iteration
     int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
-    int use_tma;                    // env DBEC_TMA (default 1): persistent TMA-fed kernels for lines of 128..512 points
+    int use_tma;                    // 1: persistent TMA-fed kernels for lines of 128..512 points
     int num_sms;
-    int use_pdl;                    // env DBEC_PDL (default 1): programmatic dependent launch of the persistent kernels
+    int use_pdl;                    // 1: programmatic dependent launch of every kernel of a step
     int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
-    int use_rev;                    // env DBEC_REV (default 1)
-    // L2 eviction policy code of every bulk / TMA access site (tma_pipe.cuh: l2_policy_code); env DBEC_POL
+    int use_rev;                    // 1: consecutive plane-ordered passes walk their tiles in opposite directions
+    // L2 eviction policy code of every bulk / TMA access site (tma_pipe.cuh: l2_policy_code)
     float pol[POL_COUNT];
-    int use_spectral;               // env DBEC_SPECTRAL (default 0): y/z transforms of a step in one kernel (k_fft_spectral)
-    int spec_xg, spec_lag;          // its tile list: column tiles per group (env DBEC_SPEC_XG, 1), lag in groups (DBEC_SPEC_LAG, 2)
     alignas(64) unsigned char tmap[TM_COUNT][DBEC_TMAP_BYTES];
 };
 
@@ -100,8 +97,6 @@ int dbec_make_tensor_maps(dbec_handle_s* h);
 int dbec_tma_supported(const dbec_handle_s* h, int axis);
 int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs);
 int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nzs);
-int dbec_spectral_supported(const dbec_handle_s* h);
-int dbec_launch_fft_spectral(dbec_handle_s* h);              // a1 (y, z) + a2 + a3 (z, y) in one kernel
 // persistent bulk-copy-fed versions of the x passes (kernels_xline.cu)
 int dbec_xline_supported(const dbec_handle_s* h);
 int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs);          // a3 (x) + a4 + a5

@@ -323,14 +323,14 @@ int dbec_launch_normalize(dbec_handle_s* h) {
     // true psi = s * stored psi: bring the stored field to s = 1 first, then take the norm factor
     int rc = dbec_launch_apply_scale(h);
     if (rc) return rc;
-    int nb = h->npartial < 148 * 8 ? h->npartial : 148 * 8;
+    int nb = h->npartial < h->num_sms * 8 ? h->npartial : h->num_sms * 8;
     k_norm<<<nb, 256, 0, h->stream>>>(h->psi, h->P, h->partial, h->ticket, h->scal, h->dV);
     h->launches++;
     return (int)cudaGetLastError();
 }
 
 int dbec_launch_apply_scale(dbec_handle_s* h) {
-    k_apply_scale<<<148 * 8, 256, 0, h->stream>>>(h->psi, h->P, h->scal);
+    k_apply_scale<<<h->num_sms * 8, 256, 0, h->stream>>>(h->psi, h->P, h->scal);
     k_reset_scale<<<1, 1, 0, h->stream>>>(h->scal);
     h->launches += 2;
     return (int)cudaGetLastError();
@@ -338,7 +338,7 @@ int dbec_launch_apply_scale(dbec_handle_s* h) {
 
 int dbec_launch_observables(dbec_handle_s* h) {
     int nb = h->npartial / OB_COUNT;
-    if (nb > 148 * 8) nb = 148 * 8;
+    if (nb > h->num_sms * 8) nb = h->num_sms * 8;
     k_obs_partial<<<nb, 256, 0, h->stream>>>(h->psi, h->phi, h->scal, h->ax[0].x2, h->ax[1].x2, h->ax[2].x2, h->nx,
                                              h->ny, h->nz, h->partial);
     const long long centre = (h->nx / 2) + (long long)h->nx * ((h->ny / 2) + (long long)h->ny * (h->p.ndim == 3 ? h->nz / 2 : 0));

@@ -362,7 +362,7 @@ int dbec_launch_phi_out(dbec_handle_s* h, double* phi) {
 }
 
 int dbec_launch_build_vdd(dbec_handle_s* h) {
-    k_build_vdd<<<148 * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->nx, h->ny, h->nz, h->nxhp, h->p.dx, h->p.dy,
+    k_build_vdd<<<h->num_sms * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->nx, h->ny, h->nz, h->nxhp, h->p.dx, h->p.dy,
                                                  h->p.dz, h->p.d_perp, h->p.cutoff, 1.0 / (double)h->P);
     h->launches++;
     return (int)cudaGetLastError();

@@ -285,146 +285,6 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
 }
 
 // ------------------------------------------------------------------------------------------------
-// All y/z transforms of a step in ONE kernel (a1 along y, z; a2; a3 along z, y), NY == NZ
-// ------------------------------------------------------------------------------------------------
-// The three passes  forward-y,  forward-z * V_dd * inverse-z,  inverse-y  touch the half spectrum three
-// times (48 B/pt + the V_dd table).  For one group of 8-column tiles the spectrum is only a few MiB: if
-// the three passes of a group follow each other closely it stays in the 126 MB L2 and HBM sees one read
-// and one write (16 B/pt + table).  So the tiles of all three passes are put in ONE list, ordered group
-// by group with a lag (block = all tiles of one pass of one group):
-//     A_0, A_1, B_0, A_2, B_1, C_0, A_3, B_2, C_1, ...        (A forward-y, B along z, C inverse-y)
-// and walked round-robin by one persistent CTA per SM.  A tile of B_g (C_g) may only be loaded when every
-// tile of A_g (B_g) has been stored: the storer bumps a global counter of the tile's block once its TMA
-// store has COMPLETED (wait_group 0), the loader of a dependent tile polls it (ld.acquire.gpu).  All
-// dependencies point backwards in the list, every CTA walks its tiles in order and all CTAs are resident
-// (cooperative launch), so the list always makes progress.
-//
-// MEASURED (round 1, C4): DRAM traffic of the three passes falls from 758 MB to 467 MB as intended, but
-// the time does not (148 us against 159 us for the three separate kernels, step time unchanged): an FFT
-// tile costs ~1.6 us of SM time (192-256 KB of shared-memory traffic per 32 KB tile at 128 B/clk, with
-// 8 worker warps per SM), which is what an HBM-fed tile costs as well.  OFF by default
-// (DBEC_SPECTRAL=1 turns it on); kept because it is the vehicle for the next reduction of HBM passes
-// once the per-tile shared-memory traffic is cut.
-#define SPEC_MAX_BLOCKS 112
-struct SpecOrder {
-    int nblocks, ntiles;
-    int start[SPEC_MAX_BLOCKS + 1];           // first tile of block b; start[nblocks] = ntiles
-    unsigned char phase[SPEC_MAX_BLOCKS];     // 0: A forward along y, 1: B forward * V_dd * inverse along z, 2: C inverse along y
-    unsigned char tx0[SPEC_MAX_BLOCKS];       // first column tile of the block's group
-    unsigned char gw[SPEC_MAX_BLOCKS];        // column tiles in the group
-    unsigned char dep[SPEC_MAX_BLOCKS];       // block that must be complete before a tile of this one loads (255: none)
-};
-
-struct SpecTile { int b, phase, tx, o; };
-__device__ __forceinline__ SpecTile spec_decode(const SpecOrder& so, int t, int& cur) {
-    while (t >= so.start[cur + 1]) ++cur;
-    SpecTile r; r.b = cur; r.phase = so.phase[cur];
-    const int idx = t - so.start[cur], gw = so.gw[cur];
-    r.tx = so.tx0[cur] + idx % gw;
-    r.o = idx / gw;
-    return r;
-}
-
-template <class P, int NG, int NST>
-__global__ void __launch_bounds__(NG* P::T* TCOLS + 96, 1)
-k_fft_spectral(const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z,
-               const __grid_constant__ SpecOrder so, const double* __restrict__ vdd, long long vdd_row_stride,
-               long long vdd_y_stride, const cd* twA_g, const cd* twN_g, int* __restrict__ cnt) {
-    constexpr int T = P::T, N = P::N, GT = T * TCOLS;
-    constexpr int STAGE_BYTES = N * TCOLS * (int)sizeof(cd);
-    extern __shared__ __align__(1024) unsigned char smraw[];
-    unsigned char* base = smraw;
-    uint64_t* bars = (uint64_t*)(base + (size_t)NST * STAGE_BYTES);
-    cd* tw = (cd*)(bars + ((3 * NST + 3) & ~1));
-    const int tid = threadIdx.x;
-    for (int k = tid; k < N; k += NG * GT + 96) { tw[k] = twA_g[k]; tw[N + k] = twN_g[k]; }
-    const cd* twA = tw; const cd* twN = tw + N;
-    const PipeBars pb = pipe_init<NST>(bars, GT / 32);
-    const int nmine = (so.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-    int cur = 0;
-    if (tid < NG * GT) {
-        const int g = tid / GT, r = tid % GT, col = r % TCOLS, m = r / TCOLS;
-        for (int i = g; i < nmine; i += NG) {
-            const int s = i % NST;
-            const SpecTile t = spec_decode(so, blockIdx.x + i * gridDim.x, cur);
-            // V_dd(k)/P of this thread's 16 spectrum points (the paper's `potdd`), straight from global
-            // memory into registers while the tile is still on its way: no shared-memory stage for it
-            double w[16];
-            if (t.phase == 1) {
-                const double* wp = vdd + (long long)t.o * vdd_y_stride + t.tx * TCOLS + col;
-#pragma unroll
-                for (int j = 0; j < 16; ++j) w[j] = __ldg(wp + (long long)(j * T + m) * vdd_row_stride);
-            }
-            wait_issued(pb.issued, i);
-            mbar_wait(pb.full + s, (i / NST) & 1);
-            cd* sm = (cd*)(base + (size_t)s * STAGE_BYTES) + col;
-            cd v[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) v[j] = sm[(j * T + m) * TCOLS];
-            if (t.phase != 2) fft_line_nb<P, -1>(v, m, sm, twA, twN, 1 + g, GT);
-            if (t.phase == 1) {
-#pragma unroll
-                for (int j = 0; j < 16; ++j) v[j] = cmul(w[j], v[j]);
-                named_bar_sync(1 + g, GT);                          // stage-2 reads of the forward pass are over
-            }
-            if (t.phase != 0) fft_line_nb<P, +1>(v, m, sm, twA, twN, 1 + g, GT);
-            named_bar_sync(1 + g, GT);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) sm[(j * T + m) * TCOLS] = v[j];
-            fence_proxy_async();
-            __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(pb.done + s);
-        }
-    } else if (tid == NG * GT) {
-        int okb = -1;                                               // last block whose dependency was seen complete
-        for (int i = 0; i < nmine; ++i) {
-            const int s = i % NST;
-            const SpecTile t = spec_decode(so, blockIdx.x + i * gridDim.x, cur);
-            const int dep = so.dep[t.b];
-            if (dep != 255 && okb != t.b) {
-                const int need = so.start[dep + 1] - so.start[dep];
-                while (ld_acquire_gpu(cnt + dep) < need) __nanosleep(200);
-                fence_proxy_async_all();
-                okb = t.b;
-            }
-            if (i >= NST) mbar_wait(pb.empty + s, ((i / NST) - 1) & 1);
-            st_release_shared(pb.issued, i + 1);
-            unsigned char* dst = base + (size_t)s * STAGE_BYTES;
-            mbar_expect_tx(pb.full + s, STAGE_BYTES);
-            if (t.phase == 1) tma_load_3d(dst, &map_z, t.tx * 2 * TCOLS, t.o, 0, pb.full + s);
-            else tma_load_3d(dst, &map_y, t.tx * 2 * TCOLS, 0, t.o, pb.full + s);
-        }
-    } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
-        const int which = (tid - NG * GT) / 32 - 1;
-        int pend = -1;                                              // block of this storer's previous store, not yet announced
-        for (int i = 0; i < nmine; ++i) {
-            const int s = i % NST;
-            if ((s & 1) != which) continue;
-            const SpecTile t = spec_decode(so, blockIdx.x + i * gridDim.x, cur);
-            // nothing to store yet: use the time to announce the pending store (it may be the very one the
-            // next tile's load is waiting for, so this must not be put off until after the wait)
-            if (pend >= 0 && !mbar_test_wait(pb.done + s, (i / NST) & 1)) {
-                bulk_wait<0>(); fence_proxy_async_all(); red_release_gpu_add(cnt + pend, 1);
-                pend = -1;
-            }
-            mbar_wait(pb.done + s, (i / NST) & 1);
-            const unsigned char* src = base + (size_t)s * STAGE_BYTES;
-            if (t.phase == 1) tma_store_3d(&map_z, t.tx * 2 * TCOLS, t.o, 0, src);
-            else tma_store_3d(&map_y, t.tx * 2 * TCOLS, 0, t.o, src);
-            bulk_commit();
-            bulk_wait_read<0>();
-            mbar_arrive(pb.empty + s);
-            // announce the PREVIOUS store once it is complete in global memory (wait_group 1: all but the
-            // newest group), so that this thread never idles on a write acknowledgement
-            if (pend >= 0) { bulk_wait<1>(); fence_proxy_async_all(); red_release_gpu_add(cnt + pend, 1); }
-            pend = t.phase != 2 ? t.b : -1;
-        }
-        bulk_wait<0>();
-        if (pend >= 0) { fence_proxy_async_all(); red_release_gpu_add(cnt + pend, 1); }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
 // tensor maps
 // ------------------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -475,10 +335,10 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-static TileGeom geom_of(const dbec_handle_s* h, int axis, int row_elems, int z0, int nzs) {
+static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int nzs) {
     TileGeom tg;
     tg.rev = h->rev_next;
-    const bool sp = row_elems == h->nxhp;
+    const int row_elems = sp ? h->nxhp : h->nx;          // a pass over the half spectrum or over psi
     tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
     tg.pol_st = h->pol[sp ? POL_FFT_ST : POL_CN_ST];
     tg.axis = axis;
@@ -495,7 +355,7 @@ static int grid_of(const dbec_handle_s* h, int ntiles) { return ntiles < h->num_
 
 template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
     constexpr int GT = NCH * TCOLS, STAGE = NCH * CN_L * TCOLS * (int)sizeof(cd);
-    const TileGeom tg = geom_of(h, axis, h->nx, z0, nzs);
+    const TileGeom tg = geom_of(h, axis, false, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
     if (NORM && grid > h->npartial) return (int)cudaErrorInvalidValue;
     const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 4) * sizeof(uint64_t) +
@@ -538,7 +398,7 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
     typedef typename PlanS<N>::P P;
     constexpr int GT = P::T * TCOLS;
     constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? N * TCOLS * (int)sizeof(double) : 0);
-    const TileGeom tg = geom_of(h, axis, h->nxhp, z0, nzs);
+    const TileGeom tg = geom_of(h, axis, true, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
     const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 4) * sizeof(uint64_t) + 2 * N * sizeof(cd);
     auto k = k_fft_tma<P, MODE, NG, NST>;
@@ -563,70 +423,4 @@ int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs) {
     if (mode == 0) return launch_fft_tma_n<0>(h, axis, z0, nzs);
     if (mode == 1) return launch_fft_tma_n<1>(h, axis, z0, nzs);
     return launch_fft_tma_n<2>(h, axis, z0, nzs);
-}
-
-// ------------------------------------------------------------------------------------------------
-// k_fft_spectral: tile list and launch
-// ------------------------------------------------------------------------------------------------
-int dbec_spectral_supported(const dbec_handle_s* h) {
-    return h->use_tma && h->use_spectral && h->p.ndim == 3 && h->ny == h->nz && (h->ny == 128 || h->ny == 256) &&
-           3 * ((h->nxhp / TCOLS + h->spec_xg - 1) / h->spec_xg) <= SPEC_MAX_BLOCKS;
-}
-
-// Groups of xg column tiles; block order A_s, B_{s-lag}, C_{s-2 lag} for s = 0, 1, ...
-static void make_spec_order(const dbec_handle_s* h, SpecOrder* so) {
-    const int ntx = h->nxhp / TCOLS, xg = h->spec_xg, lag = h->spec_lag, NL = h->ny;
-    const int G = (ntx + xg - 1) / xg;
-    int id[3][SPEC_MAX_BLOCKS];
-    int nb = 0, t = 0;
-    for (int s = 0; s < G + 2 * lag; ++s) {
-        for (int ph = 0; ph < 3; ++ph) {
-            const int g = s - ph * lag;
-            if (g < 0 || g >= G) continue;
-            const int gw = (g == G - 1) ? ntx - g * xg : xg;
-            so->phase[nb] = (unsigned char)ph;
-            so->tx0[nb] = (unsigned char)(g * xg);
-            so->gw[nb] = (unsigned char)gw;
-            so->dep[nb] = ph == 0 ? 255 : (unsigned char)id[ph - 1][g];
-            so->start[nb] = t;
-            id[ph][g] = nb;
-            t += gw * NL;
-            ++nb;
-        }
-    }
-    so->start[nb] = t;
-    so->nblocks = nb;
-    so->ntiles = t;
-}
-
-template <int N, int NG, int NST> static int launch_fft_spectral(dbec_handle_s* h) {
-    typedef typename PlanS<N>::P P;
-    constexpr int GT = P::T * TCOLS;
-    constexpr int STAGE = N * TCOLS * (int)sizeof(cd);
-    SpecOrder so;
-    make_spec_order(h, &so);
-    const int grid = grid_of(h, so.ntiles);
-    const size_t sm = (size_t)NST * STAGE + (3 * NST + 4) * sizeof(uint64_t) + 2 * N * sizeof(cd);
-    auto k = k_fft_spectral<P, NG, NST>;
-    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    CK(cudaMemsetAsync(h->sync, 0, sizeof(int) * so.nblocks, h->stream));
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(NG * GT + 96); cfg.dynamicSmemBytes = sm; cfg.stream = h->stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;      // all CTAs resident: they wait on one another
-    cfg.attrs = at; cfg.numAttrs = 1;
-    const CUtensorMap* my = (const CUtensorMap*)h->tmap[TM_SPEC_Y];
-    const CUtensorMap* mz = (const CUtensorMap*)h->tmap[TM_SPEC_Z];
-    const long long vrow = (long long)h->ny * h->nxhp, vy = h->nxhp;     // V_dd table: stride of a z row, of a y line
-    CK(cudaLaunchKernelEx(&cfg, k, *my, *mz, so, (const double*)h->vdd, vrow, vy, h->ax[1].twA, h->ax[1].twN, h->sync));
-    h->launches++;
-    return (int)cudaGetLastError();
-}
-
-int dbec_launch_fft_spectral(dbec_handle_s* h) {
-    switch (h->ny) {
-        case 128: return launch_fft_spectral<128, 4, 12>(h);
-        case 256: return launch_fft_spectral<256, 2, 6>(h);
-        default: return (int)cudaErrorInvalidValue;
-    }
 }

@@ -69,20 +69,6 @@ __device__ __forceinline__ void wait_issued(const int* issued, int i) {
     while (ld_acquire_shared(issued) <= i) __nanosleep(64);
 }
 
-// ---- CTA -> CTA hand-over through global memory (k_fft_spectral): a counter per block of tiles ----
-__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
-    int v;
-    asm volatile("ld.acquire.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void red_release_gpu_add(int* p, int v) {
-    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-// orders generic-proxy and async-proxy accesses of this thread in every state space (a counter read with
-// ld.acquire, then a TMA load of what another CTA's TMA store wrote; a completed TMA store, then the
-// counter update)
-__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
-
 // generic-proxy writes to shared memory become visible to the async proxy (TMA store reads them)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 

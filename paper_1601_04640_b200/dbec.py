@@ -21,8 +21,8 @@ DBEC_OK, DBEC_EINVAL, DBEC_ESIZE, DBEC_EWORKSPACE, DBEC_ECUDA, DBEC_ENODEVICE = 
 EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi", "dbec_set_coupling",
            "dbec_step", "dbec_observables", "dbec_destroy", "dbec_strerror", "dbec_last_cuda_error",
            "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
-           "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel"]
-KERNEL_SLOTS = 9
+           "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel", "dbec_build_id"]
+KERNEL_SLOTS = 8
 
 
 class DbecParams(C.Structure):
@@ -56,11 +56,11 @@ _lib = None
 
 
 def lib():
-    """Load libdbec.so (building it in-tree with nvcc if it is missing or stale)."""
+    """Load libdbec.so (building it in-tree with nvcc if it is missing or was built from other sources:
+    build() compares the source hash inside the library with the tree and is a no-op when they agree)."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH) or os.environ.get("DBEC_REBUILD"):
-            _build.build()
+        _build.build()
         L = C.CDLL(LIB_PATH)
         pp, vp = C.POINTER(DbecParams), C.c_void_p
         L.dbec_workspace_bytes.argtypes = [pp, C.POINTER(C.c_size_t)]
@@ -85,6 +85,8 @@ def lib():
         L.dbec_kernel_name.restype = C.c_char_p
         L.dbec_pass_kernel.argtypes = [vp, C.c_int]
         L.dbec_pass_kernel.restype = C.c_char_p
+        L.dbec_build_id.argtypes = []
+        L.dbec_build_id.restype = C.c_char_p
         _lib = L
     return _lib
 

@@ -119,6 +119,75 @@ def test_normalize_matches_oracle(gp, ob):
     sim.close()
 
 
+def test_normalize_in_real_time_is_applied_once(gp, ob):
+    """Real time never rewrites the deferred norm factor: dbec_normalize must apply it at once, or every
+    later step multiplies psi by it again (round-1 advisor finding)."""
+    w = grid3(32, 16, 64, REAL)
+    psi0 = 1.7 * random_psi(w, 8)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    sim.normalize()
+    assert relerr(sim.get_psi(), ob.normalize(ob.params_of(w), psi0)) < PSI_TOL
+    sim.step(3)
+    got = sim.get_psi()
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(ob.normalize(ob.params_of(w), psi0))
+    o.step(3)
+    assert relerr(got, o.get_psi()) < PSI_TOL
+    assert abs(sim.observables()["norm"] - o.observables()["norm"]) < 1e-13
+    sim.close()
+    o.close()
+
+
+@pytest.mark.parametrize("shape", [(32, 32, 32), (128, 16, 16)])
+def test_nonlinear_after_imaginary_time_steps(gp, ob, shape):
+    """After an imaginary-time step the stored field carries a deferred factor s != 1; dbec_nonlinear must
+    not apply it twice (round-1 advisor finding)."""
+    w = grid3(*shape, IMAG)
+    psi0 = 1.3 * initial_psi(w)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    sim.step(2)
+    sim.nonlinear()
+    got = sim.get_psi()
+    p = ob.params_of(w)
+    o = ob.Oracle(p)
+    o.set_psi(psi0)
+    o.step(2)
+    mid = o.get_psi()
+    ref = ob.nonlinear(p, mid, ob.phi_dd(p, np.abs(mid) ** 2))
+    assert relerr(got, ref) < PSI_TOL
+    a = sim.observables()["norm"]
+    assert abs(a - ob.norm(p, ref)) < 1e-12
+    sim.close()
+    o.close()
+
+
+def test_device_pointer_psi_and_foreign_stream(gp, ob):
+    """dbec_set_psi / dbec_get_psi with DEVICE pointers (the hand-off between handles) on a handle whose
+    stream is not torch's current one, driven straight through the C ABI."""
+    import ctypes as C
+    import torch
+    w = grid3(64, 32, 16, REAL)
+    psi0 = random_psi(w, 4)
+    side = torch.cuda.Stream()
+    sim = gp.Dbec(gp.params_of(w), stream=side)
+    d_in = torch.from_numpy(psi0).cuda()
+    d_out = torch.empty_like(d_in)
+    torch.cuda.synchronize()
+    L = gp.lib()
+    assert L.dbec_set_psi(sim._h, C.c_void_p(d_in.data_ptr()), 1) == 0
+    assert L.dbec_step(sim._h, 2) == 0
+    assert L.dbec_get_psi(sim._h, C.c_void_p(d_out.data_ptr()), 1) == 0
+    side.synchronize()
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(psi0)
+    o.step(2)
+    assert relerr(d_out.cpu().numpy(), o.get_psi()) < PSI_TOL
+    sim.close()
+    o.close()
+
+
 def one_step_pair(gp, ob, w, psi0, steps=1):
     sim = gp.Dbec(gp.params_of(w))
     sim.set_psi(psi0)
@@ -211,28 +280,6 @@ def test_persistent_kernels_are_bit_reproducible(gp, shape, mode):
         else:
             assert np.array_equal(got, ref), f"repetition {rep} differs"
     sim.close()
-
-
-@pytest.mark.parametrize("n", [128, 256])
-def test_single_kernel_spectral_passes_agree(gp, monkeypatch, n):
-    """DBEC_SPECTRAL=1 runs forward-y, forward-z * V_dd * inverse-z and inverse-y as ONE persistent kernel
-    whose CTAs hand blocks of tiles to one another through global counters (k_fft_spectral); the
-    arithmetic per line is the same up to the compiler's choice of FMA contraction: Phi_dd and psi must
-    agree with the three-kernel result to round-off, and two runs of the single kernel bit for bit."""
-    w = grid3(n, n, n, REAL, dx=0.1)
-    psi0 = random_psi(w, seed=9)
-    outs = []
-    for flag in ("0", "1", "1"):
-        monkeypatch.setenv("DBEC_SPECTRAL", flag)
-        sim = gp.Dbec(gp.params_of(w))
-        assert ("k_fft_spectral" in sim.pass_kernels().values()) == (flag == "1")
-        sim.set_psi(psi0)
-        outs.append(sim.phi_dd().cpu().numpy().copy())
-        sim.step(2)
-        outs.append(sim.get_psi().copy())
-        sim.close()
-    assert relerr(outs[2], outs[0]) < 1e-14 and relerr(outs[3], outs[1]) < 1e-14
-    assert np.array_equal(outs[2], outs[4]) and np.array_equal(outs[3], outs[5])
 
 
 def test_full_run_C1_observables(gp, ob):
