@@ -8,7 +8,10 @@
  * Problem (readings S1, S2, S3 of DESIGN.md; PAPER.md prints no formula):
  *     i dpsi/dt = [ -1/2 Lap + V + G |psi|^2 + D Phi_dd ] psi,   int |psi|^2 = 1,
  *     V = 1/2 (nu^2 x^2 + lambda^2 y^2 + kappa^2 z^2),
- *     Phi_dd = F^-1[ V_dd(k) F[|psi|^2] ],  V_dd(k) = 3 k_z^2/|k|^2 - 1  (3-D; 0 at k = 0).
+ *     Phi_dd = F^-1[ V_dd(k) F[|psi|^2] ],  V_dd(k) = 3 k_z^2/|k|^2 - 1  (3-D; 0 at k = 0);
+ *     2-D: that kernel averaged over the frozen Gaussian direction of width d_perp (S21, S25).
+ * The six programs of the paper are the parameter sets (ndim, plane, time_mode) =
+ *     imag2dXY (2,0,0)  imag2dXZ (2,1,0)  imag3d (3,0,0)  real2dXY (2,0,1)  real2dXZ (2,1,1)  real3d (3,0,1).
  * One step (PAPER.md:67 function list; order = reading S10):
  *     calcpsidd2 (density -> FFT -> x V_dd -> inverse FFT), calcnu (psi *= exp(-c dt (V+G n+D Phi))),
  *     calclux, calcluy, calcluz (Crank-Nicolson tridiagonal solve on every grid line),
@@ -46,7 +49,11 @@ typedef struct dbec_handle_s* dbec_handle;
 
 typedef struct {
     int32_t ndim;              /* 2 or 3                                                            */
-    int32_t plane;             /* 2-D only: 0 = XY (dipoles perpendicular to the plane)             */
+    int32_t plane;             /* 2-D only: 0 = XY (dipoles along the frozen axis, reading S21);
+                                  1 = XZ (dipoles IN the plane, the imag2dXZ / real2dXZ programs of
+                                  PAPER.md:15, :119-131, :163-177, reading S25): the second grid axis
+                                  (ny, dy, lambda) is then the polarisation axis z and y is frozen;
+                                  must be 0 in 3-D                                                   */
     int32_t nx, ny, nz;        /* nz = 1 in 2-D                                                     */
     double  dx, dy, dz;        /* grid spacings (dz ignored in 2-D)                                 */
     double  dt;                /* time step                                                         */

@@ -63,6 +63,8 @@ def lib():
         L.dbec_oracle_vdd3d.restype = C.c_double
         L.dbec_oracle_vdd2d.argtypes = [C.c_double] * 3
         L.dbec_oracle_vdd2d.restype = C.c_double
+        L.dbec_oracle_vdd2d_xz.argtypes = [C.c_double] * 3
+        L.dbec_oracle_vdd2d_xz.restype = C.c_double
         L.dbec_oracle_wavenumber.argtypes = [C.c_int, C.c_int, C.c_double]
         L.dbec_oracle_wavenumber.restype = C.c_double
         L.dbec_oracle_vdd_table.argtypes = [pp, dp]
@@ -91,7 +93,7 @@ def params_of(w, G=None, D=None) -> OracleParams:
     """OracleParams from any object with the Workload attribute names (duck-typed)."""
     return params(w.ndim, w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.dt, w.nu, w.lam, w.kappa,
                   w.G if G is None else G, w.D if D is None else D, w.time_mode,
-                  d_perp=w.d_perp, cutoff=w.cutoff)
+                  d_perp=w.d_perp, cutoff=w.cutoff, plane=getattr(w, "plane", 0))
 
 
 def _dp(a: np.ndarray):
@@ -172,6 +174,10 @@ def vdd3d(kx, ky, kz, cutoff=0.0):
 
 def vdd2d(kx, ky, d_perp):
     return lib().dbec_oracle_vdd2d(kx, ky, d_perp)
+
+
+def vdd2d_xz(kx, kz, d_perp):
+    return lib().dbec_oracle_vdd2d_xz(kx, kz, d_perp)
 
 
 def wavenumber(m, n, d):

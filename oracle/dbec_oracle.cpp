@@ -14,7 +14,8 @@
 //                             its definition (S7, S8), evaluated by a textbook iterative radix-2
 //                             FFT whose twiddles come from cos/sin of the exact angle; a separate
 //                             O(N^2) sum (oracle_dft_naive_*) pins it.
-//   * oracle_vdd3d / _vdd2d   PAPER.md:63, :75 (`potdd`) under readings S3, S4, S5, S6, S21.
+//   * oracle_vdd3d / _vdd2d   PAPER.md:63, :75 (`potdd`) under readings S3, S4, S5, S6, S21; _vdd2d_xz:
+//                             the in-plane-dipole kernel of the 2dXZ programs, reading S25.
 //   * oracle_phi_dd           PAPER.md:63, :71 (`calcpsidd2`): n -> DFT -> x V_dd -> inverse DFT.
 //                             Plain complex-to-complex transforms of the full grid; the paper's
 //                             R2C/C2R trick (:71) is an optimisation that reaches the same numbers.
@@ -51,7 +52,7 @@ extern "C" {
 // Same field order as the product's dbec_params, declared again on purpose (no shared header).
 typedef struct {
     int32_t ndim;       // 2 or 3
-    int32_t plane;      // 2-D only: 0 = XY
+    int32_t plane;      // 2-D only: 0 = XY (dipoles along the frozen z), 1 = XZ (dipoles in the plane, S25)
     int32_t nx, ny, nz; // nz = 1 in 2-D
     double dx, dy, dz;
     double dt;
@@ -205,8 +206,23 @@ static double vdd2d(double kx, double ky, double d_perp) {
     return 2.0 - 3.0 * std::sqrt(PI) * xi * erfcx_pos(xi);   // S21
 }
 
+// S25 (the imag2dXZ / real2dXZ programs): 2-D in the x-z plane, the
+// dipoles (along z) lie IN the plane and y is the frozen Gaussian direction of width d_perp.  The 3-D
+// kernel averaged over k_y with the weight of that Gaussian,
+//   int dk_y  d/sqrt(2 pi) exp(-k_y^2 d^2 / 2) (3 k_z^2 / (k_x^2 + k_y^2 + k_z^2) - 1)
+//     = -1 + 3 sqrt(pi) (xi_z^2 / xi) erfcx(xi),   xi = sqrt(k_x^2 + k_z^2) d/sqrt(2),  xi_z = k_z d/sqrt(2);
+// at k = 0 the second term vanishes (xi_z^2 <= xi^2): value -1.
+static double vdd2d_xz(double kx, double kz, double d_perp) {
+    double xi = std::sqrt(kx * kx + kz * kz) * d_perp / std::sqrt(2.0);
+    if (xi == 0.0) return -1.0;
+    double xiz = kz * d_perp / std::sqrt(2.0);
+    return -1.0 + 3.0 * std::sqrt(PI) * (xiz * xiz / xi) * erfcx_pos(xi);
+}
+
 static double vdd_at(const oracle_params& p, int mx, int my, int mz) {
     double kx = wavenumber(mx, p.nx, p.dx), ky = wavenumber(my, p.ny, p.dy);
+    // 2-D XZ: the second grid axis (ny, dy) IS the z axis
+    if (p.ndim == 2 && p.plane == 1) return vdd2d_xz(kx, ky, p.d_perp);
     if (p.ndim == 2) return vdd2d(kx, ky, p.d_perp);
     return vdd3d(kx, ky, wavenumber(mz, p.nz, p.dz), p.cutoff);
 }
@@ -222,6 +238,7 @@ static double coord(int i, int n, double d) { return (double)(i - n / 2) * d; } 
 static int check_params(const oracle_params* p) {
     if (!p) return -1;
     if (p->ndim != 2 && p->ndim != 3) return -1;
+    if (p->plane != 0 && !(p->ndim == 2 && p->plane == 1)) return -1;
     if (p->nx < 2 || p->ny < 2 || p->nz < 1) return -1;
     if (p->ndim == 2 && p->nz != 1) return -1;
     if (p->ndim == 3 && p->nz < 2) return -1;
@@ -507,6 +524,7 @@ int dbec_oracle_fft(double* a_c128, int nx, int ny, int nz, int sign, int naive)
 double dbec_oracle_erfcx(double x) { return erfcx_pos(x); }
 double dbec_oracle_vdd3d(double kx, double ky, double kz, double cutoff) { return vdd3d(kx, ky, kz, cutoff); }
 double dbec_oracle_vdd2d(double kx, double ky, double d_perp) { return vdd2d(kx, ky, d_perp); }
+double dbec_oracle_vdd2d_xz(double kx, double kz, double d_perp) { return vdd2d_xz(kx, kz, d_perp); }
 double dbec_oracle_wavenumber(int m, int n, double d) { return wavenumber(m, n, d); }
 
 // V_dd on the full index grid [nz][ny][nx].

@@ -18,7 +18,7 @@ static bool fft_len_ok(int n) { return n == 16 || n == 32 || n == 64 || n == 128
 static int check_params(const dbec_params* p) {
     if (!p) return DBEC_EINVAL;
     if (p->ndim != 2 && p->ndim != 3) return DBEC_EINVAL;
-    if (p->ndim == 2 && p->plane != 0) return DBEC_EINVAL;
+    if (p->plane != 0 && !(p->ndim == 2 && p->plane == 1)) return DBEC_EINVAL;
     if (p->time_mode != 0 && p->time_mode != 1) return DBEC_EINVAL;
     if (!(p->dx > 0.0) || !(p->dy > 0.0) || !(p->dt > 0.0)) return DBEC_EINVAL;
     if (p->ndim == 3 && !(p->dz > 0.0)) return DBEC_EINVAL;

@@ -209,7 +209,7 @@ __device__ __forceinline__ double wavenumber(int mi, int n, double d) {     // r
     return 6.283185307179586476925286766559 * (double)mt / ((double)n * d);
 }
 
-__global__ void k_build_vdd(double* __restrict__ vdd, int ndim, int nx, int ny, int nz, int nxhp, double dx,
+__global__ void k_build_vdd(double* __restrict__ vdd, int ndim, int plane, int nx, int ny, int nz, int nxhp, double dx,
                             double dy, double dz, double d_perp, double cutoff, double invP) {
     const long long total = (long long)nz * ny * nxhp;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
@@ -220,9 +220,15 @@ __global__ void k_build_vdd(double* __restrict__ vdd, int ndim, int nx, int ny, 
         double v = 0.0;
         if (mx <= nx / 2) {
             const double kx = wavenumber(mx, nx, dx), ky = wavenumber(my, ny, dy);
-            if (ndim == 2) {                                                  // reading S21
+            if (ndim == 2) {
                 const double xi = sqrt(kx * kx + ky * ky) * d_perp * 0.70710678118654752440;
-                v = 2.0 - 3.0 * 1.7724538509055160272981674833411 * xi * erfcx(xi);
+                const double g = 3.0 * 1.7724538509055160272981674833411 * erfcx(xi);
+                if (plane == 0) {                                             // XY, reading S21: 2 - 3 sqrt(pi) xi erfcx(xi)
+                    v = 2.0 - g * xi;
+                } else {                                                      // XZ, reading S25: the second grid axis is z
+                    const double xiz = ky * d_perp * 0.70710678118654752440;  //   -1 + 3 sqrt(pi) (xi_z^2 / xi) erfcx(xi)
+                    v = xi > 0.0 ? -1.0 + g * (xiz * xiz / xi) : -1.0;
+                }
             } else {
                 const double kz = wavenumber(mz, nz, dz);
                 const double k2 = kx * kx + ky * ky + kz * kz;
@@ -362,7 +368,7 @@ int dbec_launch_phi_out(dbec_handle_s* h, double* phi) {
 }
 
 int dbec_launch_build_vdd(dbec_handle_s* h) {
-    k_build_vdd<<<h->num_sms * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->nx, h->ny, h->nz, h->nxhp, h->p.dx, h->p.dy,
+    k_build_vdd<<<h->num_sms * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->p.plane, h->nx, h->ny, h->nz, h->nxhp, h->p.dx, h->p.dy,
                                                  h->p.dz, h->p.d_perp, h->p.cutoff, 1.0 / (double)h->P);
     h->launches++;
     return (int)cudaGetLastError();

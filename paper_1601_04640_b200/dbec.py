@@ -100,7 +100,7 @@ def params_of(w, G=None, D=None) -> DbecParams:
     """DbecParams from an object with the attribute names of inputs.Workload (duck-typed)."""
     return params(w.ndim, w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.dt, w.nu, w.lam, w.kappa,
                   w.G if G is None else G, w.D if D is None else D, w.time_mode,
-                  d_perp=w.d_perp, cutoff=w.cutoff)
+                  d_perp=w.d_perp, cutoff=w.cutoff, plane=getattr(w, "plane", 0))
 
 
 def workspace_bytes(p: DbecParams) -> int:

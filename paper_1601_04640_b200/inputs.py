@@ -40,6 +40,7 @@ class Workload:
     report_every: int
     d_perp: float = 1.0
     cutoff: float = 0.0
+    plane: int = 0    # 2-D only: 0 = XY, 1 = XZ (the second grid axis ny/dy/lam is then the polarisation axis z)
 
     @property
     def shape(self):
@@ -55,13 +56,13 @@ class Workload:
         return self.dx * self.dy * (self.dz if self.ndim == 3 else 1.0)
 
 
-def _w(name, ndim, n, d, dt, trap, G, D, mode, steps, seed, every, G_run=None, D_run=None):
+def _w(name, ndim, n, d, dt, trap, G, D, mode, steps, seed, every, G_run=None, D_run=None, plane=0):
     nx, ny, nz = n
     dx, dy, dz = d
     nu, lam, kappa = trap
     return Workload(name, ndim, nx, ny, nz, dx, dy, dz, dt, nu, lam, kappa, G, D,
                     G if G_run is None else G_run, D if D_run is None else D_run,
-                    mode, steps, seed, every)
+                    mode, steps, seed, every, plane=plane)
 
 
 # BASELINE.json `configs`, in order.
@@ -76,6 +77,15 @@ WORKLOADS = {
              200.0, 150.0, REAL, 500, 4, 50, D_run=180.0),
     "C5": _w("imag3d_cigar_512x512x256", 3, (512, 512, 256), (0.08, 0.08, 0.16), 0.05 * 0.08 ** 2,
              (1.0, 1.0, 0.25), 400.0, 350.0, IMAG, 200, 5, 200),
+    # Not BASELINE.json configs: the three program variants of PAPER.md:15 that C1-C5 leave out (imag2dXY,
+    # imag2dXZ, real2dXZ), so that all six (ndim, plane, time mode) combinations have a full-run golden file.
+    # In the XZ plane the second grid axis (ny, dy, lam) is the polarisation axis z (reading S25).
+    "X0": _w("imag2dXY_256", 2, (256, 256, 1), (0.15, 0.15, 1.0), 0.1 * 0.15 ** 2, (1.0, 1.5, 0.0),
+             30.0, 20.0, IMAG, 600, 6, 200),
+    "X1": _w("imag2dXZ_256x128", 2, (256, 128, 1), (0.15, 0.2, 1.0), 0.1 * 0.15 ** 2, (1.0, 0.6, 0.0),
+             30.0, 15.0, IMAG, 600, 7, 200, plane=1),
+    "X2": _w("real2dXZ_512", 2, (512, 512, 1), (0.1, 0.1, 1.0), 0.5 * 0.1 ** 2, (1.0, 0.8, 0.0),
+             20.0, 12.0, REAL, 500, 8, 250, G_run=25.0, plane=1),
 }
 
 

@@ -1,6 +1,9 @@
 """Writes tests/golden/<key>.json: observables of a full BASELINE.json run computed by the CPU oracle.
 
-    python tests/golden/make_golden.py C1 C2 C3 [C4 C5]
+    python tests/golden/make_golden.py C1 C2 C3 [C4 C5] [X0 X1 X2]
+
+C1-C5 are the BASELINE.json configs; X0-X2 the remaining program variants of PAPER.md:15 (imag2dXY,
+imag2dXZ, real2dXZ; inputs.py).
 
 Calls only oracle/ (the plain fp64 CPU implementation written from the paper under the readings of
 DESIGN.md) and the seeded input generator; nothing from the CUDA path.  These are NOT values printed

@@ -36,9 +36,9 @@ def grid3(nx, ny, nz, mode, G=30.0, D=20.0, dx=0.4, dt=None, trap=(1.0, 1.2, 0.7
     return Workload("t3", 3, nx, ny, nz, d[0], d[1], d[2], dt, *trap, G, D, G, D, mode, 1, 21, 1, cutoff=cutoff)
 
 
-def grid2(nx, ny, mode, G=20.0, D=15.0, dx=0.2, dt=None, trap=(1.0, 1.5, 0.0), dy=None):
+def grid2(nx, ny, mode, G=20.0, D=15.0, dx=0.2, dt=None, trap=(1.0, 1.5, 0.0), dy=None, plane=0):
     dt = dt if dt is not None else (0.1 if mode == IMAG else 0.5) * dx ** 2
-    return Workload("t2", 2, nx, ny, 1, dx, dy or dx, 1.0, dt, *trap, G, D, G, D, mode, 1, 22, 1)
+    return Workload("t2", 2, nx, ny, 1, dx, dy or dx, 1.0, dt, *trap, G, D, G, D, mode, 1, 22, 1, plane=plane)
 
 
 SHAPES3 = [(16, 16, 16), (32, 32, 32), (64, 16, 32), (16, 64, 128), (128, 32, 16), (256, 16, 16), (16, 256, 32),
@@ -48,6 +48,8 @@ SHAPES2 = [(16, 16), (32, 64), (128, 32), (512, 16), (16, 512), (256, 256)]
 # Crank-Nicolson coefficient of every axis and the kinetic / rms sums each take their own spacing
 ANISO3 = [(32, 16, 64), (128, 32, 16), (16, 128, 128)]
 ANISO2 = [(64, 32), (128, 256)]
+# 2-D XZ plane (in-plane dipoles, reading S25; PAPER.md:15 imag2dXZ / real2dXZ): same kernels, another V_dd table
+XZ2 = [(32, 64), (256, 128), (512, 512)]
 
 
 def all_small_workloads():
@@ -61,12 +63,14 @@ def all_small_workloads():
             out.append(grid3(*s, mode, d=(0.4, 0.3, 0.6)))
         for s in ANISO2:
             out.append(grid2(*s, mode, dx=0.2, dy=0.3))
+        for s in XZ2:
+            out.append(grid2(*s, mode, dx=0.2, dy=0.25, plane=1))
     return out
 
 
 def wid(w):
     aniso = "" if (w.dx == w.dy and (w.ndim == 2 or w.dx == w.dz)) else "-aniso"
-    return f"{w.ndim}d-{w.nx}x{w.ny}x{w.nz}-{'imag' if w.time_mode == IMAG else 'real'}{aniso}"
+    return f"{w.ndim}d{'xz' if w.plane else ''}-{w.nx}x{w.ny}x{w.nz}-{'imag' if w.time_mode == IMAG else 'real'}{aniso}"
 
 
 @pytest.mark.parametrize("w", all_small_workloads(), ids=wid)
@@ -327,7 +331,7 @@ def test_errors_and_edge_cases(gp):
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 
 
-@pytest.mark.parametrize("key", ["C1", "C2", "C3", "C4", "C5"])
+@pytest.mark.parametrize("key", ["C1", "C2", "C3", "C4", "C5", "X0", "X1", "X2"])
 def test_full_run_observables_against_oracle_golden(gp, key):
     """BASELINE.json: mu, energy, rms after the full run within 1e-9 relative.  The expected values were
     written by tests/golden/make_golden.py, which calls only oracle/ (full oracle runs of C3-C5 take

@@ -41,6 +41,8 @@ def test_workspace_bytes_validation_is_host_only(gp):
     P, SP = 256 ** 3, 256 * 256 * 136
     assert n.value >= 16 * P + 16 * SP + 8 * SP + 8 * P
     assert n.value < 16 * P + 16 * SP + 8 * SP + 8 * P + (4 << 20)
+    xz = gp.params(2, 32, 32, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=1)
+    assert L.dbec_workspace_bytes(C.byref(xz), C.byref(n)) == gp.DBEC_OK
     assert L.dbec_workspace_bytes(None, C.byref(n)) == gp.DBEC_EINVAL
     assert L.dbec_workspace_bytes(C.byref(ok), None) == gp.DBEC_EINVAL
     for bad, code in [
@@ -52,7 +54,8 @@ def test_workspace_bytes_validation_is_host_only(gp):
         (gp.params(3, 32, 32, 32, 0., .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
         (gp.params(3, 32, 32, 32, .5, .5, .5, 0., 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
         (gp.params(3, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 2), gp.DBEC_EINVAL),      # time_mode
-        (gp.params(2, 32, 32, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=1), gp.DBEC_EINVAL),  # XZ: not built
+        (gp.params(2, 32, 32, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=2), gp.DBEC_EINVAL),  # 0 = XY, 1 = XZ
+        (gp.params(3, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=1), gp.DBEC_EINVAL),  # 3-D has no plane
     ]:
         assert L.dbec_workspace_bytes(C.byref(bad), C.byref(n)) == code
     assert b"grid length" in L.dbec_strerror(gp.DBEC_ESIZE)

@@ -400,13 +400,17 @@ def _numpy_step(w, psi, G, D, V_dd):
     return np.ascontiguousarray(psi)
 
 
-@pytest.mark.parametrize("key,mode,steps", [("C1", IMAG, 3), ("C1", REAL, 3), ("2d", REAL, 3), ("2d", IMAG, 2), ("aniso", REAL, 2)])
+@pytest.mark.parametrize("key,mode,steps", [("C1", IMAG, 3), ("C1", REAL, 3), ("2d", REAL, 3), ("2d", IMAG, 2), ("aniso", REAL, 2),
+                                            ("2dxz", REAL, 3), ("2dxz", IMAG, 2)])
 def test_full_step_against_numpy_scipy_restatement(ob, key, mode, steps):
     from dataclasses import replace
     if key == "C1":
         w = replace(workload("C1"), time_mode=mode)
     elif key == "2d":
         w = Workload("t", 2, 64, 32, 1, 0.2, 0.3, 1.0, 0.004, 1.0, 1.5, 0.0, 20.0, 15.0, 25.0, 15.0, mode, 1, 2, 1)
+    elif key == "2dxz":
+        w = Workload("t", 2, 32, 64, 1, 0.3, 0.2, 1.0, 0.004, 1.0, 0.7, 0.0, 20.0, 15.0, 25.0, 15.0, mode, 1, 2, 1,
+                     d_perp=0.8, plane=1)
     else:
         w = Workload("t", 3, 16, 32, 8, 0.4, 0.3, 0.8, 0.01, 1.0, 1.2, 0.8, 50.0, 40.0, 50.0, 45.0, mode, 1, 4, 1)
     p = ob.params_of(w)
@@ -449,6 +453,11 @@ def _numpy_vdd(w):
     ky = 2 * np.pi * np.fft.fftfreq(w.ny, w.dy)
     if w.ndim == 2:
         xi = np.sqrt(kx[None, :] ** 2 + ky[:, None] ** 2) * w.d_perp / math.sqrt(2.0)
+        if w.plane == 1:                                   # S25: second grid axis = polarisation axis z
+            xiz = np.broadcast_to(ky[:, None] * w.d_perp / math.sqrt(2.0), xi.shape)
+            with np.errstate(invalid="ignore", divide="ignore"):
+                r = np.where(xi > 0, xiz ** 2 / xi, 0.0)
+            return -1.0 + 3.0 * math.sqrt(math.pi) * r * scipy.special.erfcx(xi)
         return 2.0 - 3.0 * math.sqrt(math.pi) * xi * scipy.special.erfcx(xi)
     kz = 2 * np.pi * np.fft.fftfreq(w.nz, w.dz)
     KZ, KY, KX = np.meshgrid(kz, ky, kx, indexing="ij")
@@ -552,3 +561,61 @@ def test_density_max_off_centre(ob):
     assert r["density_max"] == 25.0
     assert r["density0"] == pytest.approx(abs(psi[4, 4, 8]) ** 2, rel=1e-15)
     assert r["density0"] < 1.0
+
+
+# ------------------------------------------------------------------ S25: 2-D XZ plane (in-plane dipoles)
+def test_vdd2d_xz_properties(ob):
+    sp = math.sqrt(math.pi)
+    assert ob.vdd2d_xz(0, 0, 1.0) == -1.0                              # k = 0
+    for kx in (0.1, 1.0, 7.0, 45.0):
+        assert ob.vdd2d_xz(kx, 0.0, 1.0) == pytest.approx(-1.0, abs=1e-15)   # k perpendicular to the dipoles
+    for kz in (1e-3, 0.3, 1.3, 5.0, 40.0, 90.0):                       # k along the dipoles: 1 - h(xi)
+        xi = kz / math.sqrt(2)
+        assert ob.vdd2d_xz(0.0, kz, 1.0) == pytest.approx(-1 + 3 * sp * xi * scipy.special.erfcx(xi), rel=1e-14)
+        assert ob.vdd2d_xz(0.0, kz, 1.0) == pytest.approx(1 - ob.vdd2d(kz, 0.0, 1.0), abs=1e-14)
+    assert ob.vdd2d_xz(0.0, 1e5, 1.0) == pytest.approx(2.0, abs=1e-9)  # sqrt(pi) xi erfcx(xi) -> 1
+    # even in both components, scales with d_perp, NOT isotropic
+    assert ob.vdd2d_xz(-0.7, 1.1, 0.9) == ob.vdd2d_xz(0.7, 1.1, 0.9) == ob.vdd2d_xz(0.7, -1.1, 0.9)
+    assert ob.vdd2d_xz(2.0, 1.0, 1.0) == pytest.approx(ob.vdd2d_xz(1.0, 0.5, 2.0), abs=1e-15)
+    assert abs(ob.vdd2d_xz(3.0, 4.0, 0.5) - ob.vdd2d_xz(4.0, 3.0, 0.5)) > 0.1
+    # library value at a generic point
+    kx, kz, d = 0.9, 1.7, 0.6
+    xi, xiz = math.hypot(kx, kz) * d / math.sqrt(2), kz * d / math.sqrt(2)
+    assert ob.vdd2d_xz(kx, kz, d) == pytest.approx(-1 + 3 * sp * xiz ** 2 / xi * scipy.special.erfcx(xi), rel=1e-14)
+    # the dipolar tensor is traceless: polarisation along z (in plane) + along x (in plane: swap the
+    # arguments) + along the frozen axis (the XY kernel h) sum to zero
+    for kx, kz in ((0.3, 0.4), (2.0, 0.1), (11.0, 35.0)):
+        tr = ob.vdd2d_xz(kx, kz, 1.0) + ob.vdd2d_xz(kz, kx, 1.0) + ob.vdd2d(kx, kz, 1.0)
+        assert abs(tr) < 4e-15
+    # defining property: the 3-D kernel (dipoles along z) averaged over k_y with the Gaussian weight of the
+    # frozen direction
+    ky = np.linspace(-40, 40, 400001)
+    wgt = np.exp(-ky ** 2 / 2.0) / math.sqrt(2 * math.pi)
+    for kx, kz in ((1.3, 0.0), (0.0, 1.3), (0.8, 1.9), (3.0, 0.5)):
+        avg = np.trapezoid((3 * kz ** 2 / (kx ** 2 + ky ** 2 + kz ** 2) - 1) * wgt, ky)
+        assert ob.vdd2d_xz(kx, kz, 1.0) == pytest.approx(avg, abs=1e-9)
+    # large arguments stay finite (C2-sized grids reach xi ~ 31, where exp(xi^2) erfc(xi) is inf * 0)
+    assert np.isfinite(ob.vdd2d_xz(30.0, 30.0, 1.0)) and -1 <= ob.vdd2d_xz(30.0, 30.0, 1.0) <= 2
+
+
+def test_phi_dd_2d_xz_plane_waves_and_table(ob):
+    w = Workload("t", 2, 16, 8, 1, 0.2, 0.35, 1.0, 0.01, 1, 1, 0, 0, 0, 0, 0, IMAG, 1, 1, 1, d_perp=0.7, plane=1)
+    p = ob.params_of(w)
+    assert p.plane == 1
+    jy, jx = np.meshgrid(np.arange(8), np.arange(16), indexing="ij")
+    for m in ((1, 0), (0, 1), (3, 2), (5, 3)):
+        wave = np.cos(2 * np.pi * (m[0] * jx / 16 + m[1] * jy / 8))
+        kx, kz = 2 * np.pi * m[0] / (16 * 0.2), 2 * np.pi * m[1] / (8 * 0.35)    # second grid axis = z
+        xi, xiz = math.hypot(kx, kz) * 0.7 / math.sqrt(2), kz * 0.7 / math.sqrt(2)
+        lam = -1 + 3 * math.sqrt(math.pi) * xiz ** 2 / xi * scipy.special.erfcx(xi)
+        assert np.max(np.abs(ob.phi_dd(p, wave) - lam * wave)) < 1e-13, m
+    assert np.max(np.abs(ob.vdd_table(p) - _numpy_vdd(w))) < 1e-14
+    # a uniform density feels V(0) = -1 (XY: +2)
+    assert np.max(np.abs(ob.phi_dd(p, np.full(w.shape, 0.25)) + 0.25)) < 1e-14
+    # plane is rejected in 3-D and for values other than 0 / 1
+    import ctypes as C
+    bad = ob.params(3, 8, 8, 8, .5, .5, .5, .01, 1, 1, 1, 0, 0, 0, plane=1)
+    h = C.c_void_p()
+    assert ob.lib().dbec_oracle_create(C.byref(bad), C.byref(h)) != 0
+    bad = ob.params(2, 8, 8, 1, .5, .5, .5, .01, 1, 1, 1, 0, 0, 0, plane=2)
+    assert ob.lib().dbec_oracle_create(C.byref(bad), C.byref(h)) != 0
