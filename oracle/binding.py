@@ -55,6 +55,10 @@ def lib():
         L.dbec_oracle_get_psi.argtypes = [C.c_void_p, dp]
         L.dbec_oracle_set_coupling.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.dbec_oracle_step.argtypes = [C.c_void_p, C.c_int]
+        L.dbec_oracle_set_ramp.argtypes = [C.c_void_p, C.c_int] + [C.c_double] * 4
+        L.dbec_oracle_get_coupling.argtypes = [C.c_void_p, dp, dp]
+        L.dbec_oracle_density_1d.argtypes = [C.c_void_p, C.c_int, dp]
+        L.dbec_oracle_density_2d.argtypes = [C.c_void_p, C.c_int, dp]
         L.dbec_oracle_observables.argtypes = [C.c_void_p, C.POINTER(OracleObs)]
         L.dbec_oracle_fft.argtypes = [dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
         L.dbec_oracle_erfcx.argtypes = [C.c_double]
@@ -144,6 +148,28 @@ class Oracle:
 
     def step(self, n=1):
         _check(lib().dbec_oracle_step(self._h, int(n)), "step")
+
+    def set_ramp(self, nstp, G0, D0, G1, D1):
+        _check(lib().dbec_oracle_set_ramp(self._h, int(nstp), G0, D0, G1, D1), "set_ramp")
+
+    def get_coupling(self):
+        g, d = C.c_double(), C.c_double()
+        _check(lib().dbec_oracle_get_coupling(self._h, C.byref(g), C.byref(d)), "get_coupling")
+        return g.value, d.value
+
+    def density_1d(self, axis) -> np.ndarray:
+        n = (self.p.nx, self.p.ny, self.p.nz)[axis]
+        out = np.empty(n, dtype=np.float64)
+        _check(lib().dbec_oracle_density_1d(self._h, int(axis), _dp(out)), "density_1d")
+        return out
+
+    def density_2d(self, axis) -> np.ndarray:
+        """axis = the integrated one; shape (nz, ny, nx) with that axis removed."""
+        shp = [self.p.nz, self.p.ny, self.p.nx]
+        del shp[2 - axis]
+        out = np.empty(shp, dtype=np.float64)
+        _check(lib().dbec_oracle_density_2d(self._h, int(axis), _dp(out)), "density_2d")
+        return out
 
     def observables(self) -> dict:
         o = OracleObs()

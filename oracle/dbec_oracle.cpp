@@ -25,6 +25,10 @@
 //   * oracle_normalize        PAPER.md:67 (`calcnorm`), reading S13.
 //   * oracle_observables      PAPER.md:67, :71 (`calcmuen`, `calcrms`), readings S13..S16.
 //   * dbec_oracle_step        the order nonlinear -> x -> y -> z -> norm (reading S10).
+//   * dbec_oracle_set_ramp    PAPER.md:157, :173, :191 ("NSTP"): linear ramp of G and D over the first
+//                             NSTP steps, reading S26.
+//   * dbec_oracle_density_*   PAPER.md:69 (output of the wave function): integrated 1-D / 2-D densities,
+//                             reading S27.
 //
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): naive DFT, Parseval, dense tridiagonal solve,
 // sine-mode closed form, sampled-Gaussian closed forms, V_dd symmetries, Gaussian dipolar-energy
@@ -71,6 +75,9 @@ struct oracle_state {
     oracle_params p;
     std::vector<cplx> psi;
     std::vector<double> vdd;   // V_dd(k) on the full index grid, built once (PAPER.md:75 `potdd`)
+    // S26: ramp of the nonlinear coefficients over the first NSTP steps ("NSTP")
+    int ramp_n = 0, ramp_k = 0;
+    double G0 = 0, D0 = 0, G1 = 0, D1 = 0;
 };
 
 } // extern "C"
@@ -494,12 +501,79 @@ int dbec_oracle_get_psi(oracle_state* s, double* psi_c128) {
 int dbec_oracle_set_coupling(oracle_state* s, double G, double D) {   // S18
     if (!s) return -1;
     s->p.G = G; s->p.D = D;
+    s->ramp_n = s->ramp_k = 0;                                        // an explicit value ends any ramp
+    return 0;
+}
+
+// S26: the k-th step after this call (k = 1..nstp) runs with G0 + (G1 - G0) k/nstp and
+// D0 + (D1 - D0) k/nstp; every later step with (G1, D1).  nstp = 0: (G1, D1) at once.
+int dbec_oracle_set_ramp(oracle_state* s, int nstp, double G0, double D0, double G1, double D1) {
+    if (!s || nstp < 0) return -1;
+    s->ramp_n = nstp; s->ramp_k = 0;
+    s->G0 = G0; s->D0 = D0; s->G1 = G1; s->D1 = D1;
+    if (nstp == 0) { s->p.G = G1; s->p.D = D1; }
+    else { s->p.G = G0; s->p.D = D0; }
+    return 0;
+}
+
+int dbec_oracle_get_coupling(oracle_state* s, double* G, double* D) {
+    if (!s || !G || !D) return -1;
+    *G = s->p.G; *D = s->p.D;
+    return 0;
+}
+
+// S27: integrated densities (the lineage's 1-D / 2-D density output, "wave function array is
+// returned back to CPU when it is required for writing output"): |psi|^2 summed over the other axes
+// times their spacings (plain sums, S13).
+//   1-D, axis a:           out[i_a]            = prod_{b != a} d_b  sum_{other indices} |psi|^2
+//   2-D, integrated axis a (3-D grids only): out over the two remaining axes, the lower axis fastest
+//                          (a = 2: [ny][nx], a = 1: [nz][nx], a = 0: [nz][ny]),  = d_a sum_{i_a} |psi|^2
+int dbec_oracle_density_1d(oracle_state* s, int axis, double* out) {
+    if (!s || !out || axis < 0 || axis >= s->p.ndim) return -1;
+    const oracle_params& p = s->p;
+    const int n[3] = {p.nx, p.ny, p.nz};
+    const double d[3] = {p.dx, p.dy, p.ndim == 3 ? p.dz : 1.0};
+    long double w = 1.0L;
+    for (int b = 0; b < p.ndim; ++b) if (b != axis) w *= d[b];
+    std::vector<long double> acc(n[axis], 0.0L);
+    for (int iz = 0; iz < p.nz; ++iz)
+        for (int iy = 0; iy < p.ny; ++iy)
+            for (int ix = 0; ix < p.nx; ++ix) {
+                const int idx[3] = {ix, iy, iz};
+                const cplx v = s->psi[ix + (long long)p.nx * (iy + (long long)p.ny * iz)];
+                acc[idx[axis]] += (long double)v.real() * v.real() + (long double)v.imag() * v.imag();
+            }
+    for (int i = 0; i < n[axis]; ++i) out[i] = (double)(acc[i] * w);
+    return 0;
+}
+
+int dbec_oracle_density_2d(oracle_state* s, int axis, double* out) {
+    if (!s || !out || s->p.ndim != 3 || axis < 0 || axis > 2) return -1;
+    const oracle_params& p = s->p;
+    const int n[3] = {p.nx, p.ny, p.nz};
+    const double d[3] = {p.dx, p.dy, p.dz};
+    const int lo = axis == 0 ? 1 : 0, hi = axis == 2 ? 1 : 2;          // the two axes that remain
+    std::vector<long double> acc((size_t)n[lo] * n[hi], 0.0L);
+    for (int iz = 0; iz < p.nz; ++iz)
+        for (int iy = 0; iy < p.ny; ++iy)
+            for (int ix = 0; ix < p.nx; ++ix) {
+                const int idx[3] = {ix, iy, iz};
+                const cplx v = s->psi[ix + (long long)p.nx * (iy + (long long)p.ny * iz)];
+                acc[idx[lo] + (size_t)n[lo] * idx[hi]] += (long double)v.real() * v.real() + (long double)v.imag() * v.imag();
+            }
+    for (size_t i = 0; i < acc.size(); ++i) out[i] = (double)(acc[i] * (long double)d[axis]);
     return 0;
 }
 
 int dbec_oracle_step(oracle_state* s, int nsteps) {
     if (!s || nsteps < 0) return -1;
     for (int i = 0; i < nsteps; ++i) {
+        if (s->ramp_k < s->ramp_n) {                                  // S26
+            s->ramp_k += 1;
+            const double f = (double)s->ramp_k / (double)s->ramp_n;
+            s->p.G = s->G0 + (s->G1 - s->G0) * f;
+            s->p.D = s->D0 + (s->D1 - s->D0) * f;
+        }
         int rc = one_step(s->p, s->vdd.data(), s->psi.data());
         if (rc) return rc;
     }

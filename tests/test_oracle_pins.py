@@ -619,3 +619,95 @@ def test_phi_dd_2d_xz_plane_waves_and_table(ob):
     assert ob.lib().dbec_oracle_create(C.byref(bad), C.byref(h)) != 0
     bad = ob.params(2, 8, 8, 1, .5, .5, .5, .01, 1, 1, 1, 0, 0, 0, plane=2)
     assert ob.lib().dbec_oracle_create(C.byref(bad), C.byref(h)) != 0
+
+
+# ------------------------------------------------------------------ S26: NSTP ramp of the nonlinearity
+@pytest.mark.parametrize("mode", [IMAG, REAL])
+def test_ramp_schedule_equals_explicit_couplings(ob, mode):
+    w = small3d(16, mode, G=0.0, D=0.0, dt=0.02)
+    p = ob.params_of(w)
+    psi0 = initial_psi(w)
+    G0, D0, G1, D1, n = 2.0, 1.0, 30.0, 18.0, 5
+    a = ob.Oracle(p)
+    a.set_psi(psi0)
+    a.set_ramp(n, G0, D0, G1, D1)
+    assert a.get_coupling() == (G0, D0)                # nothing has run yet
+    b = ob.Oracle(p)
+    b.set_psi(psi0)
+    for k in range(1, n + 4):
+        a.step(1)
+        f = min(k, n) / n                              # the schedule written out here, not taken from the oracle
+        b.set_coupling(G0 + (G1 - G0) * f, D0 + (D1 - D0) * f)
+        b.step(1)
+        assert a.get_coupling() == pytest.approx((G0 + (G1 - G0) * f, D0 + (D1 - D0) * f), rel=1e-15)
+        assert np.array_equal(a.get_psi(), b.get_psi()), k
+    assert a.get_coupling() == (G1, D1)                # exactly the end values once the ramp is over
+    # first ramp step is NOT at the start value: step 1 of n runs with G0 + (G1 - G0)/n
+    c = ob.Oracle(p)
+    c.set_psi(psi0)
+    c.set_coupling(G0, D0)
+    c.step(1)
+    d = ob.Oracle(p)
+    d.set_psi(psi0)
+    d.set_ramp(n, G0, D0, G1, D1)
+    d.step(1)
+    assert not np.array_equal(c.get_psi(), d.get_psi())
+    # nstp = 0: end values at once; set_coupling cancels a running ramp
+    e = ob.Oracle(p)
+    e.set_ramp(0, G0, D0, G1, D1)
+    assert e.get_coupling() == (G1, D1)
+    e.set_ramp(4, 0.0, 0.0, 8.0, 4.0)
+    e.set_psi(psi0)
+    e.step(1)
+    assert e.get_coupling() == (2.0, 1.0)
+    e.set_coupling(5.0, 5.0)
+    e.step(3)
+    assert e.get_coupling() == (5.0, 5.0)
+
+
+# ------------------------------------------------------------------ S27: integrated densities
+def test_integrated_densities_closed_form_and_numpy(ob):
+    om = (1.0, 1.3, 0.6)
+    d = (0.5, 0.4, 0.25)
+    w = Workload("t", 3, 32, 32, 64, *d, 0.01, *om, 0, 0, 0, 0, IMAG, 1, 1, 1)
+    o = ob.Oracle(ob.params_of(w))
+    cs = [axis_coords(n, dd) for n, dd in zip((32, 32, 64), d)]
+    g = [(om[i] / math.pi) ** 0.25 * np.exp(-0.5 * om[i] * c * c) for i, c in enumerate(cs)]
+    o.set_psi((g[2][:, None, None] * g[1][None, :, None] * g[0][None, None, :]).astype(complex))
+    # marginals of a product Gaussian: sqrt(om/pi) exp(-om x^2) (the sampled sums over the other axes are 1
+    # to ~1e-14, see test_observables_sampled_gaussian_anisotropic_spacing)
+    for ax in range(3):
+        n1 = o.density_1d(ax)
+        ref = math.sqrt(om[ax] / math.pi) * np.exp(-om[ax] * cs[ax] ** 2)
+        assert np.max(np.abs(n1 - ref)) < 1e-13, ax
+        assert np.sum(n1) * d[ax] == pytest.approx(1.0, abs=1e-13)
+    for ax in range(3):
+        n2 = o.density_2d(ax)
+        lo, hi = [b for b in range(3) if b != ax]
+        ref = np.outer(math.sqrt(om[hi] / math.pi) * np.exp(-om[hi] * cs[hi] ** 2),
+                       math.sqrt(om[lo] / math.pi) * np.exp(-om[lo] * cs[lo] ** 2))      # [hi][lo], lower axis fastest
+        assert n2.shape == ref.shape
+        assert np.max(np.abs(n2 - ref)) < 1e-13, ax
+    # a rough complex field: numpy sums with each axis' own spacing
+    wr = Workload("t", 3, 16, 8, 32, 0.3, 0.5, 0.7, 0.01, 1, 1, 1, 0, 0, 0, 0, REAL, 1, 1, 1)
+    psi = random_psi(wr, 4)
+    o2 = ob.Oracle(ob.params_of(wr))
+    o2.set_psi(psi)
+    n = np.abs(psi) ** 2                                              # [z][y][x]
+    assert np.allclose(o2.density_1d(0), n.sum(axis=(0, 1)) * 0.5 * 0.7, rtol=1e-13, atol=0)
+    assert np.allclose(o2.density_1d(1), n.sum(axis=(0, 2)) * 0.3 * 0.7, rtol=1e-13, atol=0)
+    assert np.allclose(o2.density_1d(2), n.sum(axis=(1, 2)) * 0.3 * 0.5, rtol=1e-13, atol=0)
+    assert np.allclose(o2.density_2d(2), n.sum(axis=0) * 0.7, rtol=1e-13, atol=0)
+    assert np.allclose(o2.density_2d(1), n.sum(axis=1) * 0.5, rtol=1e-13, atol=0)
+    assert np.allclose(o2.density_2d(0), n.sum(axis=2) * 0.3, rtol=1e-13, atol=0)
+    # 2-D problem: 1-D densities only, weights dx / dy alone
+    w2 = Workload("t", 2, 32, 16, 1, 0.2, 0.35, 1.0, 0.01, 1, 1, 0, 0, 0, 0, 0, REAL, 1, 1, 1)
+    p2 = random_psi(w2, 5)
+    o3 = ob.Oracle(ob.params_of(w2))
+    o3.set_psi(p2)
+    assert np.allclose(o3.density_1d(0), (np.abs(p2) ** 2).sum(axis=0) * 0.35, rtol=1e-13, atol=0)
+    assert np.allclose(o3.density_1d(1), (np.abs(p2) ** 2).sum(axis=1) * 0.2, rtol=1e-13, atol=0)
+    with pytest.raises(RuntimeError):
+        o3.density_1d(2)
+    with pytest.raises(RuntimeError):
+        o3.density_2d(2)
