@@ -86,17 +86,49 @@ int dbec_set_psi(dbec_handle h, const void* psi_c128, int on_device);
 /* Copy psi out (same pointer rules), with the deferred imaginary-time norm factor applied. */
 int dbec_get_psi(dbec_handle h, void* psi_c128, int on_device);
 
-/* Change G and D (quench / ramp, reading S18).  Takes effect from the next step. */
+/* Change G and D (quench, reading S18).  Takes effect from the next step; ends a running ramp.  On a batch
+ * handle every member gets the same pair. */
 int dbec_set_coupling(dbec_handle h, double G, double D);
+
+/* NSTP ramp of the nonlinearity ("NSTP"; reading S26): the k-th dbec_step after this
+ * call (k = 1..nstp) runs with G0 + (G1 - G0) k/nstp and D0 + (D1 - D0) k/nstp, every later one with (G1, D1).
+ * nstp = 0: (G1, D1) at once — the paper's NSTP = 0 restart is then dbec_set_psi of a stored state, e.g. the
+ * device buffer dbec_get_psi filled from an imaginary-time handle.  The schedule lives in device memory, so the
+ * CUDA graph of a step sees it; dbec_observables / dbec_phi_dd do not advance it. */
+int dbec_set_ramp(dbec_handle h, int nstp, double G0, double D0, double G1, double D1);
 
 /* nsteps SSCN steps, asynchronous on the handle's stream, no host sync. */
 int dbec_step(dbec_handle h, int nsteps);
 
 /* calcmuen + calcrms on the current psi.  host_out: HOST pointer.  Synchronises
- * the stream. */
+ * the stream.  In 2-D rms_x / rms_y are those of the two grid axes, rms_z = 0. */
 int dbec_observables(dbec_handle h, dbec_obs* host_out);
 
 int dbec_destroy(dbec_handle h);
+
+/* ---- batched handles: nbatch independent simulations with the same parameters advance in the
+ * same kernel launches — the only way grids as small as 32^3 or 512^2, whose single step is bound by launch
+ * latency ("launching of all required kernels would create a sizeable overhead"), fill the GPU.
+ * Every field is member-major: dbec_set_psi / dbec_get_psi move nbatch * NX*NY*NZ values; dbec_step,
+ * dbec_set_ramp, dbec_set_coupling, dbec_normalize, dbec_cn_sweep, dbec_nonlinear, dbec_phi_dd act on all
+ * members.  1 <= nbatch <= 65536.  dbec_create == dbec_create_batch with nbatch = 1. ---- */
+int dbec_workspace_bytes_batch(const dbec_params* p, int nbatch, size_t* bytes);
+int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, size_t bytes, void* cuda_stream,
+                      dbec_handle* out);
+int dbec_batch_size(dbec_handle h, int* nbatch);
+/* Per-member couplings (parameter scans): G, D HOST arrays of nbatch values. */
+int dbec_set_coupling_batch(dbec_handle h, const double* G, const double* D);
+/* host_out: HOST array of nbatch records.  dbec_observables itself returns DBEC_EINVAL on a handle with
+ * more than one member. */
+int dbec_observables_batch(dbec_handle h, dbec_obs* host_out);
+
+/* ---- integrated densities (reading S27; the lineage's density output): |psi|^2 of batch member
+ * `member` summed over the other axes times their spacings.  out: HOST (synchronises) or DEVICE pointer. ----
+ * 1-D along `axis` (0 x, 1 y, 2 z; < ndim): N_axis doubles. */
+int dbec_density_1d(dbec_handle h, int member, int axis, double* out, int on_device);
+/* 2-D, 3-D grids only, integrated over `axis_integrated`: the two remaining axes, the lower one fastest
+ * (2: [NY][NX], 1: [NZ][NX], 0: [NZ][NY]). */
+int dbec_density_2d(dbec_handle h, int member, int axis_integrated, double* out, int on_device);
 
 const char* dbec_strerror(int code);
 /* CUDA error code behind this handle's last DBEC_ECUDA (0 if none).  h == NULL: the CUDA error behind the

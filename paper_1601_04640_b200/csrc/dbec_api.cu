@@ -10,8 +10,8 @@
 #include "cn_chunk.cuh"
 #include "host_tables.hpp"
 
-#define DBEC_VERSION 100
-#define NPARTIAL 32768
+#define DBEC_VERSION 200
+#define DBEC_MAX_BATCH 65536
 
 static bool fft_len_ok(int n) { return n == 16 || n == 32 || n == 64 || n == 128 || n == 256 || n == 512; }
 
@@ -49,19 +49,28 @@ static size_t axis_table_bytes(int n) {
     return b;
 }
 
-static void make_layout(const dbec_params* p, Layout* L) {
-    const size_t nx = p->nx, ny = p->ny, nz = p->nz;
+// Reduction partials: one per block of the last Crank-Nicolson sweep (<= one per 256 points), ten per block
+// of the observables pass.
+static size_t npartial_of(size_t P, size_t nb) {
+    size_t n = 32768, a = nb * P / 256 + nb, b = nb * 10 * 8;
+    if (a > n) n = a;
+    if (b > n) n = b;
+    return n;
+}
+
+static void make_layout(const dbec_params* p, int nbatch, Layout* L) {
+    const size_t nx = p->nx, ny = p->ny, nz = p->nz, nb = nbatch;
     const size_t nxhp = ((nx / 2 + 1) + DBEC_SPEC_COLS - 1) / DBEC_SPEC_COLS * DBEC_SPEC_COLS;
     const size_t P = nx * ny * nz, SP = nz * ny * nxhp;
     size_t o = 0;
-    L->psi = o;     o += up256(P * sizeof(cd));
-    L->spec = o;    o += up256(SP * sizeof(cd));
+    L->psi = o;     o += up256(nb * P * sizeof(cd));
+    L->spec = o;    o += up256(nb * SP * sizeof(cd));
     L->vdd = o;     o += up256(SP * sizeof(double));
-    L->phi = o;     o += up256(P * sizeof(double));
-    L->scal = o;    o += up256(SC_COUNT * sizeof(double));
-    L->partial = o; o += up256(NPARTIAL * sizeof(double));
+    L->phi = o;     o += up256(nb * P * sizeof(double));
+    L->scal = o;    o += up256(nb * SC_COUNT * sizeof(double));
+    L->partial = o; o += up256(npartial_of(P, nb) * sizeof(double));
     L->ticket = o;  o += 256;
-    L->obs = o;     o += 256;
+    L->obs = o;     o += up256(nb * 16 * sizeof(double));
     L->tables = o;
     L->tab_bytes = axis_table_bytes(p->nx) + axis_table_bytes(p->ny) + axis_table_bytes(p->nz);
     o += L->tab_bytes;
@@ -130,16 +139,22 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     return DBEC_OK;
 }
 
-static int write_scalars(dbec_handle h, bool reset_scale) {
-    double v[SC_COUNT] = {0};
-    if (!reset_scale) {
-        CU(h, cudaMemcpyAsync(v, h->scal, sizeof(v), cudaMemcpyDeviceToHost, h->stream));
-        CU(h, cudaStreamSynchronize(h->stream));
-    } else {
-        v[SC_S] = 1.0; v[SC_S2] = 1.0;
+// Every member's scalar block at create time: s = 1, G and D of the parameters, no ramp.
+static int init_scalars(dbec_handle h) {
+    std::vector<double> v((size_t)h->nb * SC_COUNT, 0.0);
+    for (int b = 0; b < h->nb; ++b) {
+        double* sc = v.data() + (size_t)b * SC_COUNT;
+        sc[SC_S] = 1.0; sc[SC_S2] = 1.0; sc[SC_G] = h->p.G; sc[SC_D] = h->p.D;
     }
-    v[SC_G] = h->p.G; v[SC_D] = h->p.D;
-    CU(h, cudaMemcpyAsync(h->scal, v, sizeof(v), cudaMemcpyHostToDevice, h->stream));
+    CU(h, cudaMemcpyAsync(h->scal, v.data(), v.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
+// Columns [first, first + count) of every member's scalar block <- vals[member][count] (HOST).
+static int write_member_scalars(dbec_handle h, int first, int count, const double* vals) {
+    CU(h, cudaMemcpy2DAsync(h->scal + first, SC_COUNT * sizeof(double), vals, count * sizeof(double), count * sizeof(double),
+                            h->nb, cudaMemcpyHostToDevice, h->stream));
     CU(h, cudaStreamSynchronize(h->stream));
     return DBEC_OK;
 }
@@ -165,19 +180,28 @@ static const char* const kernel_names[DBEC_MAX_KERNELS] = {
 // previous pass has just left (dirty) in the 126 MB L2.
 static int launch_fft_pass(dbec_handle h, int axis, int mode, int rev = 0) {
     h->rev_next = rev && h->use_rev;
-    return dbec_tma_supported(h, axis) ? dbec_launch_fft_tma(h, axis, mode, 0, h->nz) : dbec_launch_fft_strided(h, axis, mode);
+    return dbec_tma_supported(h, axis) ? dbec_launch_fft_tma(h, axis, mode, 0, h->nplanes) : dbec_launch_fft_strided(h, axis, mode);
 }
 static int launch_cn_pass(dbec_handle h, int axis, int with_norm, int rev = 0) {
     h->rev_next = rev && h->use_rev;
-    return (axis > 0 && dbec_tma_supported(h, axis)) ? dbec_launch_cn_tma(h, axis, with_norm, 0, h->nz)
-                                                     : dbec_launch_cn(h, axis, with_norm);
+    if (axis > 0 && dbec_tma_supported(h, axis)) {
+        // a batch: the tiles of one CTA of the persistent sweep span several members, so calcnorm takes a
+        // pass of its own (the fields of a batch are small: it runs out of L2)
+        if (with_norm && h->nb > 1) {
+            int rc = dbec_launch_cn_tma(h, axis, 0, 0, h->nplanes);
+            return rc ? rc : dbec_launch_norm_only(h);
+        }
+        return dbec_launch_cn_tma(h, axis, with_norm, 0, h->nplanes);
+    }
+    return dbec_launch_cn(h, axis, with_norm);
 }
 
 // calcpsidd2 up to the x-inverse: density -> half spectrum -> x V_dd -> back along z, y.
-static int enqueue_dipolar_spectrum(dbec_handle h) {
+// advance: 1 inside a step (the density pass also moves the NSTP ramp on, reading S26).
+static int enqueue_dipolar_spectrum(dbec_handle h, int advance) {
     h->rev_next = 0;
-    if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nz));
-    else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h));
+    if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nplanes, advance));
+    else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h, advance));
     if (h->p.ndim == 3) {
         KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
         KLAUNCH(h, KS_FFT_LAST_FMI, launch_fft_pass(h, 2, 2));
@@ -192,10 +216,10 @@ static int enqueue_dipolar_spectrum(dbec_handle h) {
 static int enqueue_step(dbec_handle h) {
     const bool imag = h->p.time_mode == 0;
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
-    int rc = enqueue_dipolar_spectrum(h);
+    int rc = enqueue_dipolar_spectrum(h, 1);
     if (rc) return rc;
     h->rev_next = h->use_rev;                                       // inverse y pass went up: come back down
-    if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nz));
+    if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nplanes));
     else KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
     if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, launch_cn_pass(h, 0, 0));
     for (int ax = 1; ax <= last_axis; ++ax)
@@ -219,23 +243,31 @@ const char* dbec_strerror(int code) {
     }
 }
 
-int dbec_workspace_bytes(const dbec_params* p, size_t* bytes) {
-    if (!bytes) return DBEC_EINVAL;
+int dbec_workspace_bytes_batch(const dbec_params* p, int nbatch, size_t* bytes) {
+    if (!bytes || nbatch < 1 || nbatch > DBEC_MAX_BATCH) return DBEC_EINVAL;
     int rc = check_params(p);
     if (rc) return rc;
     Layout L;
-    make_layout(p, &L);
+    make_layout(p, nbatch, &L);
     *bytes = L.total;
     return DBEC_OK;
 }
 
+int dbec_workspace_bytes(const dbec_params* p, size_t* bytes) { return dbec_workspace_bytes_batch(p, 1, bytes); }
+
 int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* cuda_stream, dbec_handle* out) {
+    return dbec_create_batch(p, 1, dev_workspace, bytes, cuda_stream, out);
+}
+
+int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, size_t bytes, void* cuda_stream,
+                      dbec_handle* out) {
     if (!out) return DBEC_EINVAL;
     *out = nullptr;
+    if (nbatch < 1 || nbatch > DBEC_MAX_BATCH) return DBEC_EINVAL;
     int rc = check_params(p);
     if (rc) return rc;
     Layout L;
-    make_layout(p, &L);
+    make_layout(p, nbatch, &L);
     if (!dev_workspace || ((uintptr_t)dev_workspace & 255) || bytes < L.total) return DBEC_EWORKSPACE;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return DBEC_ENODEVICE;
@@ -254,6 +286,8 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->P = (long long)p->nx * p->ny * p->nz;
     h->SP = (long long)p->nz * p->ny * h->nxhp;
     h->dV = p->ndim == 3 ? p->dx * p->dy * p->dz : p->dx * p->dy;
+    h->nb = nbatch;
+    h->nplanes = p->nz * nbatch;
     char* w = (char*)dev_workspace;
     h->psi = (cd*)(w + L.psi);
     h->spec = (cd*)(w + L.spec);
@@ -263,7 +297,7 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
     h->partial = (double*)(w + L.partial);
     h->ticket = (unsigned int*)(w + L.ticket);
     h->obs_dev = (double*)(w + L.obs);
-    h->npartial = NPARTIAL;
+    h->npartial = (int)npartial_of((size_t)h->P, (size_t)nbatch);
     // the only two switches (both exercised by tests/test_gpu_parity.py): the CUDA graph of a step and the
     // x sweep fused into the nonlinear kernel
     const char* fe = getenv("DBEC_FUSE_CNX");
@@ -284,9 +318,9 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
 #define FAIL(code) do { create_cuda_error = h->last_cuda ? h->last_cuda : (int)cudaGetLastError(); delete h; return (code); } while (0)
 #define TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { h->last_cuda = (int)e_; FAIL(DBEC_ECUDA); } } while (0)
     create_cuda_error = 0;
-    TRY(cudaMemsetAsync(h->psi, 0, sizeof(cd) * h->P, h->stream));
+    TRY(cudaMemsetAsync(h->psi, 0, sizeof(cd) * h->P * h->nb, h->stream));
     TRY(cudaMemsetAsync(h->ticket, 0, 256, h->stream));
-    TRY(cudaMemsetAsync(h->spec, 0, sizeof(cd) * h->SP, h->stream));
+    TRY(cudaMemsetAsync(h->spec, 0, sizeof(cd) * h->SP * h->nb, h->stream));
     char* t = w + L.tables;
     const double om[3] = {p->nu, p->lambda, p->kappa};
     const double dd[3] = {p->dx, p->dy, p->ndim == 3 ? p->dz : 1.0};
@@ -298,7 +332,7 @@ int dbec_create(const dbec_params* p, void* dev_workspace, size_t bytes, void* c
         t += used;
     }
     if (h->use_tma) TRY((cudaError_t)dbec_make_tensor_maps(h));
-    if (write_scalars(h, true)) FAIL(DBEC_ECUDA);
+    if (init_scalars(h)) FAIL(DBEC_ECUDA);
     TRY((cudaError_t)dbec_launch_build_vdd(h));
     TRY(cudaStreamSynchronize(h->stream));
 #undef TRY
@@ -326,11 +360,10 @@ const char* dbec_build_id(void) {
 
 int dbec_set_psi(dbec_handle h, const void* psi, int on_device) {
     if (!h || !psi) return DBEC_EINVAL;
-    CU(h, cudaMemcpyAsync(h->psi, psi, sizeof(cd) * h->P, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+    CU(h, cudaMemcpyAsync(h->psi, psi, sizeof(cd) * h->P * h->nb, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
                           h->stream));
     // a fresh field carries no deferred norm factor
-    double one[2] = {1.0, 1.0};
-    CU(h, cudaMemcpyAsync(h->scal + SC_S, one, sizeof(one), cudaMemcpyHostToDevice, h->stream));
+    LAUNCH(h, dbec_launch_reset_scale(h));
     if (!on_device) CU(h, cudaStreamSynchronize(h->stream));
     return DBEC_OK;
 }
@@ -338,18 +371,48 @@ int dbec_set_psi(dbec_handle h, const void* psi, int on_device) {
 int dbec_get_psi(dbec_handle h, void* psi, int on_device) {
     if (!h || !psi) return DBEC_EINVAL;
     if (h->p.time_mode == 0) LAUNCH(h, dbec_launch_apply_scale(h));     // s is 1 for ever in real time
-    CU(h, cudaMemcpyAsync(psi, h->psi, sizeof(cd) * h->P, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+    CU(h, cudaMemcpyAsync(psi, h->psi, sizeof(cd) * h->P * h->nb, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
                           h->stream));
     if (!on_device) CU(h, cudaStreamSynchronize(h->stream));
     return DBEC_OK;
 }
 
+// Columns SC_G .. SC_RN of every member: the current (G, D), then a ramp G0, D0, G1, D1, k = 0, n.
+static int write_couplings(dbec_handle h, const double* G, int gs, const double* D, int ds, int nstp, const double* G0,
+                           const double* D0) {
+    const int cols = SC_RN - SC_G + 1;
+    std::vector<double> v((size_t)h->nb * cols);
+    for (int b = 0; b < h->nb; ++b) {
+        double* r = v.data() + (size_t)b * cols;
+        const double g1 = G[b * gs], d1 = D[b * ds];
+        const double g0 = nstp > 0 ? G0[0] : g1, d0 = nstp > 0 ? D0[0] : d1;
+        r[SC_G - SC_G] = g0; r[SC_D - SC_G] = d0;
+        r[SC_G0 - SC_G] = g0; r[SC_D0 - SC_G] = d0; r[SC_G1 - SC_G] = g1; r[SC_D1 - SC_G] = d1;
+        r[SC_RK - SC_G] = 0.0; r[SC_RN - SC_G] = (double)nstp;
+    }
+    return write_member_scalars(h, SC_G, cols, v.data());
+}
+
 int dbec_set_coupling(dbec_handle h, double G, double D) {
     if (!h) return DBEC_EINVAL;
     h->p.G = G; h->p.D = D;
-    double v[2] = {G, D};
-    CU(h, cudaMemcpyAsync(h->scal + SC_G, v, sizeof(v), cudaMemcpyHostToDevice, h->stream));
-    CU(h, cudaStreamSynchronize(h->stream));
+    return write_couplings(h, &G, 0, &D, 0, 0, nullptr, nullptr);
+}
+
+int dbec_set_coupling_batch(dbec_handle h, const double* G, const double* D) {
+    if (!h || !G || !D) return DBEC_EINVAL;
+    return write_couplings(h, G, 1, D, 1, 0, nullptr, nullptr);
+}
+
+int dbec_set_ramp(dbec_handle h, int nstp, double G0, double D0, double G1, double D1) {
+    if (!h || nstp < 0) return DBEC_EINVAL;
+    h->p.G = G1; h->p.D = D1;
+    return write_couplings(h, &G1, 0, &D1, 0, nstp, &G0, &D0);
+}
+
+int dbec_batch_size(dbec_handle h, int* nbatch) {
+    if (!h || !nbatch) return DBEC_EINVAL;
+    *nbatch = h->nb;
     return DBEC_OK;
 }
 
@@ -384,7 +447,7 @@ int dbec_step(dbec_handle h, int nsteps) {
 
 int dbec_phi_dd(dbec_handle h, void* phi_f64_dev) {
     if (!h || !phi_f64_dev) return DBEC_EINVAL;
-    { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
+    { int rc = enqueue_dipolar_spectrum(h, 0); if (rc) return rc; }
     LAUNCH(h, dbec_launch_phi_out(h, (double*)phi_f64_dev));
     return DBEC_OK;
 }
@@ -400,7 +463,7 @@ int dbec_nonlinear(dbec_handle h) {
     // the nonlinear kernel multiplies by the deferred norm factor s but leaves it in place (inside a step the
     // last sweep rewrites it): bring the stored field to s = 1 first, or every later consumer applies s again
     LAUNCH(h, dbec_launch_apply_scale(h));
-    { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
+    { int rc = enqueue_dipolar_spectrum(h, 0); if (rc) return rc; }
     LAUNCH(h, dbec_launch_nonlinear(h, 0));
     return DBEC_OK;
 }
@@ -414,18 +477,52 @@ int dbec_normalize(dbec_handle h) {
     return DBEC_OK;
 }
 
-int dbec_observables(dbec_handle h, dbec_obs* out) {
+int dbec_observables_batch(dbec_handle h, dbec_obs* out) {
     if (!h || !out) return DBEC_EINVAL;
-    { int rc = enqueue_dipolar_spectrum(h); if (rc) return rc; }
+    { int rc = enqueue_dipolar_spectrum(h, 0); if (rc) return rc; }
     LAUNCH(h, dbec_launch_phi_out(h, h->phi));
     LAUNCH(h, dbec_launch_observables(h));
-    double v[16];
-    CU(h, cudaMemcpyAsync(v, h->obs_dev, sizeof(double) * 9, cudaMemcpyDeviceToHost, h->stream));
+    std::vector<double> v((size_t)h->nb * 16);
+    CU(h, cudaMemcpyAsync(v.data(), h->obs_dev, v.size() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CU(h, cudaStreamSynchronize(h->stream));
-    out->norm = v[0]; out->mu = v[1]; out->energy = v[2];
-    out->rms_x = v[3]; out->rms_y = v[4]; out->rms_z = v[5]; out->rms_r = v[6];
-    out->density0 = v[7]; out->density_max = v[8];
+    for (int b = 0; b < h->nb; ++b) {
+        const double* r = v.data() + (size_t)b * 16;
+        dbec_obs& o = out[b];
+        o.norm = r[0]; o.mu = r[1]; o.energy = r[2];
+        o.rms_x = r[3]; o.rms_y = r[4]; o.rms_z = r[5]; o.rms_r = r[6];
+        o.density0 = r[7]; o.density_max = r[8];
+    }
     return DBEC_OK;
+}
+
+int dbec_observables(dbec_handle h, dbec_obs* out) {
+    if (!h || !out || h->nb != 1) return DBEC_EINVAL;      // a batch has one record per member: dbec_observables_batch
+    return dbec_observables_batch(h, out);
+}
+
+// Integrated densities (reading S27).  The result is produced on the device; out may be HOST or DEVICE.
+static int density_out(dbec_handle h, const double* dev, size_t count, void* out, int on_device) {
+    CU(h, cudaMemcpyAsync(out, dev, count * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    if (!on_device) CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
+int dbec_density_1d(dbec_handle h, int member, int axis, double* out, int on_device) {
+    if (!h || !out || member < 0 || member >= h->nb || axis < 0 || axis >= h->p.ndim) return DBEC_EINVAL;
+    // h->phi (P doubles per member, scratch outside dbec_observables) holds the intermediate 2-D density and the result
+    const int n[3] = {h->nx, h->ny, h->nz};
+    double* scratch = h->phi;
+    double* res = h->phi + (h->P - n[axis]);              // the tail of the first member's block: never overlaps a 2-D density
+    LAUNCH(h, dbec_launch_density_1d(h, member, axis, res, scratch));
+    return density_out(h, res, (size_t)n[axis], out, on_device);
+}
+
+int dbec_density_2d(dbec_handle h, int member, int axis_integrated, double* out, int on_device) {
+    if (!h || !out || member < 0 || member >= h->nb || h->p.ndim != 3 || axis_integrated < 0 || axis_integrated > 2)
+        return DBEC_EINVAL;
+    const size_t count = (size_t)h->P / (size_t)(axis_integrated == 0 ? h->nx : axis_integrated == 1 ? h->ny : h->nz);
+    LAUNCH(h, dbec_launch_density_2d(h, member, axis_integrated, h->phi));
+    return density_out(h, h->phi, count, out, on_device);
 }
 
 // nsteps steps with plain launches and a CUDA event pair around every kernel.  ms_per_slot receives

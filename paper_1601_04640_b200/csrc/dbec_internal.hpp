@@ -19,12 +19,30 @@ enum { POL_CN_LD = 0, POL_CN_ST, POL_NL_LD, POL_NL_ST, POL_NL_SPEC, POL_D_PSI, P
 // Tensor maps of the handle (kernels_tma.cu): field x direction of the box rows.
 enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD_Y, TM_VDD_Z, TM_COUNT };
 
-// Device scalars every kernel reads (so that a captured CUDA graph never bakes them in).
+// Device scalars every kernel reads (so that a captured CUDA graph never bakes them in), one block of
+// SC_COUNT doubles per batch member (dbec_create_batch; a plain handle has one member).
 //   [0] s      deferred norm factor: true psi = s * stored psi (calcnorm; 1 in real time)
 //   [1] s^2
-//   [2] G      coefficient of |psi|^2            (dbec_set_coupling)
+//   [2] G      coefficient of |psi|^2 used by the current step   (dbec_set_coupling / the ramp below)
 //   [3] D      coefficient of Phi_dd
-enum { SC_S = 0, SC_S2 = 1, SC_G = 2, SC_D = 3, SC_COUNT = 8 };
+//   [4..7]     G0, D0, G1, D1 of the NSTP ramp (dbec_set_ramp, reading S26)
+//   [8], [9]   ramp steps begun so far, ramp length (as doubles); no ramp: both 0
+enum { SC_S = 0, SC_S2 = 1, SC_G = 2, SC_D = 3, SC_G0 = 4, SC_D0 = 5, SC_G1 = 6, SC_D1 = 7, SC_RK = 8, SC_RN = 9, SC_COUNT = 16 };
+
+#if defined(__CUDACC__)
+// Reading S26 ("NSTP"): the k-th step after dbec_set_ramp (k = 1..n) runs with
+// G0 + (G1 - G0) k/n and D0 + (D1 - D0) k/n.  Called by ONE thread per member in the first kernel of a step
+// (the density pass, which reads neither G nor D); the nonlinear kernel later in the stream sees the result.
+__device__ __forceinline__ void ramp_advance(double* __restrict__ sc) {
+    const double k = sc[SC_RK], n = sc[SC_RN];
+    if (k < n) {
+        const double k1 = k + 1.0, f = k1 / n;
+        sc[SC_RK] = k1;
+        sc[SC_G] = sc[SC_G0] + (sc[SC_G1] - sc[SC_G0]) * f;
+        sc[SC_D] = sc[SC_D0] + (sc[SC_D1] - sc[SC_D0]) * f;
+    }
+}
+#endif
 
 // Per-axis tables on the device.
 struct AxisTables {
@@ -48,18 +66,22 @@ struct dbec_handle_s {
     long long launches;
     // geometry
     int nx, ny, nz, nxhp;           // nxhp = padded half-spectrum row length (multiple of DBEC_SPEC_COLS)
-    long long P;                    // nx*ny*nz
-    long long SP;                   // nz*ny*nxhp
+    long long P;                    // nx*ny*nz   (per batch member)
+    long long SP;                   // nz*ny*nxhp (per batch member)
     double dV;
+    // batch (dbec_create_batch): nb independent members with the same parameters; every field
+    // below holds the members back to back (member-major), the V_dd table and the axis tables are shared
+    int nb;
+    int nplanes;                    // nz * nb: xy planes in psi / spec (a batch of 2-D grids is a stack of planes)
     // device memory (all inside the caller's workspace)
     cd* psi;                        // [nz][ny][nx]
     cd* spec;                       // [nz][ny][nxhp] half spectrum of the density
     double* vdd;                    // [nz][ny][nxhp] V_dd(k)/P
     double* phi;                    // [nz][ny][nx] Phi_dd (observables / dbec_phi_dd only)
-    double* scal;                   // SC_COUNT doubles
+    double* scal;                   // nb x SC_COUNT doubles
     double* partial;                // reduction partials
     unsigned int* ticket;           // last-block tickets
-    double* obs_dev;                // 16 doubles
+    double* obs_dev;                // nb x 16 doubles
     AxisTables ax[3];
     int npartial;
     // CUDA graph of one step
@@ -82,15 +104,20 @@ struct dbec_handle_s {
 };
 
 // ---- launchers (each returns a cudaError_t as int; all asynchronous on h->stream) ----
-int dbec_launch_density_fftx(dbec_handle_s* h);            // a1, x axis: psi -> half spectrum
+// advance: 1 in a step (the density pass also moves the NSTP ramp on), 0 for observables / dbec_phi_dd
+int dbec_launch_density_fftx(dbec_handle_s* h, int advance);   // a1, x axis: psi -> half spectrum
 int dbec_launch_fft_strided(dbec_handle_s* h, int axis, int mode);   // a1/a3 along y or z; mode 0 forward, 1 inverse,
                                                            // 2 forward * V_dd(k)/P * inverse (a2 fused)
 int dbec_launch_nonlinear(dbec_handle_s* h, int fuse_cnx); // a3 (x, C2R) + a4 [+ a5]
-int dbec_launch_phi_out(dbec_handle_s* h, double* phi);    // a3 writing Phi_dd only
+int dbec_launch_phi_out(dbec_handle_s* h, double* phi);    // a3 writing Phi_dd only (all members)
 int dbec_launch_cn(dbec_handle_s* h, int axis, int with_norm);   // a5..a7 (+ a8 partial sums and factor)
-int dbec_launch_normalize(dbec_handle_s* h);               // a8 alone
+int dbec_launch_normalize(dbec_handle_s* h);               // a8 alone (applies any deferred factor first)
+int dbec_launch_norm_only(dbec_handle_s* h);               // a8 on a stored field with s = 1 (batched persistent sweeps)
 int dbec_launch_apply_scale(dbec_handle_s* h);             // psi <- s psi, s <- 1
-int dbec_launch_observables(dbec_handle_s* h);             // a9 (expects h->phi filled)
+int dbec_launch_reset_scale(dbec_handle_s* h);             // s <- 1
+int dbec_launch_observables(dbec_handle_s* h);             // a9 (expects h->phi filled), every member
+int dbec_launch_density_2d(dbec_handle_s* h, int member, int axis, double* out);   // reading S27 (3-D grids)
+int dbec_launch_density_1d(dbec_handle_s* h, int member, int axis, double* out, double* scratch);
 int dbec_launch_build_vdd(dbec_handle_s* h);               // potdd table
 // persistent TMA-fed versions of the strided passes (kernels_tma.cu); z0, nzs: slab of planes (y passes)
 int dbec_make_tensor_maps(dbec_handle_s* h);
@@ -100,4 +127,4 @@ int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nz
 // persistent bulk-copy-fed versions of the x passes (kernels_xline.cu)
 int dbec_xline_supported(const dbec_handle_s* h);
 int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs);          // a3 (x) + a4 + a5
-int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs);         // a1 (x)
+int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance);   // a1 (x)

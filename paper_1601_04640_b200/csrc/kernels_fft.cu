@@ -30,7 +30,8 @@ template <class P> struct XLine {
 template <class P, int LP>
 __global__ void __launch_bounds__(P::T* LP)
 k_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA,
-               const cd* __restrict__ twN, const double* __restrict__ scal, int npairs, int nxhp) {
+               const cd* __restrict__ twN, double* __restrict__ scal, int npairs, int nxhp, int pairs_per_member,
+               int nb, int advance) {
     extern __shared__ cd smem[];
     pdl_launch_dependents(); pdl_wait();       // (tma_pipe.cuh) launch latency overlaps the previous kernel
     constexpr int T = P::T, N = P::N;
@@ -38,7 +39,9 @@ k_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __re
     const long long pair = (long long)blockIdx.x * LP + lp;
     const bool active = pair < npairs;
     cd* sm = smem + lp * XLine<P>::SMF;
-    const double s2 = scal[SC_S2];
+    const double s2 = scal[(active ? pair / pairs_per_member : 0) * SC_COUNT + SC_S2];
+    if (advance && blockIdx.x == 0)            // first kernel of a step: move the NSTP ramp on (reads neither G nor D)
+        for (int b = threadIdx.x; b < nb; b += blockDim.x) ramp_advance(scal + (size_t)b * SC_COUNT);
     const cd* pa = psi + (active ? pair : 0) * 2 * N;
     const cd* pb = pa + N;
     cd v[16];
@@ -81,7 +84,7 @@ template <class P, int MODE, int TILES>
 __global__ void __launch_bounds__(P::T* DBEC_SPEC_COLS* TILES)
 k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twA,
               const cd* __restrict__ twN, long long line_stride, long long outer_stride, int ntiles_x,
-              long long ntiles) {
+              long long ntiles, int vdd_outer_mod) {
     extern __shared__ cd smem[];
     pdl_launch_dependents(); pdl_wait();
     constexpr int T = P::T, C = DBEC_SPEC_COLS;
@@ -99,7 +102,8 @@ k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* _
     for (int j = 0; j < 16; ++j) v[j] = g[(long long)(j * T + m) * line_stride];
     if (MODE == MODE_FWD || MODE == MODE_FMI) fft_line<P, -1, 1>(v, m, sm, C, twA, twN);
     if (MODE == MODE_FMI) {
-        const double* w = vdd + base;
+        // the V_dd table is shared by the members of a batch: its outer coordinate wraps
+        const double* w = vdd + (outer % vdd_outer_mod) * outer_stride + tx * C + col;
 #pragma unroll
         for (int j = 0; j < 16; ++j) v[j] = cmul(w[(long long)(j * T + m) * line_stride], v[j]);
         if (T > 1) __syncthreads();
@@ -124,7 +128,7 @@ __global__ void __launch_bounds__(P::T* LP, NL_MINB)
 k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out,
                const cd* __restrict__ twA, const cd* __restrict__ twN, const double* __restrict__ scal,
                const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
-               double dt, int npairs, int nxhp, int ny, CnTab<RT> cn) {
+               double dt, int npairs, int nxhp, int ny, int nz, CnTab<RT> cn) {
     extern __shared__ cd smem[];
     pdl_launch_dependents(); pdl_wait();
     typedef typename CnCoef<RT>::type CT;
@@ -165,9 +169,10 @@ k_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __rest
         }
         return;
     }
-    const double s = scal[SC_S], s2 = scal[SC_S2], G = scal[SC_G], D = scal[SC_D];
     const long long row = pair * 2;
-    const int y = (int)(row % ny), z = (int)(row / ny);
+    const int y = (int)(row % ny), zz = (int)(row / ny), z = zz % nz;
+    const double* sc = scal + (size_t)(zz / nz) * SC_COUNT;          // this row's batch member
+    const double s = sc[SC_S], s2 = sc[SC_S2], G = sc[SC_G], D = sc[SC_D];
     const double vzz = vz[z];
     if (MODE == NL_STEP_CNX) __syncwarp();               // FFT exchange rows are reused by the sweep
 #pragma unroll
@@ -278,18 +283,16 @@ template <> struct PlanOf<512> { typedef FftPlan<16, 2, true> X; typedef FftPlan
 static const int XTHREADS = 256;   // threads per block of k_density_fftx
 static const int NLTHREADS = 128;  // threads per block of k_ifftx_nonlin
 
-template <int N> static int launch_density_fftx(dbec_handle_s* h) {
+template <int N> static int launch_density_fftx(dbec_handle_s* h, int advance) {
     typedef typename PlanOf<N>::X P;
     constexpr int LP = XTHREADS / P::T;
-    const int npairs = h->ny * h->nz / 2;
-    const int lp = npairs < LP ? npairs : LP;   // tiny grids: fewer pairs than a block holds
-    (void)lp;
+    const int ppm = h->ny * h->nz / 2, npairs = ppm * h->nb;
     const size_t sm = (size_t)LP * XLine<P>::SMF * sizeof(cd);
     auto k = k_density_fftx<P, LP>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
     cudaError_t e = launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(P::T * LP), sm, h->stream, h->use_pdl, h->psi, h->spec,
-                               h->ax[0].twA, h->ax[0].twN, h->scal, npairs, h->nxhp);
+                               h->ax[0].twA, h->ax[0].twN, h->scal, npairs, h->nxhp, ppm, h->nb, advance);
     h->launches++;
     return (int)e;
 }
@@ -299,20 +302,20 @@ template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int a
     constexpr int C = DBEC_SPEC_COLS;
     constexpr int TILES = (P::T * C >= 128) ? 1 : 128 / (P::T * C);
     long long line_stride, outer_stride, ntiles;
-    int ntx;
-    if (axis == 1) {        // y lines: for each z, columns = kx
+    int ntx, vmod;
+    if (axis == 1) {        // y lines: for each plane (z, member), columns = kx
         line_stride = h->nxhp; outer_stride = (long long)h->ny * h->nxhp; ntx = h->nxhp / C;
-        ntiles = (long long)ntx * h->nz;
-    } else {                // z lines: columns = (ky, kx) flattened
-        line_stride = (long long)h->ny * h->nxhp; outer_stride = 0; ntx = (int)(line_stride / C);
-        ntiles = ntx;
+        ntiles = (long long)ntx * h->nplanes; vmod = h->nz;
+    } else {                // z lines: columns = (ky, kx) flattened; outer = batch member
+        line_stride = (long long)h->ny * h->nxhp; outer_stride = h->SP; ntx = (int)(line_stride / C);
+        ntiles = (long long)ntx * h->nb; vmod = 1;
     }
     const size_t sm = (size_t)TILES * P::SMEM * C * sizeof(cd);
     auto k = k_fft_strided<P, MODE, TILES>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
     cudaError_t e = launch_pdl(k, dim3((unsigned)((ntiles + TILES - 1) / TILES)), dim3(P::T * C * TILES), sm, h->stream, h->use_pdl,
-                               h->spec, (const double*)h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles);
+                               h->spec, (const double*)h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles, vmod);
     h->launches++;
     return (int)e;
 }
@@ -320,7 +323,7 @@ template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int a
 template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, double* phi) {
     typedef typename PlanOf<N>::X P;
     constexpr int LP = NLTHREADS / P::T;
-    const int npairs = h->ny * h->nz / 2;
+    const int npairs = h->ny * h->nz / 2 * h->nb;
     const size_t sm = (size_t)LP * XLine<P>::SM * sizeof(cd) +
                       (MODE == NL_STEP_CNX ? 3 * cn_tab_elems(N) * sizeof(typename CnCoef<RT>::type) : 0);
     auto k = k_ifftx_nonlin<P, LP, RT, MODE>;
@@ -328,14 +331,14 @@ template <int N, bool RT, int MODE> static int launch_ifftx(dbec_handle_s* h, do
     if (rc) return rc;
     cudaError_t e = launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(P::T * LP), sm, h->stream, h->use_pdl,
                                (const cd*)h->spec, h->psi, phi, h->ax[0].twA, h->ax[0].twN, (const double*)h->scal, h->ax[0].vtrap,
-                               h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, npairs, h->nxhp, h->ny, make_cntab<RT>(h->ax[0]));
+                               h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, npairs, h->nxhp, h->ny, h->nz, make_cntab<RT>(h->ax[0]));
     h->launches++;
     return (int)e;
 }
 
-int dbec_launch_density_fftx(dbec_handle_s* h) {
+int dbec_launch_density_fftx(dbec_handle_s* h, int advance) {
     int rc;
-    DISPATCH_N(h->nx, rc = launch_density_fftx<N_>(h));
+    DISPATCH_N(h->nx, rc = launch_density_fftx<N_>(h, advance));
     return rc;
 }
 

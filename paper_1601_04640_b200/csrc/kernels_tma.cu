@@ -26,6 +26,8 @@ struct TileGeom {
     int box_rows;    // rows of one TMA box (<= 256)
     int nbox;        // boxes per tile (N / box_rows)
     int outer0;      // first outer coordinate (slab offset; axis 1 only)
+    int vmod;        // planes of the V_dd table (nz): the outer coordinate of its tile wraps, because a batch of
+                     // 2-D grids is a stack of planes that share one table
     int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
     float pol_ld, pol_st;   // L2 eviction policy codes of the tile loads / stores (tma_pipe.cuh: l2_policy_code)
 };
@@ -75,6 +77,7 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
             tma_load_3d_hint(dst + (size_t)b * (MAIN_BYTES / tg.nbox), map, c0, c1, c2, pb.full + s, pol);
             if (EXTRA_BYTES) {
                 tile_coords(tg, t, b, TCOLS, c0, c1, c2);
+                if (tg.axis == 1) c2 %= tg.vmod;
                 tma_load_3d_hint(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.nbox), extra, c0, c1, c2, pb.full + s,
                                  l2_policy_evict_first());      // the V_dd table is read once per step
             }
@@ -323,10 +326,13 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
     static_assert(sizeof(CUtensorMap) == DBEC_TMAP_BYTES, "tensor map size");
     const int by = box_rows_of(h->ny), bz = box_rows_of(h->nz);
     int rc = 0;
-    rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Y], h->psi, 2LL * h->nx, h->ny, h->nz, 2 * TCOLS, by, 1);
-    rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Z], h->psi, 2LL * h->nx, h->ny, h->nz, 2 * TCOLS, 1, bz);
-    rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Y], h->spec, 2LL * h->nxhp, h->ny, h->nz, 2 * TCOLS, by, 1);
-    rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Z], h->spec, 2LL * h->nxhp, h->ny, h->nz, 2 * TCOLS, 1, bz);
+    // psi and the spectrum hold nplanes = nz * nb planes (a batch of 2-D grids is a stack of planes; the
+    // persistent strided kernels do not serve batches of 3-D grids, see dbec_tma_supported)
+    const int np = h->nplanes;
+    rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Y], h->psi, 2LL * h->nx, h->ny, np, 2 * TCOLS, by, 1);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Z], h->psi, 2LL * h->nx, h->ny, np, 2 * TCOLS, 1, bz);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Y], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, by, 1);
+    rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Z], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, 1, bz);
     rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Y], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, by, 1);
     rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Z], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, 1, bz);
     return rc ? (int)cudaErrorInvalidValue : 0;
@@ -342,6 +348,7 @@ static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int n
     tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
     tg.pol_st = h->pol[sp ? POL_FFT_ST : POL_CN_ST];
     tg.axis = axis;
+    tg.vmod = h->nz;
     tg.ntiles_x = row_elems / TCOLS;
     const int n = axis == 1 ? h->ny : h->nz;
     tg.box_rows = box_rows_of(n);
@@ -357,7 +364,7 @@ template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma
     constexpr int GT = NCH * TCOLS, STAGE = NCH * CN_L * TCOLS * (int)sizeof(cd);
     const TileGeom tg = geom_of(h, axis, false, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
-    if (NORM && grid > h->npartial) return (int)cudaErrorInvalidValue;
+    if (NORM && (grid > h->npartial || h->nb > 1)) return (int)cudaErrorInvalidValue;   // a CTA's tiles span members
     const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 4) * sizeof(uint64_t) +
                       (3 * cn_tab_elems(NCH * CN_L) + 2 * NCH) * sizeof(typename CnCoef<RT>::type);
     auto k = k_cn_tma<RT, NCH, NG, NST, NORM>;
@@ -380,6 +387,9 @@ template <bool RT, bool NORM> static int launch_cn_tma_n(dbec_handle_s* h, int a
 
 int dbec_tma_supported(const dbec_handle_s* h, int axis) {
     const int n = h->ax[axis].n;
+    // batches: 2-D grids only (their planes stack along the tensor maps' outer coordinate); a batch of 3-D
+    // grids runs its strided passes in the one-tile-per-block kernels
+    if (h->nb > 1 && h->p.ndim == 3) return 0;
     return h->use_tma && (n == 128 || n == 256 || n == 512);
 }
 

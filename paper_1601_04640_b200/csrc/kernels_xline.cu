@@ -40,8 +40,8 @@ template <class P, int XP, bool RT, int NG, int NST>
 __global__ void __launch_bounds__(NG * 2 * XP * P::T + 96, 1)
 k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __restrict__ twA_g,
                const cd* __restrict__ twN_g, const double* __restrict__ scal, const double* __restrict__ vx_g,
-               const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny,
-               long long row0, CnTab<RT> cn, int rev, float pol_ld, float pol_st, float pol_spec) {
+               const double* __restrict__ vy, const double* __restrict__ vz, double dt, int ntiles, int ny, int nz,
+               int nb, long long row0, CnTab<RT> cn, int rev, float pol_ld, float pol_st, float pol_spec) {
     typedef typename CnCoef<RT>::type CT;
     // A group of GT = 8*T threads owns one tile: its first half runs the four pair transforms (T threads
     // per pair), then all of it runs calcnu (T threads per line) and calclux (one 16-point chunk each).
@@ -82,19 +82,27 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
         const int lp = t / T, m = t % T;                 // transform: pair lp (t < GT/2); calcnu: line lp, x = j*T + m
         const int r = t % XR, c = t / XR;                // calclux: line r, chunk c
         const cd* twA = tw; const cd* twN = tw + N;
-        const double s = scal[SC_S];
-        const double dtG = dt * (scal[SC_G] * scal[SC_S2]), dtD = dt * scal[SC_D];   // u = dt V + dtG |q|^2 + dtD Phi
+        // u = dt V + dtG |q|^2 + dtD Phi; the scalars belong to the tile's batch member (one member: loaded once)
+        double s = scal[SC_S];
+        double dtG = dt * (scal[SC_G] * scal[SC_S2]), dtD = dt * scal[SC_D];
         // trap potential of this thread's line, V_y + V_z, fetched one tile ahead (global tables)
-        auto vrow_of = [&](int i) {
+        auto row_of = [&](int i) {
             long long tile = (long long)blockIdx.x + (long long)i * gridDim.x;
             if (rev) tile = ntiles - 1 - tile;
-            const int row = (int)(row0 + tile * XR) + lp;
-            return dt * (vy[row % ny] + vz[row / ny]);
+            return (int)(row0 + tile * XR) + lp;
+        };
+        auto vrow_of = [&](int i) {
+            const int row = row_of(i);
+            return dt * (vy[row % ny] + vz[(row / ny) % nz]);
         };
         double vrow = (g < nmine) ? vrow_of(g) : 0.0;
         for (int i = g; i < nmine; i += NG) {
             const int st = i % NST;
             const double vrow_next = (i + NG < nmine) ? vrow_of(i + NG) : 0.0;
+            if (nb > 1) {
+                const double* sc = scal + (size_t)(row_of(i) / (ny * nz)) * SC_COUNT;
+                s = sc[SC_S]; dtG = dt * (sc[SC_G] * sc[SC_S2]); dtD = dt * sc[SC_D];
+            }
             wait_issued(issued, i);
             mbar_wait(full + st, (i / NST) & 1);
             cd* ps = (cd*)(base + (size_t)st * STAGE_BYTES);
@@ -235,8 +243,8 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
 template <class P, int XP, int NG, int NST>
 __global__ void __launch_bounds__(NG* XP* P::T + 96, 1)
 k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA_g,
-                const cd* __restrict__ twN_g, const double* __restrict__ scal, int ntiles, int rev, float pol_psi,
-                float pol_spec) {
+                const cd* __restrict__ twN_g, double* __restrict__ scal, int ntiles, int tiles_per_member, int nb,
+                int advance, int rev, float pol_psi, float pol_spec) {
     constexpr int XR = 2 * XP;
     constexpr int T = P::T, N = P::N, GT = XP * T, NT = NG * GT + 96;
     constexpr int NXHP = nxhp_of(N);
@@ -266,9 +274,10 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
     if (tid < NG * GT) {
         const int g = tid / GT, t = tid % GT, lp = t / T, m = t % T;
         const cd* twA = tw; const cd* twN = tw + N;
-        const double s2 = scal[SC_S2];
+        double s2 = scal[SC_S2];
         for (int i = g; i < nmine; i += NG) {
             const int st = i % NST;
+            if (nb > 1) s2 = scal[(size_t)(tile_of(i) / tiles_per_member) * SC_COUNT + SC_S2];    // the tile's batch member
             wait_issued(issued, i);
             mbar_wait(full + st, (i / NST) & 1);
             cd* pr = (cd*)(base + (size_t)st * STAGE_BYTES) + lp * 2 * N;     // the pair's area
@@ -309,6 +318,9 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
             if ((tid & 31) == 0) mbar_arrive(done + st);
         }
     } else if (tid == NG * GT) {
+        // first kernel of a step: move the NSTP ramp on (nothing in this kernel reads G or D)
+        if (advance && blockIdx.x == 0)
+            for (int b = 0; b < nb; ++b) ramp_advance(scal + (size_t)b * SC_COUNT);
         const uint64_t pol = l2_policy_code(pol_psi);
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
@@ -341,6 +353,7 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
 // launchers
 // ------------------------------------------------------------------------------------------------
 int dbec_xline_supported(const dbec_handle_s* h) {
+    // (a tile of 8 lines never straddles two batch members: ny * nz is a multiple of 8)
     return h->use_tma && (h->nx == 128 || h->nx == 256 || h->nx == 512) && ((h->ny * h->nz) % 8 == 0);
 }
 
@@ -360,7 +373,7 @@ template <int N, bool RT, int NG, int NST, int XP = XPlan<N>::XP> static int lau
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
     CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, h->spec + row0 * NXHP, h->psi + row0 * N, h->ax[0].twA, h->ax[0].twN, h->scal,
-                                             h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, row0,
+                                             h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, h->nz, h->nb, row0,
                                              make_cntab<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]));
     h->launches++;
     return (int)cudaGetLastError();
@@ -376,7 +389,7 @@ int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs) {
     }
 }
 
-template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s* h, int z0, int nzs) {
+template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance) {
     typedef typename XPlan<N>::P P;
     constexpr int XP = XPlan<N>::XP, XR = 2 * XP;
     constexpr int GT = XP * P::T, NXHP = nxhp_of(N);
@@ -388,16 +401,16 @@ template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s*
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
     CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
-                                             ntiles, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC]));
+                                             ntiles, h->ny * h->nz / XR, h->nb, advance, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC]));
     h->launches++;
     return (int)cudaGetLastError();
 }
 
-int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs) {
+int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance) {
     switch (h->nx) {
-        case 128: return launch_xline_density<128, 4, 12>(h, z0, nzs);
-        case 256: return launch_xline_density<256, 4, 6>(h, z0, nzs);
-        case 512: return launch_xline_density<512, 4, 6>(h, z0, nzs);
+        case 128: return launch_xline_density<128, 4, 12>(h, z0, nzs, advance);
+        case 256: return launch_xline_density<256, 4, 6>(h, z0, nzs, advance);
+        case 512: return launch_xline_density<512, 4, 6>(h, z0, nzs, advance);
         default: return (int)cudaErrorInvalidValue;
     }
 }

@@ -21,7 +21,9 @@ DBEC_OK, DBEC_EINVAL, DBEC_ESIZE, DBEC_EWORKSPACE, DBEC_ECUDA, DBEC_ENODEVICE = 
 EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi", "dbec_set_coupling",
            "dbec_step", "dbec_observables", "dbec_destroy", "dbec_strerror", "dbec_last_cuda_error",
            "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
-           "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel", "dbec_build_id"]
+           "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel", "dbec_build_id",
+           "dbec_set_ramp", "dbec_workspace_bytes_batch", "dbec_create_batch", "dbec_batch_size",
+           "dbec_set_coupling_batch", "dbec_observables_batch", "dbec_density_1d", "dbec_density_2d"]
 KERNEL_SLOTS = 8
 
 
@@ -85,6 +87,15 @@ def lib():
         L.dbec_kernel_name.restype = C.c_char_p
         L.dbec_pass_kernel.argtypes = [vp, C.c_int]
         L.dbec_pass_kernel.restype = C.c_char_p
+        dp = C.POINTER(C.c_double)
+        L.dbec_set_ramp.argtypes = [vp, C.c_int] + [C.c_double] * 4
+        L.dbec_workspace_bytes_batch.argtypes = [pp, C.c_int, C.POINTER(C.c_size_t)]
+        L.dbec_create_batch.argtypes = [pp, C.c_int, vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.dbec_batch_size.argtypes = [vp, C.POINTER(C.c_int)]
+        L.dbec_set_coupling_batch.argtypes = [vp, dp, dp]
+        L.dbec_observables_batch.argtypes = [vp, C.POINTER(DbecObs)]
+        L.dbec_density_1d.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
+        L.dbec_density_2d.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.dbec_build_id.argtypes = []
         L.dbec_build_id.restype = C.c_char_p
         _lib = L
@@ -103,39 +114,41 @@ def params_of(w, G=None, D=None) -> DbecParams:
                   d_perp=w.d_perp, cutoff=w.cutoff, plane=getattr(w, "plane", 0))
 
 
-def workspace_bytes(p: DbecParams) -> int:
+def workspace_bytes(p: DbecParams, nbatch: int = 1) -> int:
     n = C.c_size_t(0)
-    rc = lib().dbec_workspace_bytes(C.byref(p), C.byref(n))
+    rc = lib().dbec_workspace_bytes_batch(C.byref(p), int(nbatch), C.byref(n))
     if rc:
-        raise DbecError(rc, "dbec_workspace_bytes")
+        raise DbecError(rc, "dbec_workspace_bytes_batch")
     return int(n.value)
 
 
 class Dbec:
-    """One simulation on the current CUDA device.  Methods mirror the C entry points."""
+    """One simulation (or a batch of `nbatch` independent ones with the same parameters) behind the C ABI."""
 
-    def __init__(self, p: DbecParams, device="cuda:0", stream=None):
+    def __init__(self, p: DbecParams, device="cuda:0", stream=None, nbatch: int = 1):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1601_04640_b200 needs a CUDA device (sm_100a); there is no CPU path")
         self._torch = torch
         self.p = p
+        self.nbatch = int(nbatch)
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         # a stream of its own by default: the step is replayed as a CUDA graph, which the legacy default
         # stream cannot capture
         self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
-        nbytes = workspace_bytes(p)
+        nbytes = workspace_bytes(p, self.nbatch)
         # caller-owned workspace; torch allocations are 512-byte aligned
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         assert self.workspace.data_ptr() % 256 == 0
         self._h = C.c_void_p()
-        rc = lib().dbec_create(C.byref(p), C.c_void_p(self.workspace.data_ptr()), nbytes,
-                               C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
+        rc = lib().dbec_create_batch(C.byref(p), self.nbatch, C.c_void_p(self.workspace.data_ptr()), nbytes,
+                                     C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
         if rc:
-            raise DbecError(rc, "dbec_create")
-        self.shape = (p.nz, p.ny, p.nx) if p.ndim == 3 else (p.ny, p.nx)
-        self.npoints = p.nx * p.ny * p.nz
+            raise DbecError(rc, "dbec_create_batch", lib().dbec_last_cuda_error(None))
+        self.grid_shape = (p.nz, p.ny, p.nx) if p.ndim == 3 else (p.ny, p.nx)
+        self.shape = self.grid_shape if self.nbatch == 1 else (self.nbatch,) + self.grid_shape
+        self.npoints = p.nx * p.ny * p.nz * self.nbatch
 
     # -- helpers
     def _ck(self, rc, what):
@@ -183,15 +196,43 @@ class Dbec:
         return out
 
     def set_coupling(self, G, D):
-        self._ck(lib().dbec_set_coupling(self._h, float(G), float(D)), "dbec_set_coupling")
+        """Scalars: every member; sequences of nbatch values: per member."""
+        if np.ndim(G) == 0 and np.ndim(D) == 0:
+            self._ck(lib().dbec_set_coupling(self._h, float(G), float(D)), "dbec_set_coupling")
+            return
+        g = np.ascontiguousarray(np.broadcast_to(np.asarray(G, dtype=np.float64), (self.nbatch,)))
+        d = np.ascontiguousarray(np.broadcast_to(np.asarray(D, dtype=np.float64), (self.nbatch,)))
+        dp = C.POINTER(C.c_double)
+        self._ck(lib().dbec_set_coupling_batch(self._h, g.ctypes.data_as(dp), d.ctypes.data_as(dp)), "dbec_set_coupling_batch")
+
+    def set_ramp(self, nstp, G0, D0, G1, D1):
+        self._ck(lib().dbec_set_ramp(self._h, int(nstp), float(G0), float(D0), float(G1), float(D1)), "dbec_set_ramp")
 
     def step(self, n=1):
         self._ck(lib().dbec_step(self._h, int(n)), "dbec_step")
 
-    def observables(self) -> dict:
-        o = DbecObs()
-        self._ck(lib().dbec_observables(self._h, C.byref(o)), "dbec_observables")
-        return o.as_dict()
+    def observables(self):
+        """One dict (plain handle) or a list of nbatch dicts (batch handle)."""
+        if self.nbatch == 1:
+            o = DbecObs()
+            self._ck(lib().dbec_observables(self._h, C.byref(o)), "dbec_observables")
+            return o.as_dict()
+        arr = (DbecObs * self.nbatch)()
+        self._ck(lib().dbec_observables_batch(self._h, arr), "dbec_observables_batch")
+        return [o.as_dict() for o in arr]
+
+    def density_1d(self, axis, member=0) -> np.ndarray:
+        out = np.empty((self.p.nx, self.p.ny, self.p.nz)[axis], dtype=np.float64)
+        self._ck(lib().dbec_density_1d(self._h, int(member), int(axis), C.c_void_p(out.ctypes.data), 0), "dbec_density_1d")
+        return out
+
+    def density_2d(self, axis_integrated, member=0) -> np.ndarray:
+        shp = [self.p.nz, self.p.ny, self.p.nx]
+        del shp[2 - axis_integrated]
+        out = np.empty(shp, dtype=np.float64)
+        self._ck(lib().dbec_density_2d(self._h, int(member), int(axis_integrated), C.c_void_p(out.ctypes.data), 0),
+                 "dbec_density_2d")
+        return out
 
     def phi_dd(self):
         out = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)

@@ -328,6 +328,193 @@ def test_errors_and_edge_cases(gp):
     sim.close()
 
 
+# ------------------------------------------------------------------ f3: run protocol (readings S26, S27)
+@pytest.mark.parametrize("w", [grid3(32, 32, 32, IMAG, G=0.0, D=0.0), grid3(128, 16, 32, REAL, G=0.0, D=0.0),
+                               grid2(256, 128, REAL, G=0.0, D=0.0), grid2(32, 64, IMAG, G=0.0, D=0.0)], ids=wid)
+def test_nstp_ramp_matches_oracle(gp, ob, w):
+    """dbec_set_ramp: the schedule lives in device scalars that the first kernel of every step advances, so the
+    replayed CUDA graph sees it; observables in between must not advance it."""
+    psi0 = random_psi(w, 9) if w.time_mode == REAL else initial_psi(w)
+    sim = gp.Dbec(gp.params_of(w))
+    o = ob.Oracle(ob.params_of(w))
+    sim.set_psi(psi0)
+    o.set_psi(psi0)
+    sim.set_ramp(5, 1.0, 0.5, 30.0, 18.0)
+    o.set_ramp(5, 1.0, 0.5, 30.0, 18.0)
+    for n in (2, 1, 4):                                # 7 steps: the ramp ends inside the last call
+        sim.step(n)
+        o.step(n)
+        a, b = sim.observables(), o.observables()      # uses the CURRENT ramp value of G and D in mu / E
+        for k in ("norm", "mu", "energy", "rms_x", "rms_y"):
+            assert abs(a[k] - b[k]) <= OBS_TOL * abs(b[k]), (n, k)
+        assert relerr(sim.get_psi(), o.get_psi()) < PSI_TOL
+    for x in (sim, o):                                 # an explicit value ends a running ramp
+        x.set_ramp(3, 0.0, 0.0, 9.0, 6.0)
+        x.step(1)
+        x.set_coupling(7.0, 3.0)
+        x.step(2)
+    assert relerr(sim.get_psi(), o.get_psi()) < PSI_TOL
+    sim.close()
+    o.close()
+
+
+def test_imag_to_real_handoff_on_device(gp, ob):
+    """The paper's NSTP = 0 restart: a real-time run starts from the state an
+    imaginary-time run produced.  Here the state goes from one handle to the other as a DEVICE buffer."""
+    import torch
+    w = grid3(32, 32, 64, IMAG, G=20.0, D=10.0)
+    from dataclasses import replace
+    wr = replace(w, time_mode=REAL, dt=0.5 * w.dx ** 2)
+    psi0 = initial_psi(w)
+    a = gp.Dbec(gp.params_of(w))
+    b = gp.Dbec(gp.params_of(wr))
+    a.set_psi(psi0)
+    a.step(20)
+    buf = torch.empty(w.shape, dtype=torch.complex128, device="cuda")
+    a.get_psi(buf)                                     # applies the deferred norm factor
+    b.set_psi(buf)
+    b.set_ramp(0, 0.0, 0.0, 25.0, 12.0)                # NSTP = 0: end values at once
+    b.step(5)
+    got = b.get_psi()
+    oa = ob.Oracle(ob.params_of(w))
+    oa.set_psi(psi0)
+    oa.step(20)
+    orr = ob.Oracle(ob.params_of(wr))
+    orr.set_psi(oa.get_psi())
+    orr.set_ramp(0, 0.0, 0.0, 25.0, 12.0)
+    orr.step(5)
+    assert relerr(got, orr.get_psi()) < 1e-11           # 25 steps of round-off
+    assert abs(b.observables()["norm"] - 1.0) < 1e-12
+    for s in (a, b):
+        s.close()
+
+
+@pytest.mark.parametrize("w", [grid3(32, 16, 64, IMAG, d=(0.4, 0.3, 0.6)), grid3(128, 128, 128, REAL),
+                               grid2(64, 32, REAL, dy=0.3), grid2(512, 256, IMAG)], ids=wid)
+def test_integrated_densities_match_oracle(gp, ob, w):
+    psi0 = random_psi(w, 12)
+    sim = gp.Dbec(gp.params_of(w))
+    o = ob.Oracle(ob.params_of(w))
+    sim.set_psi(1.3 * psi0)
+    o.set_psi(1.3 * psi0)
+    if w.time_mode == IMAG:                            # leaves a deferred norm factor in the handle
+        sim.step(1)
+        o.step(1)
+    for ax in range(w.ndim):
+        assert relerr(sim.density_1d(ax), o.density_1d(ax)) < PSI_TOL, ax
+    if w.ndim == 3:
+        for ax in range(3):
+            assert relerr(sim.density_2d(ax), o.density_2d(ax)) < PSI_TOL, ax
+    else:
+        import ctypes as C
+        buf = np.empty(8)
+        assert gp.lib().dbec_density_2d(sim._h, 0, 0, C.c_void_p(buf.ctypes.data), 0) == gp.DBEC_EINVAL
+    # the observables still work afterwards (the densities borrow their scratch buffer)
+    assert abs(sim.observables()["mu"] - o.observables()["mu"]) <= OBS_TOL * abs(o.observables()["mu"])
+    sim.close()
+    o.close()
+
+
+# ------------------------------------------------------------------ f4: batched handles
+BATCH_CASES = [(grid3(32, 32, 32, IMAG), 5), (grid3(32, 32, 32, REAL), 3), (grid3(16, 64, 32, IMAG), 4),
+               (grid3(128, 16, 16, REAL), 3), (grid3(128, 32, 128, IMAG), 2), (grid2(512, 512, REAL), 3),
+               (grid2(256, 128, IMAG), 4), (grid2(32, 64, IMAG), 7), (grid2(128, 16, REAL, plane=1), 3)]
+
+
+@pytest.mark.parametrize("w,nb", BATCH_CASES, ids=[f"{wid(w)}-x{nb}" for w, nb in BATCH_CASES])
+def test_batch_members_match_single_oracle_runs(gp, ob, w, nb):
+    """dbec_create_batch: nb independent members (different psi, different G and D) advance in the same
+    launches; each must match its own oracle run, observables included."""
+    psis = np.stack([(1.0 + 0.1 * m) * (random_psi(w, 30 + m) if w.time_mode == REAL else initial_psi(w, noise=1e-3 * (m + 1)))
+                     for m in range(nb)])
+    Gs = np.array([w.G * (1 + 0.2 * m) for m in range(nb)])
+    Ds = np.array([w.D * (1 - 0.1 * m) for m in range(nb)])
+    sim = gp.Dbec(gp.params_of(w), nbatch=nb)
+    assert sim.shape == (nb,) + w.shape
+    sim.set_psi(psis)
+    sim.set_coupling(Gs, Ds)
+    sim.step(3)
+    got = sim.get_psi()
+    obs = sim.observables()
+    assert len(obs) == nb
+    for m in range(nb):
+        o = ob.Oracle(ob.params_of(w, G=Gs[m], D=Ds[m]))
+        o.set_psi(psis[m])
+        o.step(3)
+        assert relerr(got[m], o.get_psi()) < PSI_TOL, m
+        b = o.observables()
+        for k in b:
+            if w.ndim == 2 and k == "rms_z":
+                continue
+            assert abs(obs[m][k] - b[k]) <= OBS_TOL * max(abs(b[k]), 1e-300), (m, k)
+        if m == nb - 1:
+            assert relerr(sim.density_1d(0, member=m), o.density_1d(0)) < PSI_TOL
+        o.close()
+    # the single-part entry points act on every member
+    sim.set_psi(psis)
+    sim.cn_sweep(1)
+    sim.normalize()
+    got = sim.get_psi()
+    for m in (0, nb - 1):
+        p = ob.params_of(w)
+        ref = ob.normalize(p, ob.cn_sweep(p, psis[m], 1))
+        assert relerr(got[m], ref) < PSI_TOL, m
+    import ctypes as C
+    one = gp.DbecObs()
+    assert gp.lib().dbec_observables(sim._h, C.byref(one)) == gp.DBEC_EINVAL
+    sim.close()
+
+
+def test_batch_is_bitwise_the_single_handle(gp):
+    """Member m of a batch goes through the same arithmetic as a handle of its own."""
+    for w, nb in ((grid3(32, 32, 32, IMAG), 3), (grid2(256, 128, REAL), 2)):
+        psis = np.stack([random_psi(w, 40 + m) for m in range(nb)])
+        sim = gp.Dbec(gp.params_of(w), nbatch=nb)
+        sim.set_psi(psis)
+        sim.step(4)
+        got = sim.get_psi()
+        sim.close()
+        for m in range(nb):
+            one = gp.Dbec(gp.params_of(w))
+            one.set_psi(psis[m])
+            one.step(4)
+            assert np.array_equal(one.get_psi(), got[m]), (wid(w), m)
+            one.close()
+
+
+def test_workspace_guard_bands_stay_intact(gp):
+    """compute-sanitizer is not available on this pool: instead, every persistent / one-tile-per-block kernel
+    runs on a workspace with 1 MiB guard bands on both sides (and between nothing else the caller owns); a
+    bulk or TMA store that leaves the workspace would land in them."""
+    import ctypes as C
+    import torch
+    L = gp.lib()
+    shapes = [grid3(32, 32, 32, IMAG), grid3(128, 128, 128, REAL), grid3(256, 16, 16, IMAG), grid3(16, 256, 32, REAL),
+              grid3(32, 16, 512, IMAG), grid2(512, 512, REAL), grid2(16, 16, IMAG), grid2(128, 256, IMAG, plane=1)]
+    for w in shapes:
+        for nb in (1, 3):
+            p = gp.params_of(w)
+            n = C.c_size_t()
+            assert L.dbec_workspace_bytes_batch(C.byref(p), nb, C.byref(n)) == 0
+            G = 1 << 20
+            buf = torch.full((n.value + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+            st = torch.cuda.Stream()
+            torch.cuda.synchronize()
+            h = C.c_void_p()
+            assert L.dbec_create_batch(C.byref(p), nb, C.c_void_p(buf.data_ptr() + G), n.value, C.c_void_p(st.cuda_stream), C.byref(h)) == 0
+            psi = np.stack([random_psi(w, 3 + m) for m in range(nb)])
+            assert L.dbec_set_psi(h, C.c_void_p(psi.ctypes.data), 0) == 0
+            assert L.dbec_step(h, 3) == 0
+            obs = (gp.DbecObs * nb)()
+            assert L.dbec_observables_batch(h, obs) == 0
+            out = np.empty_like(psi)
+            assert L.dbec_get_psi(h, C.c_void_p(out.ctypes.data), 0) == 0
+            assert L.dbec_destroy(h) == 0
+            torch.cuda.synchronize()
+            assert bool((buf[:G] == 0xA5).all()) and bool((buf[-G:] == 0xA5).all()), (wid(w), nb)
+            assert np.all(np.isfinite(out.view(np.float64)))
+
+
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 
 
