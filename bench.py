@@ -16,11 +16,18 @@ pairs (dbec_step_profile); `cpu_baseline` = the CPU oracle timed on this box's h
 Multi-GPU: the step does not shard without all-to-all transposes: N ranks
 run N independent replicas, no data-path collective, `scaling` = "weak".
 
-`--impl reference` times the oracle (oracle/, as it stands) on the host cores, rank 0 only.
+Beside the headline the line carries `configs` (all five BASELINE.json workloads: ms/step, updates/s, model
+fraction, dominant kernel and its roofline fraction — `north_star` asks for the five), `observables` (one
+calcmuen + calcrms evaluation, excluded from the step and reported separately) and `batch`
+(dbec_create_batch: many small grids per launch against one of them alone).
+
+`--impl reference` times the oracle (oracle/, as it stands) on the host cores, rank 0 only; `config.workload`
+names the grid it really ran.
 """
 from __future__ import annotations
 
 import argparse
+import datetime
 import json
 import os
 import subprocess
@@ -51,6 +58,13 @@ ALG_BYTES_PER_POINT = {
     "cn_z": 32,
 }
 MODEL_BYTES_PER_POINT = {3: 208, 2: 144}    # SURVEY.md §8(d) "Model M": fixed reference accounting
+# What this repository's fused pipeline itself has to stream (x sweep inside the nonlinear kernel): the honest
+# denominator beside M.
+FUSED_BYTES_PER_POINT = {3: 176, 2: 112}
+# One calcmuen + calcrms evaluation (reported separately): the forward passes and the spectral
+# multiply as in a step, the last inverse writing Phi (8 + 8), the reduction pass reading psi and Phi (16 + 8).
+OBS_BYTES_PER_POINT = {3: 24 + 16 + 16 + 16 + 16 + 24, 2: 24 + 16 + 16 + 24}
+REF_BUDGET_S = 240.0                        # --impl reference: whole run (K + W oracle steps)
 
 
 def measured_peaks():
@@ -62,7 +76,9 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clock / throttle-reason samples while the timed region runs."""
+    """nvidia-smi clock / throttle-reason samples.  Each line is stamped by nvidia-smi itself (`timestamp`
+    field), so that the window [mark_start, mark_stop] selects the samples taken while the timed region ran,
+    however late Python reads them from the pipe.  No fall-back to samples outside the window."""
     Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -72,16 +88,26 @@ class ClockSampler:
         self.t0 = self.t1 = None
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
-                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                ["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
         except Exception:
             self.proc = None
 
+    @staticmethod
+    def _stamp(text):
+        try:
+            return datetime.datetime.strptime(text.strip(), "%Y/%m/%d %H:%M:%S.%f").timestamp()
+        except ValueError:
+            return None
+
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append((time.time(), line.strip()))
+            f = [x.strip() for x in line.split(",")]
+            t = self._stamp(f[0]) if f else None
+            if t is not None and len(f) >= 8:
+                self.rows.append((t, f))
 
     def mark_start(self):
         self.t0 = time.time()
@@ -91,22 +117,21 @@ class ClockSampler:
 
     def close(self):
         if self.proc:
-            time.sleep(0.12)
+            time.sleep(0.1)
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=2)
             except Exception:
                 self.proc.kill()
 
-    def summary(self):
+    def in_window(self):
+        if self.t0 is None or self.t1 is None:
+            return []
+        return [f for t, f in self.rows if self.t0 <= t <= self.t1]
+
+    def summary(self, note=""):
         sm, smax, reasons = [], [], set()
-        rows = [r for t, r in self.rows if self.t0 is not None and self.t0 - 0.05 <= t <= (self.t1 or 1e30) + 0.1]
-        if not rows:
-            rows = [r for _, r in self.rows]
-        for r in rows:
-            f = [x.strip() for x in r.split(",")]
-            if len(f) < 8:
-                continue
+        for f in self.in_window():
             try:
                 sm.append(float(f[1]))
                 smax.append(float(f[2]))
@@ -115,10 +140,12 @@ class ClockSampler:
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[4:8]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
-        if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
-                "samples": len(sm)}
+        out = {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(smax)) if smax else None,
+               "reasons": sorted(reasons), "samples": len(sm),
+               "window_s": None if self.t0 is None or self.t1 is None else self.t1 - self.t0}
+        if note:
+            out["window"] = note
+        return out
 
 
 def oracle_time(w, steps, threads_hint=None):
@@ -144,8 +171,9 @@ def shrunk(w, n):
 
 
 def run_reference(args, w):
-    """The reference arm: the oracle on the host cores; each step is one oracle SSCN step on a bounded
-    sample (a coarser grid of the same box, same parameters) sized so that K+W steps end in minutes."""
+    """The reference arm: the oracle on the host cores.  Each step is one oracle SSCN step of the named
+    workload; if K + W steps of the full grid would take longer than REF_BUDGET_S, the grid is coarsened
+    (same box and parameters) and `config.workload` / `config.grid` name the grid that really ran."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -154,9 +182,8 @@ def run_reference(args, w):
     probe = shrunk(w, 32)
     t_probe, threads = oracle_time(probe, 2)
     per_point = t_probe / probe.npoints
-    budget = 120.0
     n = max(w.nx, w.ny, w.nz)
-    while n > 32 and per_point * shrunk(w, n).npoints * (args.steps + args.warmup) * 1.3 > budget:
+    while n > 32 and per_point * shrunk(w, n).npoints * (args.steps + args.warmup) * 1.3 > REF_BUDGET_S:
         n //= 2
     ws = shrunk(w, n)
     o = ob.Oracle(ob.params_of(ws, G=ws.G_run, D=ws.D_run))
@@ -167,13 +194,17 @@ def run_reference(args, w):
     dt = time.perf_counter() - t0
     o.close()
     value = ws.npoints * args.steps / dt
-    sample = (f"{args.steps} oracle steps on a {ws.nx}x{ws.ny}x{ws.nz} grid of the same box and parameters "
-              f"(1/{w.npoints // ws.npoints} of the {w.name} grid points)")
+    full = ws.npoints == w.npoints
+    name = w.name if full else f"{w.name} coarsened to {ws.nx}x{ws.ny}x{ws.nz}"
+    sample = (f"{args.steps} oracle steps on the full {ws.nx}x{ws.ny}x{ws.nz} grid" if full else
+              f"{args.steps} oracle steps on a {ws.nx}x{ws.ny}x{ws.nz} grid of the same box and parameters "
+              f"(1/{w.npoints // ws.npoints} of the {w.name} grid points: {args.steps + args.warmup} full-grid steps "
+              f"would exceed the {REF_BUDGET_S:.0f} s budget)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "sample_grid": [ws.nx, ws.ny, ws.nz],
-                       "mode": "real" if w.time_mode else "imag"},
+            "config": {"workload": name, "grid": [ws.nx, ws.ny, ws.nz], "named_grid": [w.nx, w.ny, w.nz],
+                       "full_grid": full, "mode": "real" if w.time_mode else "imag"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -194,6 +225,92 @@ def max_over_ranks(x, world, device="cpu"):
 def whole_job_value(npoints, steps, world, seconds):
     """Replicas only: every rank advances its own npoints-grid `steps` times; the job took `seconds`."""
     return world * npoints * steps / seconds
+
+
+def timed_steps(torch, sim, steps):
+    """Milliseconds for `steps` steps: CUDA events on the library's own stream, synchronised on both sides."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.synchronize()
+    e0.record(sim.stream)
+    sim.step(steps)
+    e1.record(sim.stream)
+    sim.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def kernel_profile(sim, w, steps, peak):
+    """Per-pass average milliseconds (CUDA event pairs around every launch, dbec_step_profile) and the roofline
+    fraction of each pass by its algorithmic bytes."""
+    sim.step_profile(2)
+    prof = sim.step_profile(steps)
+    kernels = sim.pass_kernels()
+    per_kernel = {}
+    for name, (tot_ms, cnt) in prof.items():
+        avg_ms = tot_ms / cnt
+        gbs = ALG_BYTES_PER_POINT[name] * w.npoints / (avg_ms * 1e-3) / 1e9
+        per_kernel[name] = {"kernel": kernels.get(name, ""), "ms": avg_ms, "alg_GBps": gbs, "frac": gbs / peak}
+    return per_kernel
+
+
+def observables_ms(torch, sim, reps=3):
+    """One dbec_observables call (calcmuen + calcrms: a dipolar pass, Phi written, one reduction pass)."""
+    sim.observables()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.synchronize()
+    e0.record(sim.stream)
+    for _ in range(reps):
+        sim.observables()
+    e1.record(sim.stream)
+    sim.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def measure_config(torch, dbec, key, dev, peak, steps=None):
+    """ms/step, updates/s, model fraction and dominant kernel of one BASELINE.json workload."""
+    w = workload(key)
+    sim = dbec.Dbec(dbec.params_of(w), device=dev)
+    sim.set_psi(initial_psi(w))
+    if (w.G_run, w.D_run) != (w.G, w.D):
+        sim.set_coupling(w.G_run, w.D_run)
+    sim.step(5)
+    if steps is None:
+        est = timed_steps(torch, sim, 5) / 5
+        steps = int(min(2000, max(20, 150.0 / max(est, 1e-3))))      # ~0.15 s of steps
+    ms = timed_steps(torch, sim, steps) / steps
+    per_kernel = kernel_profile(sim, w, 5, peak)
+    top = max(per_kernel, key=lambda k: per_kernel[k]["ms"])
+    obs_ms = observables_ms(torch, sim)
+    sim.close()
+    model, fused = MODEL_BYTES_PER_POINT[w.ndim], FUSED_BYTES_PER_POINT[w.ndim]
+    gb = w.npoints / (ms * 1e-3) / 1e9
+    return {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "mode": "real" if w.time_mode else "imag", "steps": steps,
+            "ms_per_step": ms, "updates_per_s": w.npoints / (ms * 1e-3),
+            "step_model": {"bytes_per_point": model, "frac": model * gb / peak},
+            "fused_pipeline": {"bytes_per_point": fused, "frac": fused * gb / peak},
+            "top_kernel": {"pass": top, "kernel": per_kernel[top]["kernel"], "ms": per_kernel[top]["ms"],
+                           "frac": per_kernel[top]["frac"]},
+            "field_MiB": 16 * w.npoints / 2 ** 20,
+            "observables_ms": obs_ms}
+
+
+def measure_batch(torch, dbec, key, nbatch, dev):
+    """dbec_create_batch: nbatch members of workload `key` per launch against one member alone."""
+    w = workload(key)
+    psi0 = initial_psi(w)
+    out = {}
+    for nb in (1, nbatch):
+        sim = dbec.Dbec(dbec.params_of(w), device=dev, nbatch=nb)
+        sim.set_psi(psi0 if nb == 1 else np.broadcast_to(psi0, (nb,) + psi0.shape).copy())
+        if (w.G_run, w.D_run) != (w.G, w.D):
+            sim.set_coupling(w.G_run, w.D_run)
+        sim.step(10)
+        est = timed_steps(torch, sim, 10) / 10
+        steps = int(min(2000, max(20, 100.0 / max(est, 1e-3))))
+        ms = timed_steps(torch, sim, steps) / steps
+        sim.close()
+        out[nb] = {"ms_per_step": ms, "updates_per_s": nb * w.npoints / (ms * 1e-3)}
+    return {"workload": w.name, "nbatch": nbatch, "single": out[1], "batched": out[nbatch],
+            "throughput_ratio": out[nbatch]["updates_per_s"] / out[1]["updates_per_s"]}
 
 
 def run_ours(args, w):
@@ -241,6 +358,17 @@ def run_ours(args, w):
     launches = sim.launch_count() - l0
     ms = max_over_ranks(ms, world, dev)
     value = whole_job_value(w.npoints, args.steps, world, ms * 1e-3)
+    clock_note = "the timed region"
+    if sampler and len(sampler.in_window()) < 3:
+        # the region was too short for nvidia-smi's sampling period: keep the same load running for 0.5 s more
+        # and report the clocks of that stretch (timing above is untouched)
+        leg = max(args.steps, int(500.0 / max(ms / args.steps, 1e-3)))
+        sampler.mark_start()
+        sim.step(leg)
+        sim.synchronize()
+        sampler.mark_stop()
+        clock_note = (f"{leg} further steps of the same workload right after the timed region "
+                      f"(the region itself lasted {ms:.1f} ms, shorter than three sampling periods)")
     obs = sim.observables()
 
     # ---- end to end through the C ABI with host buffers ----
@@ -265,26 +393,22 @@ def run_ours(args, w):
     line = None
     if rank == 0:
         sim.set_psi(psi0)
-        sim.step_profile(3)
-        prof_steps = max(5, min(args.steps, 50))
-        prof = sim.step_profile(prof_steps)
         peak, peak_src = measured_peaks()
-        per_kernel = {}
-        kernels = sim.pass_kernels()
-        for name, (tot_ms, cnt) in prof.items():
-            avg_ms = tot_ms / cnt
-            gbs = ALG_BYTES_PER_POINT[name] * w.npoints / (avg_ms * 1e-3) / 1e9
-            per_kernel[name] = {"kernel": kernels.get(name, ""), "ms": avg_ms, "alg_GBps": gbs, "frac": gbs / peak}
+        per_kernel = kernel_profile(sim, w, max(5, min(args.steps, 50)), peak)
         top = max(per_kernel, key=lambda k: per_kernel[k]["ms"])
         step_ms_prof = sum(v["ms"] for v in per_kernel.values())
-        model = MODEL_BYTES_PER_POINT[w.ndim]
-        model_gbs = model * w.npoints / (ms / args.steps * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": kernels.get(top, top), "pass": top, "achieved": per_kernel[top]["alg_GBps"], "peak": peak,
-                    "unit": "GB/s", "frac": per_kernel[top]["frac"], "traffic": None, "peak_source": peak_src,
+        model, fused = MODEL_BYTES_PER_POINT[w.ndim], FUSED_BYTES_PER_POINT[w.ndim]
+        pts_per_ns = w.npoints / (ms / args.steps * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": per_kernel[top]["kernel"], "pass": top, "achieved": per_kernel[top]["alg_GBps"],
+                    "peak": peak, "unit": "GB/s", "frac": per_kernel[top]["frac"], "traffic": None, "peak_source": peak_src,
                     "kernel_ms": per_kernel[top]["ms"], "kernel_share_of_step": per_kernel[top]["ms"] / step_ms_prof,
                     "alg_bytes_per_launch": ALG_BYTES_PER_POINT[top] * w.npoints,
                     "per_kernel": per_kernel,
-                    "step_model": {"bytes_per_point": model, "achieved_GBps": model_gbs, "frac": model_gbs / peak}}
+                    "step_model": {"bytes_per_point": model, "achieved_GBps": model * pts_per_ns, "frac": model * pts_per_ns / peak,
+                                   "note": "SURVEY 8(d) fixed accounting M (counts an x sweep pass the fused kernels never make)"},
+                    "fused_pipeline": {"bytes_per_point": fused, "achieved_GBps": fused * pts_per_ns,
+                                       "frac": fused * pts_per_ns / peak,
+                                       "note": "algorithmic bytes of this repository's own seven-pass pipeline"}}
         tr = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram__bytes_{read,write}.sum per launch
         if os.path.exists(tr):
             import csv
@@ -292,7 +416,29 @@ def run_ours(args, w):
                 for row in csv.DictReader(f):
                     if row["workload"] == w.name and row["pass"] == top:
                         roofline["traffic"] = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
-                        roofline["traffic_source"] = row["source"]
+                        roofline["traffic_source"] = f'{row["source"]} (ncu capture of commit {row.get("commit", "?")})'
+        obs_ms = observables_ms(torch, sim)
+        observables = {"ms": obs_ms, "dram_alg_bytes": OBS_BYTES_PER_POINT[w.ndim] * w.npoints,
+                       "alg_GBps": OBS_BYTES_PER_POINT[w.ndim] * w.npoints / (obs_ms * 1e-3) / 1e9,
+                       "what": "one dbec_observables call (calcmuen + calcrms), excluded from ms_per_step"}
+        sim.close()
+
+        # ---- the five BASELINE.json workloads and the batched small grids (1 GPU only) ----
+        configs, batch = None, None
+        if world == 1 and not args.headline_only:
+            configs = {}
+            for key in ("C1", "C2", "C3", "C4", "C5"):
+                if workload(key).name == w.name:
+                    configs[key] = {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "mode": "real" if w.time_mode else "imag",
+                                    "steps": args.steps, "ms_per_step": ms / args.steps, "updates_per_s": value,
+                                    "step_model": {"bytes_per_point": model, "frac": model * pts_per_ns / peak},
+                                    "fused_pipeline": {"bytes_per_point": fused, "frac": fused * pts_per_ns / peak},
+                                    "top_kernel": {"pass": top, "kernel": per_kernel[top]["kernel"], "ms": per_kernel[top]["ms"],
+                                                   "frac": per_kernel[top]["frac"]},
+                                    "field_MiB": 16 * w.npoints / 2 ** 20, "observables_ms": obs_ms}
+                else:
+                    configs[key] = measure_config(torch, dbec, key, dev, peak)
+            batch = [measure_batch(torch, dbec, "C1", 64, dev), measure_batch(torch, dbec, "C2", 16, dev)]
 
         # ---- CPU baseline: the oracle on this box's cores, bounded sample ----
         cpu = None
@@ -316,16 +462,23 @@ def run_ours(args, w):
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "mode": "real" if w.time_mode else "imag",
                            "psi": "complex128", "parallelism": f"replicas x{world}",
-                           "l2": f"psi is {16 * w.npoints / 2**20:.0f} MiB per field (L2 126 MB); no flush between steps",
+                           "l2": (f"inputs larger than L2: psi is {16 * w.npoints / 2**20:.0f} MiB per field (L2 126 MB), "
+                                  "every pass streams it; no flush between steps"
+                                  if 16 * w.npoints > 126e6 else
+                                  f"psi is {16 * w.npoints / 2**20:.1f} MiB: the working set is L2-resident by nature, no flush"),
                            "G": w.G_run, "D": w.D_run, "dt": w.dt},
-                "clocks": sampler.summary(),
+                "clocks": sampler.summary(clock_note),
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.npoints,
                         "d2h_bytes_per_step": 16 * w.npoints, "steps": e2e_steps},
                 "gpu_launches": launches,
                 "roofline": roofline,
                 "cpu_baseline": cpu,
+                "observables": observables,
+                "configs": configs,
+                "batch": batch,
                 "observables_after_run": obs}
-    sim.close()
+    else:
+        sim.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -341,6 +494,7 @@ def main():
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--headline-only", action="store_true", help="skip the `configs` and `batch` entries")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = workload(args.workload)
