@@ -30,12 +30,13 @@ DBEC_HD cd cn_fma(cd h, cd a, cd b) { return cfma(h, a, b); }
 
 // Forward pass on one chunk from a zero start.  u[i] = p_{j0+i} on entry, d~_{j0+i} on exit.
 // lo = p_{j0-1}, hi = p_{j0+L} (0 outside the line).  h points at h_{j0}.
-template <class CT> DBEC_HD void cn_chunk_forward(cd (&u)[CN_L], cd lo, cd hi, CT kap, const CT* __restrict__ h) {
+// (The chunk length L is deduced from the register array: 16 in the tile kernels, 8 in the warp-per-line kernel.)
+template <class CT, int L> DBEC_HD void cn_chunk_forward(cd (&u)[L], cd lo, cd hi, CT kap, const CT* __restrict__ h) {
     cd prev = lo, d = cmake(0.0, 0.0);
 #pragma unroll
-    for (int i = 0; i < CN_L; ++i) {
+    for (int i = 0; i < L; ++i) {
         cd cur = u[i];
-        cd nxt = (i + 1 < CN_L) ? u[i + 1] : hi;
+        cd nxt = (i + 1 < L) ? u[i + 1] : hi;
         cd r = cn_fma(kap, cur, cadd(prev, nxt));
         d = cn_mul(h[i], cadd(r, d));
         u[i] = d;
@@ -45,11 +46,11 @@ template <class CT> DBEC_HD void cn_chunk_forward(cd (&u)[CN_L], cd lo, cd hi, C
 
 // Backward pass on one chunk: applies the forward fix-up (d_j = d~_j + PF_j D_in) and runs
 // u~_j = d_j + h_j u~_{j+1} from a zero start.  u[i] = u~_{j0+i} on exit.
-template <class CT> DBEC_HD void cn_chunk_backward(cd (&u)[CN_L], cd d_in, const CT* __restrict__ h,
-                                                   const CT* __restrict__ pf) {
+template <class CT, int L> DBEC_HD void cn_chunk_backward(cd (&u)[L], cd d_in, const CT* __restrict__ h,
+                                                          const CT* __restrict__ pf) {
     cd ut = cmake(0.0, 0.0);
 #pragma unroll
-    for (int i = CN_L - 1; i >= 0; --i) {
+    for (int i = L - 1; i >= 0; --i) {
         cd dj = cn_fma(pf[i], d_in, u[i]);
         ut = cn_fma(h[i], ut, dj);
         u[i] = ut;
@@ -57,9 +58,9 @@ template <class CT> DBEC_HD void cn_chunk_backward(cd (&u)[CN_L], cd d_in, const
 }
 
 // Final fix-up: u_j = u~_j + PB_j U_in.
-template <class CT> DBEC_HD void cn_chunk_fix(cd (&u)[CN_L], cd u_in, const CT* __restrict__ pb) {
+template <class CT, int L> DBEC_HD void cn_chunk_fix(cd (&u)[L], cd u_in, const CT* __restrict__ pb) {
 #pragma unroll
-    for (int i = 0; i < CN_L; ++i) u[i] = cn_fma(pb[i], u_in, u[i]);
+    for (int i = 0; i < L; ++i) u[i] = cn_fma(pb[i], u_in, u[i]);
 }
 
 // Carry into chunk c of the forward pass: D_in = d_{c*L-1}, from the zero-start chunk ends

@@ -4,6 +4,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
+#include <cmath>
 #include <new>
 #include <vector>
 #include "dbec_internal.hpp"
@@ -40,13 +42,28 @@ static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 static size_t axis_table_bytes(int n) {
     // twA, twN (cd n each); vtrap, x2 (double n each); h, pf, pb (cd n each) + pfe, pbs (cd 32 each);
-    // the same five as doubles
+    // the same five as doubles; pf, pb for chunks of 8 (cd n each) + their pfe, pbs (cd 128 each), and as doubles
     size_t b = 0;
     b += up256(sizeof(cd) * n) * 2;
     b += up256(sizeof(double) * n) * 2;
     b += up256(sizeof(cd) * n) * 3 + up256(sizeof(cd) * 32) * 2;
     b += up256(sizeof(double) * n) * 3 + up256(sizeof(double) * 32) * 2;
+    b += up256(sizeof(cd) * n) * 2 + up256(sizeof(cd) * 128) * 2;
+    b += up256(sizeof(double) * n) * 2 + up256(sizeof(double) * 128) * 2;
     return b;
+}
+
+// Carry terms of the chunked Thomas solve that matter in fp64: the carry into a chunk is
+// e[c-1] + f[c-1] (e[c-2] + f[c-2] (...)) with |f| = product of L consecutive |h_j| < 1; the q-th term is below
+// fmax^(q-1) of the first.  Smallest K with fmax^K < 2^-73 (then every dropped term is below a quarter ulp of
+// the sum even if the e's differ by three orders of magnitude), at most nchunks - 1.
+static int carry_terms(const std::vector<dbec_host::zc>& f, int nchunks) {
+    double fmax = 0.0;
+    for (int c = 0; c < nchunks; ++c) fmax = std::max(fmax, std::abs(f[c]));
+    if (nchunks <= 1 || fmax == 0.0) return 1;
+    if (fmax >= 1.0) return nchunks - 1;
+    const int k = (int)std::ceil(-73.0 * std::log(2.0) / std::log(fmax));
+    return std::max(1, std::min(k, nchunks - 1));
 }
 
 // Reduction partials: one per block of the last Crank-Nicolson sweep (<= one per 256 points), ten per block
@@ -132,6 +149,24 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     CU(h, put(pb_re.data(), sizeof(double) * n, (const void**)&A.pb_re));
     CU(h, put(pfe_re.data(), sizeof(double) * 32, (const void**)&A.pfe_re));
     CU(h, put(pbs_re.data(), sizeof(double) * 32, (const void**)&A.pbs_re));
+    A.K8 = 0;
+    if (axis == 0 && n >= 16 && n % 8 == 0 && n / 8 <= 128) {
+        // the x axis again with chunks of 8 points (one 128-byte row of psi per lane, kernels_xwarp.cu)
+        std::vector<zc> h8, pf8, pb8, pfe8(128, zc(0, 0)), pbs8(128, zc(0, 0));
+        make_cn(n, 8, a, h8, pf8, pb8);
+        for (int c = 0; c < n / 8; ++c) { pfe8[c] = pf8[c * 8 + 7]; pbs8[c] = pb8[c * 8]; }
+        std::vector<double> pf8_re = re(pf8), pb8_re = re(pb8), pfe8_re = re(pfe8), pbs8_re = re(pbs8);
+        CU(h, put(pf8.data(), sizeof(zc) * n, (const void**)&A.pf8));
+        CU(h, put(pb8.data(), sizeof(zc) * n, (const void**)&A.pb8));
+        CU(h, put(pfe8.data(), sizeof(zc) * 128, (const void**)&A.pfe8));
+        CU(h, put(pbs8.data(), sizeof(zc) * 128, (const void**)&A.pbs8));
+        CU(h, put(pf8_re.data(), sizeof(double) * n, (const void**)&A.pf8_re));
+        CU(h, put(pb8_re.data(), sizeof(double) * n, (const void**)&A.pb8_re));
+        CU(h, put(pfe8_re.data(), sizeof(double) * 128, (const void**)&A.pfe8_re));
+        CU(h, put(pbs8_re.data(), sizeof(double) * 128, (const void**)&A.pbs8_re));
+        A.K8 = std::max(carry_terms(pfe8, n / 8), carry_terms(pbs8, n / 8));
+        CU(h, cudaStreamSynchronize(h->stream));          // the host vectors of this block go out of scope
+    }
     // the host vectors must outlive the asynchronous copies from pageable memory: those copies are
     // staged synchronously by the runtime, but be explicit
     CU(h, cudaStreamSynchronize(h->stream));
@@ -219,7 +254,8 @@ static int enqueue_step(dbec_handle h) {
     int rc = enqueue_dipolar_spectrum(h, 1);
     if (rc) return rc;
     h->rev_next = h->use_rev;                                       // inverse y pass went up: come back down
-    if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nplanes));
+    if (dbec_xwarp_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xwarp_nonlin(h));
+    else if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nplanes));
     else KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
     if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, launch_cn_pass(h, 0, 0));
     for (int ax = 1; ax <= last_axis; ++ax)
@@ -565,7 +601,8 @@ const char* dbec_pass_kernel(dbec_handle h, int slot) {
             return h->p.ndim == 3 ? (dbec_tma_supported(h, 1) ? "k_fft_tma" : "k_fft_strided") : "";
         case KS_FFT_LAST_FMI:
             return dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
-        case KS_IFFTX_NONLIN: return (h->fuse_cnx && dbec_xline_supported(h)) ? "k_xline_nonlin" : "k_ifftx_nonlin";
+        case KS_IFFTX_NONLIN: return dbec_xwarp_supported(h) ? "k_xwarp_nonlin"
+                                     : (h->fuse_cnx && dbec_xline_supported(h)) ? "k_xline_nonlin" : "k_ifftx_nonlin";
         case KS_CN_X: return h->fuse_cnx ? "" : "k_cn_x";
         case KS_CN_Y: return dbec_tma_supported(h, 1) ? "k_cn_tma" : "k_cn_strided";
         case KS_CN_Z: return h->p.ndim == 3 ? (dbec_tma_supported(h, 2) ? "k_cn_tma" : "k_cn_strided") : "";

@@ -17,7 +17,8 @@
 enum { POL_CN_LD = 0, POL_CN_ST, POL_NL_LD, POL_NL_ST, POL_NL_SPEC, POL_D_PSI, POL_D_SPEC, POL_FFT_LD, POL_FFT_ST, POL_COUNT };
 
 // Tensor maps of the handle (kernels_tma.cu): field x direction of the box rows.
-enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD_Y, TM_VDD_Z, TM_COUNT };
+// TM_PSI_XW: psi as [line][NX/8][8 complex] with the 128-byte swizzle (kernels_xwarp.cu).
+enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD_Y, TM_VDD_Z, TM_PSI_XW, TM_COUNT };
 
 // Device scalars every kernel reads (so that a captured CUDA graph never bakes them in), one block of
 // SC_COUNT doubles per batch member (dbec_create_batch; a plain handle has one member).
@@ -57,6 +58,11 @@ struct AxisTables {
     const cd* h;  const cd* pf;  const cd* pb;  const cd* pfe;  const cd* pbs;
     const double* h_re; const double* pf_re; const double* pb_re; const double* pfe_re; const double* pbs_re;
     cd kap;                 // (1 - 2a)/a
+    // the same tables for chunks of 8 points (kernels_xwarp.cu; built for the x axis only) and the number of
+    // carry terms that are above 2^-73 of the leading one (0: tables not built)
+    const cd* pf8; const cd* pb8; const cd* pfe8; const cd* pbs8;
+    const double* pf8_re; const double* pb8_re; const double* pfe8_re; const double* pbs8_re;
+    int K8;
 };
 
 struct dbec_handle_s {
@@ -128,3 +134,6 @@ int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nz
 int dbec_xline_supported(const dbec_handle_s* h);
 int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs);          // a3 (x) + a4 + a5
 int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance);   // a1 (x)
+// one warp per line pair (kernels_xwarp.cu): a3 (x) + a4 + a5 for lines of 128 / 256 points
+int dbec_xwarp_supported(const dbec_handle_s* h);
+int dbec_launch_xwarp_nonlin(dbec_handle_s* h);

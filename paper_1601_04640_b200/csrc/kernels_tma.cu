@@ -307,7 +307,8 @@ static EncodeTiledFn encode_fn() {
 }
 
 // A field of doubles [n2][n1][n0] (n0 fastest) and a box of (b0, b1, b2) elements.
-static int make_map(CUtensorMap* m, void* ptr, long long n0, long long n1, long long n2, int b0, int b1, int b2) {
+static int make_map(CUtensorMap* m, void* ptr, long long n0, long long n1, long long n2, int b0, int b1, int b2,
+                    bool swizzle128 = false) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return (int)cudaErrorNotSupported;
     cuuint64_t dims[3] = {(cuuint64_t)n0, (cuuint64_t)n1, (cuuint64_t)n2};
@@ -315,7 +316,8 @@ static int make_map(CUtensorMap* m, void* ptr, long long n0, long long n1, long 
     cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
     cuuint32_t es[3] = {1, 1, 1};
     CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, ptr, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
 }
 
@@ -335,6 +337,12 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
     rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Z], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, 1, bz);
     rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Y], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, by, 1);
     rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Z], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, 1, bz);
+    if (h->nx == 128 || h->nx == 256) {
+        // kernels_xwarp.cu: an x-line as NX/8 rows of 128 bytes (8 complex), a box = all rows of 2 (NX = 256) or
+        // 4 (NX = 128) lines, 16-byte units of a row rotated by the row index (SWIZZLE_128B)
+        const int lpt = h->nx == 256 ? 2 : 4;
+        rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_XW], h->psi, 16, h->nx / 8, (long long)h->ny * np, 16, h->nx / 8, lpt, true);
+    }
     return rc ? (int)cudaErrorInvalidValue : 0;
 }
 
