@@ -63,6 +63,42 @@ template <class CT, int L> DBEC_HD void cn_chunk_fix(cd (&u)[L], cd u_in, const 
     for (int i = 0; i < L; ++i) u[i] = cn_fma(pb[i], u_in, u[i]);
 }
 
+// The same three steps on the chunks of TWO lines at once (same chunk position, same tables): every table
+// entry is loaded once for both, and the two dependent chains interleave.
+template <class CT, int L> DBEC_HD void cn_chunk_forward2(cd (&u)[L], cd (&w)[L], cd lou, cd hiu, cd low, cd hiw, CT kap,
+                                                          const CT* __restrict__ h) {
+    cd pu = lou, pw = low, du = cmake(0.0, 0.0), dw = cmake(0.0, 0.0);
+#pragma unroll
+    for (int i = 0; i < L; ++i) {
+        const CT hh = h[i];
+        const cd cu = u[i], cw = w[i];
+        const cd nu = (i + 1 < L) ? u[i + 1] : hiu, nw = (i + 1 < L) ? w[i + 1] : hiw;
+        du = cn_mul(hh, cadd(cn_fma(kap, cu, cadd(pu, nu)), du));
+        dw = cn_mul(hh, cadd(cn_fma(kap, cw, cadd(pw, nw)), dw));
+        u[i] = du; w[i] = dw;
+        pu = cu; pw = cw;
+    }
+}
+template <class CT, int L> DBEC_HD void cn_chunk_backward2(cd (&u)[L], cd (&w)[L], cd du_in, cd dw_in, const CT* __restrict__ h,
+                                                           const CT* __restrict__ pf) {
+    cd tu = cmake(0.0, 0.0), tw = cmake(0.0, 0.0);
+#pragma unroll
+    for (int i = L - 1; i >= 0; --i) {
+        const CT hh = h[i], pp = pf[i];
+        tu = cn_fma(hh, tu, cn_fma(pp, du_in, u[i]));
+        tw = cn_fma(hh, tw, cn_fma(pp, dw_in, w[i]));
+        u[i] = tu; w[i] = tw;
+    }
+}
+template <class CT, int L> DBEC_HD void cn_chunk_fix2(cd (&u)[L], cd (&w)[L], cd uu_in, cd uw_in, const CT* __restrict__ pb) {
+#pragma unroll
+    for (int i = 0; i < L; ++i) {
+        const CT pp = pb[i];
+        u[i] = cn_fma(pp, uu_in, u[i]);
+        w[i] = cn_fma(pp, uw_in, w[i]);
+    }
+}
+
 // Carry into chunk c of the forward pass: D_in = d_{c*L-1}, from the zero-start chunk ends
 // e[i*es] = d~ at the last element of chunk i and pfend[i] = PF at that element.
 template <class CT> DBEC_HD cd cn_carry_forward(int c, const cd* e, int es, const CT* __restrict__ pfend) {

@@ -6,7 +6,7 @@
 // the group idles during the pair transforms, and psi crosses shared memory twice.  Here a warp owns its lines
 // from the moment they land to the moment they leave:
 //   * the pair's spectrum rows -> 8 values per lane -> 256-point inverse FFT inside the warp (fft_linev.cuh:
-//     V = 8, T = 32; every exchange is a __syncwarp) -> Phi_dd of both lines as real rows in shared memory;
+//     V = 8, T = 32; every exchange is a __syncwarp) -> Phi_dd of both lines, interleaved (a, b), in shared memory;
 //   * each lane then takes 8 CONSECUTIVE points of each line: calcnu on them in registers, and the very same
 //     registers are one chunk of the Crank-Nicolson solve (cn_chunk.cuh with L = 8).  Neighbour values, the
 //     zero-start chunk ends and the carries travel by warp shuffles: no shared-memory round trip, no barrier.
@@ -37,7 +37,11 @@ __host__ __device__ constexpr int w_nxhp(int n) { return ((n / 2 + 1) + DBEC_SPE
 // positions inside the padded rows: a lane's 8 values sit 80 (doubles) / 144 (complex table entries) bytes
 // after its neighbour's, so that the 128-bit loads of a quarter warp fall into eight different bank groups
 __host__ __device__ constexpr int padd(int k) { return k + 2 * (k >> 3); }          // doubles (Phi, trap)
-__host__ __device__ constexpr int padt(int k) { return k + (k >> 3); }              // table entries (h, PF, PB)
+__host__ __device__ constexpr int padt(int k) { return k + (k >> 3); }              // table entries (h, PF, PB), Phi pairs
+// elements of a pair's area: its two spectrum rows, later the FFT exchange, later the padded row of Phi pairs
+__host__ __device__ constexpr int w_pair_el(int fft, int nxhp, int ntab) {
+    return fft > 2 * nxhp ? (fft > ntab ? fft : ntab) : (2 * nxhp > ntab ? 2 * nxhp : ntab);
+}
 
 template <bool RT> struct CnTabW {
     typedef typename CnCoef<RT>::type CT;
@@ -64,18 +68,17 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
     constexpr int T = P::T, PAIRS = 32 / T, LPT = 2 * PAIRS;         // lines per tile (= per warp)
     constexpr int CPL = N / WL;                                      // chunks per line = lanes per line
     constexpr int NXHP = w_nxhp(N);
-    constexpr int PAIR_EL = (P::SMEM > 2 * NXHP) ? P::SMEM : 2 * NXHP;   // a pair's area: spectrum rows, FFT exchange, Phi
+    constexpr int NTAB = N + N / 8;                                  // padded table / padded Phi row (entries)
+    constexpr int PAIR_EL = w_pair_el(P::SMEM, NXHP, NTAB);          // a pair's area: spectrum rows, FFT exchange, Phi
     constexpr int NPD = N + N / 4;                                   // padded real row (doubles)
-    static_assert(2 * NPD * (int)sizeof(double) <= PAIR_EL * (int)sizeof(cd), "Phi rows must fit the pair's area");
     constexpr int PSI_BYTES = LPT * N * (int)sizeof(cd), SLOT_BYTES = PAIRS * PAIR_EL * (int)sizeof(cd);
-    constexpr int STAGE_BYTES = PSI_BYTES + SLOT_BYTES;
-    static_assert(STAGE_BYTES % 1024 == 0 && PSI_BYTES % 1024 == 0, "the swizzle pattern needs 1024-byte aligned psi tiles");
-    constexpr int NTAB = N + N / 8;                                  // padded table (entries)
+    static_assert(PSI_BYTES % 1024 == 0, "the swizzle pattern needs 1024-byte aligned psi tiles");
     constexpr int NT = (NW + 3) * 32;
     extern __shared__ __align__(1024) unsigned char smraw[];
     unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
-    cd* tw = (cd*)(base + (size_t)NST * STAGE_BYTES);            // twA [N] (stage-1 twiddles), twN [N]
-    CT* tab = (CT*)(tw + 2 * N);                                 // h, PF, PB (padded), PFE, PBS
+    unsigned char* slots = base + (size_t)NST * PSI_BYTES;       // psi tiles first (1024-byte aligned), then the pair areas
+    cd* tw = (cd*)(slots + (size_t)NST * SLOT_BYTES);            // twA [N] (stage-1 twiddles), tw2 [R3*R2] (stage 2)
+    CT* tab = (CT*)(tw + N + P::T);                              // h, PF, PB (padded), PFE, PBS
     double* vxs = (double*)(tab + 3 * NTAB + 2 * CPL);           // dt * trap along x (padded)
     uint64_t* bars = (uint64_t*)(vxs + NPD);
     uint64_t* full = bars; uint64_t* empty = bars + NST; uint64_t* done = bars + 2 * NST;
@@ -83,7 +86,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
     const int tid = threadIdx.x;
     for (int k = tid; k < N; k += NT) {
         tw[k] = twN_g[((k % T) * (k / T)) % N];                  // twA[k1*T + m] = W_N^{m k1}
-        tw[N + k] = twN_g[k];
+        if (k < T) tw[N + k] = twN_g[(P::V * (k / P::R2) * (k % P::R2)) % N];   // tw2[n3*R2 + k2] = W_N^{V n3 k2}
         vxs[padd(k)] = dt * vx_g[k];
         tab[padt(k)] = cn.h[k]; tab[NTAB + padt(k)] = cn.pf[k]; tab[2 * NTAB + padt(k)] = cn.pb[k];
     }
@@ -103,7 +106,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
     };
     const int warp = tid >> 5, lane = tid & 31;
     if (warp < NW) {
-        const cd* twA = tw; const cd* twN = tw + N;
+        const cd* twA = tw; const cd* tw2 = tw + N;
         const CT* th = tab; const CT* tpf = tab + NTAB; const CT* tpb = tab + 2 * NTAB;
         const CT* pfe = tab + 3 * NTAB; const CT* pbs = pfe + CPL;
         const CT kap = cn.kap;
@@ -128,8 +131,9 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
             }
             wait_issued(issued, i);
             mbar_wait(full + st, (i / NST) & 1);
-            cd* ps = (cd*)(base + (size_t)st * STAGE_BYTES);
-            cd* sa = (cd*)(base + (size_t)st * STAGE_BYTES + PSI_BYTES) + pr * PAIR_EL;
+            cd* ps = (cd*)(base + (size_t)st * PSI_BYTES);
+            cd* slot = (cd*)(slots + (size_t)st * SLOT_BYTES);
+            cd* sa = slot + pr * PAIR_EL;
             // ---- inverse transform of the pair's spectrum: v[j] = (Phi on line a, Phi on line b) at x = j*T + m
             {
                 const cd* sb = sa + NXHP;
@@ -146,11 +150,12 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
                     }
                 }
                 __syncwarp();                                        // the rows are in registers: reuse their area
-                fftv_line_warp<P, +1>(v, m, sa, twA, twN);
+                fftv_line_warp<P, +1>(v, m, sa, twA, tw2);
                 __syncwarp();
-                double* ph = (double*)sa;                            // Phi as two padded real rows
+                // (Phi on line a, Phi on line b) at x, one padded row of pairs: a lane's 8 consecutive x sit 144
+                // bytes after its neighbour's
 #pragma unroll
-                for (int j = 0; j < P::V; ++j) { ph[padd(j * T + m)] = v[j].x; ph[NPD + padd(j * T + m)] = v[j].y; }
+                for (int j = 0; j < P::V; ++j) sa[padt(j * T + m)] = v[j];
             }
             __syncwarp();
             // ---- calcnu on 8 consecutive points of two lines (registers u0, u1), then calclux on the same registers
@@ -161,21 +166,24 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
 #pragma unroll
             for (int k = 0; k < WL; ++k) { u0[k] = p0[k ^ sw]; u1[k] = p1[k ^ sw]; }
             {
-                const double* base_ph = (const double*)(base + (size_t)st * STAGE_BYTES + PSI_BYTES);
-                const double* ph0 = base_ph + (size_t)(l0 >> 1) * (PAIR_EL * 2) + (l0 & 1) * NPD + padd(c * WL);
-                const double* ph1 = base_ph + (size_t)(l1 >> 1) * (PAIR_EL * 2) + (l1 & 1) * NPD + padd(c * WL);
+                // N = 256: both lines belong to pair 0, line 0 takes Phi.x and line 1 Phi.y of the same entries;
+                // N = 128: slot s belongs to pair s, and `sub` says which component is this lane's line
+                const cd* ph0 = slot + (l0 >> 1) * PAIR_EL + padt(c * WL);
+                const cd* ph1 = slot + (l1 >> 1) * PAIR_EL + padt(c * WL);
                 const double* vxc = vxs + padd(c * WL);
 #pragma unroll
                 for (int half = 0; half < 2; ++half) {
 #pragma unroll
                     for (int k0 = 0; k0 < WL; k0 += NLW_C) {
                         cd* u = half ? u1 : u0;
-                        const double* ph = half ? ph1 : ph0;
+                        const cd* ph = half ? ph1 : ph0;
                         const double vr = half ? vr1 : vr0;
+                        const bool second = half ? (l1 & 1) : (l0 & 1);
                         double a[NLW_C];
 #pragma unroll
                         for (int kk = 0; kk < NLW_C; ++kk) {
-                            a[kk] = fma(dtD, ph[k0 + kk], vxc[k0 + kk] + vr);
+                            const cd f = ph[k0 + kk];
+                            a[kk] = fma(dtD, second ? f.y : f.x, vxc[k0 + kk] + vr);
                             a[kk] = fma(dtG, cnorm2(u[k0 + kk]), a[kk]);
                         }
 #pragma unroll
@@ -198,24 +206,21 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
             if (c == 0) { lo0 = zero; lo1 = zero; }
             if (c == CPL - 1) { hi0 = zero; hi1 = zero; }
             const CT* hc = th + padt(c * WL);
-            cn_chunk_forward<CT>(u0, lo0, hi0, kap, hc);
-            cn_chunk_forward<CT>(u1, lo1, hi1, kap, hc);
+            cn_chunk_forward2<CT>(u0, u1, lo0, hi0, lo1, hi1, kap, hc);
             cd d0 = zero, d1 = zero;
             for (int q = K; q >= 1; --q) {                           // D_in = e[c-1] + pfe[c-1] (e[c-2] + pfe[c-2] (...))
                 const cd e0 = shfl_up_cd(u0[WL - 1], q, CPL), e1 = shfl_up_cd(u1[WL - 1], q, CPL);
                 if (c - q >= 0) { const CT f = pfe[c - q]; d0 = cn_fma(f, d0, e0); d1 = cn_fma(f, d1, e1); }
             }
             const CT* pfc = tpf + padt(c * WL);
-            cn_chunk_backward<CT>(u0, d0, hc, pfc);
-            cn_chunk_backward<CT>(u1, d1, hc, pfc);
+            cn_chunk_backward2<CT>(u0, u1, d0, d1, hc, pfc);
             cd w0 = zero, w1 = zero;
             for (int q = K; q >= 1; --q) {                           // U_in = e[c+1] + pbs[c+1] (e[c+2] + ...)
                 const cd e0 = shfl_down_cd(u0[0], q, CPL), e1 = shfl_down_cd(u1[0], q, CPL);
                 if (c + q < CPL) { const CT f = pbs[c + q]; w0 = cn_fma(f, w0, e0); w1 = cn_fma(f, w1, e1); }
             }
             const CT* pbc = tpb + padt(c * WL);
-            cn_chunk_fix<CT>(u0, w0, pbc);
-            cn_chunk_fix<CT>(u1, w1, pbc);
+            cn_chunk_fix2<CT>(u0, u1, w0, w1, pbc);
 #pragma unroll
             for (int k = 0; k < WL; ++k) { p0[k ^ sw] = u0[k]; p1[k ^ sw] = u1[k]; }
             fence_proxy_async();
@@ -230,12 +235,11 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
             st_release_shared(issued, i + 1);
             mbar_expect_tx(full + st, PSI_BYTES + PAIRS * 2 * NXHP * (int)sizeof(cd));
             const long long tile = tile_of(i);
-            unsigned char* dst = base + (size_t)st * STAGE_BYTES;
-            tma_load_3d_hint(dst, &map_psi, 0, 0, (int)(tile * LPT), full + st, polp);
+            tma_load_3d_hint(base + (size_t)st * PSI_BYTES, &map_psi, 0, 0, (int)(tile * LPT), full + st, polp);
 #pragma unroll 1
             for (int pp = 0; pp < PAIRS; ++pp)
-                bulk_load_hint(dst + PSI_BYTES + (size_t)pp * PAIR_EL * sizeof(cd), spec + (tile * PAIRS + pp) * 2 * NXHP,
-                               2 * NXHP * (int)sizeof(cd), full + st, pol);
+                bulk_load_hint(slots + (size_t)st * SLOT_BYTES + (size_t)pp * PAIR_EL * sizeof(cd),
+                               spec + (tile * PAIRS + pp) * 2 * NXHP, 2 * NXHP * (int)sizeof(cd), full + st, pol);
         }
     } else if (tid == (NW + 1) * 32 || tid == (NW + 2) * 32) {
         // two storers (even / odd stages): while one sits in wait_group.read, the other drains the next stage
@@ -245,7 +249,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
             const int st = i % NST;
             if ((st & 1) != which) continue;
             mbar_wait(done + st, (i / NST) & 1);
-            tma_store_3d_hint(&map_psi, 0, 0, (int)(tile_of(i) * LPT), base + (size_t)st * STAGE_BYTES, polp);
+            tma_store_3d_hint(&map_psi, 0, 0, (int)(tile_of(i) * LPT), base + (size_t)st * PSI_BYTES, polp);
             bulk_commit();
             bulk_wait_read<0>();
             mbar_arrive(empty + st);
@@ -276,12 +280,12 @@ template <int N, bool RT, int NW, int NST> static int launch_xwarp(dbec_handle_s
     typedef typename CnCoef<RT>::type CT;
     typedef typename WPlan<N>::P P;
     constexpr int PAIRS = 32 / P::T, LPT = 2 * PAIRS, NXHP = w_nxhp(N), CPL = N / WL;
-    constexpr int PAIR_EL = (P::SMEM > 2 * NXHP) ? P::SMEM : 2 * NXHP;
+    constexpr int PAIR_EL = w_pair_el(P::SMEM, NXHP, N + N / 8);
     constexpr int STAGE = LPT * N * (int)sizeof(cd) + PAIRS * PAIR_EL * (int)sizeof(cd);
     if (h->nxhp != NXHP) return (int)cudaErrorInvalidValue;
     const int ntiles = (int)((long long)h->ny * h->nplanes / LPT);
     const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
-    const size_t sm = (size_t)NST * STAGE + 2 * N * sizeof(cd) + (3 * (N + N / 8) + 2 * CPL) * sizeof(CT) +
+    const size_t sm = (size_t)NST * STAGE + (N + P::T) * sizeof(cd) + (3 * (N + N / 8) + 2 * CPL) * sizeof(CT) +
                       (N + N / 4) * sizeof(double) + (3 * NST + 1) * sizeof(uint64_t);
     auto k = k_xwarp_nonlin<N, RT, NW, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
@@ -296,8 +300,8 @@ template <int N, bool RT, int NW, int NST> static int launch_xwarp(dbec_handle_s
 int dbec_launch_xwarp_nonlin(dbec_handle_s* h) {
     const bool rt = h->p.time_mode == 1;
     switch (h->nx) {
-        case 128: return rt ? launch_xwarp<128, true, 12, 14>(h) : launch_xwarp<128, false, 12, 14>(h);
-        case 256: return rt ? launch_xwarp<256, true, 12, 15>(h) : launch_xwarp<256, false, 12, 15>(h);
+        case 128: return rt ? launch_xwarp<128, true, 12, 15>(h) : launch_xwarp<128, false, 12, 15>(h);
+        case 256: return rt ? launch_xwarp<256, true, 12, 16>(h) : launch_xwarp<256, false, 12, 16>(h);
         default: return (int)cudaErrorInvalidValue;
     }
 }
