@@ -47,7 +47,8 @@ template <class P> DBEC_HD void fftv_x1_write(const cd (&v)[P::V], int m, cd* sm
     for (int k1 = 0; k1 < P::V; ++k1) sm[k1 * P::P1 + m] = v[k1];
 }
 
-// tw2[n3*R2 + k2] = exp(-2 pi i V n3 k2 / N): the R3*R2 stage-2 twiddles, contiguous
+// tw2[k2*R3 + n3] = exp(-2 pi i V n3 k2 / N): the R2*R3 stage-2 twiddles; the R3 entries the lanes of a warp read
+// in one instruction are neighbours (one wavefront)
 template <class P, int S> DBEC_HD void fftv_stage2(cd (&v)[P::V], int m, const cd* sm, const cd* __restrict__ tw2) {
     cd w[P::R2];
 #pragma unroll
@@ -63,7 +64,7 @@ template <class P, int S> DBEC_HD void fftv_stage2(cd (&v)[P::V], int m, const c
         } else {
             v[i * P::R2] = w[0];
 #pragma unroll
-            for (int k2 = 1; k2 < P::R2; ++k2) v[i * P::R2 + k2] = cmul(w[k2], tw_dir<S>(tw2[n3 * P::R2 + k2]));
+            for (int k2 = 1; k2 < P::R2; ++k2) v[i * P::R2 + k2] = cmul(w[k2], tw_dir<S>(tw2[k2 * P::R3 + n3]));
         }
     }
 }

@@ -27,7 +27,9 @@
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
 constexpr int WL = 8;              // Crank-Nicolson chunk: 8 points = one 128-byte row of psi
-constexpr int NLW_C = 4;           // calcnu: points evaluated side by side (same reason as NLU_C in kernels_xline.cu)
+// calcnu: points evaluated side by side (same reason as NLU_C in kernels_xline.cu); the library exp of imaginary
+// time needs more registers per evaluation than the branch-free sin/cos
+template <bool RT> struct NlwBatch { static constexpr int C = RT ? 4 : 2; };
 
 template <int N> struct WPlan;
 template <> struct WPlan<256> { typedef FftPlanV<8, 8, 4> P; };     // one pair per warp (32 lanes)
@@ -65,6 +67,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
                float pol_ld, float pol_st, float pol_spec) {
     typedef typename CnCoef<RT>::type CT;
     typedef typename WPlan<N>::P P;
+    constexpr int NLW_C = NlwBatch<RT>::C;
     constexpr int T = P::T, PAIRS = 32 / T, LPT = 2 * PAIRS;         // lines per tile (= per warp)
     constexpr int CPL = N / WL;                                      // chunks per line = lanes per line
     constexpr int NXHP = w_nxhp(N);
@@ -86,7 +89,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
     const int tid = threadIdx.x;
     for (int k = tid; k < N; k += NT) {
         tw[k] = twN_g[((k % T) * (k / T)) % N];                  // twA[k1*T + m] = W_N^{m k1}
-        if (k < T) tw[N + k] = twN_g[(P::V * (k / P::R2) * (k % P::R2)) % N];   // tw2[n3*R2 + k2] = W_N^{V n3 k2}
+        if (k < T) tw[N + k] = twN_g[(P::V * (k % P::R3) * (k / P::R3)) % N];   // tw2[k2*R3 + n3] = W_N^{V n3 k2}
         vxs[padd(k)] = dt * vx_g[k];
         tab[padt(k)] = cn.h[k]; tab[NTAB + padt(k)] = cn.pf[k]; tab[2 * NTAB + padt(k)] = cn.pb[k];
     }
