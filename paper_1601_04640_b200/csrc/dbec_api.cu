@@ -82,7 +82,7 @@ static void make_layout(const dbec_params* p, int nbatch, Layout* L) {
     size_t o = 0;
     L->psi = o;     o += up256(nb * P * sizeof(cd));
     L->spec = o;    o += up256(nb * SP * sizeof(cd));
-    L->vdd = o;     o += up256(SP * sizeof(double));
+    L->vdd = o;     o += up256((nz / 2 + 1) * (ny / 2 + 1) * nxhp * sizeof(double));      // folded (dbec_internal.hpp)
     L->phi = o;     o += up256(nb * P * sizeof(double));
     L->scal = o;    o += up256(nb * SC_COUNT * sizeof(double));
     L->partial = o; o += up256(npartial_of(P, nb) * sizeof(double));
@@ -322,6 +322,8 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     h->P = (long long)p->nx * p->ny * p->nz;
     h->SP = (long long)p->nz * p->ny * h->nxhp;
     h->dV = p->ndim == 3 ? p->dx * p->dy * p->dz : p->dx * p->dy;
+    h->nyf = p->ny / 2 + 1;
+    h->nzf = p->nz / 2 + 1;
     h->nb = nbatch;
     h->nplanes = p->nz * nbatch;
     char* w = (char*)dev_workspace;

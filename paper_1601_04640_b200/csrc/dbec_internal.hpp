@@ -18,7 +18,8 @@ enum { POL_CN_LD = 0, POL_CN_ST, POL_NL_LD, POL_NL_ST, POL_NL_SPEC, POL_D_PSI, P
 
 // Tensor maps of the handle (kernels_tma.cu): field x direction of the box rows.
 // TM_PSI_XW: psi as [line][NX/8][8 complex] with the 128-byte swizzle (kernels_xwarp.cu).
-enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD_Y, TM_VDD_Z, TM_PSI_XW, TM_COUNT };
+// TM_VDD: the folded V_dd table, boxes along the last axis of the grid.
+enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD, TM_PSI_XW, TM_COUNT };
 
 // Device scalars every kernel reads (so that a captured CUDA graph never bakes them in), one block of
 // SC_COUNT doubles per batch member (dbec_create_batch; a plain handle has one member).
@@ -82,7 +83,11 @@ struct dbec_handle_s {
     // device memory (all inside the caller's workspace)
     cd* psi;                        // [nz][ny][nx]
     cd* spec;                       // [nz][ny][nxhp] half spectrum of the density
-    double* vdd;                    // [nz][ny][nxhp] V_dd(k)/P
+    // V_dd(k)/P folded by its even symmetry in k_y and k_z (V_dd(k) depends on the squares of the wavenumbers and
+    // index m and N - m carry +-k: bitwise the same value): [nzf][nyf][nxhp], nyf = ny/2 + 1, nzf = nz/2 + 1 (1 in
+    // 2-D).  A quarter of the full table (17 MiB instead of 68 MiB at 256^3).
+    double* vdd;
+    int nyf, nzf;
     double* phi;                    // [nz][ny][nx] Phi_dd (observables / dbec_phi_dd only)
     double* scal;                   // nb x SC_COUNT doubles
     double* partial;                // reduction partials

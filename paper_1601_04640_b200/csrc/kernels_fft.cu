@@ -84,7 +84,7 @@ template <class P, int MODE, int TILES>
 __global__ void __launch_bounds__(P::T* DBEC_SPEC_COLS* TILES)
 k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twA,
               const cd* __restrict__ twN, long long line_stride, long long outer_stride, int ntiles_x,
-              long long ntiles, int vdd_outer_mod) {
+              long long ntiles, int n, int nxhp, int ny3, long long vdd_line_stride) {
     extern __shared__ cd smem[];
     pdl_launch_dependents(); pdl_wait();
     constexpr int T = P::T, C = DBEC_SPEC_COLS;
@@ -102,10 +102,17 @@ k_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* _
     for (int j = 0; j < 16; ++j) v[j] = g[(long long)(j * T + m) * line_stride];
     if (MODE == MODE_FWD || MODE == MODE_FMI) fft_line<P, -1, 1>(v, m, sm, C, twA, twN);
     if (MODE == MODE_FMI) {
-        // the V_dd table is shared by the members of a batch: its outer coordinate wraps
-        const double* w = vdd + (outer % vdd_outer_mod) * outer_stride + tx * C + col;
+        // the folded V_dd table (shared by the members of a batch): index r along the line -> min(r, n - r);
+        // 3-D (ny3 = NY, lines along z): the tile's columns are (k_y, k_x) flattened, k_y folds the same way
+        const long long cix = tx * C + col;
+        long long voff = cix;
+        if (ny3) { const int ky = (int)(cix / nxhp), kx = (int)(cix % nxhp); voff = (long long)(ky < ny3 - ky ? ky : ny3 - ky) * nxhp + kx; }
+        const double* w = vdd + voff;
 #pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = cmul(w[(long long)(j * T + m) * line_stride], v[j]);
+        for (int j = 0; j < 16; ++j) {
+            const int r = j * T + m;
+            v[j] = cmul(w[(long long)(r < n - r ? r : n - r) * vdd_line_stride], v[j]);
+        }
         if (T > 1) __syncthreads();
     }
     if (MODE == MODE_INV || MODE == MODE_FMI) fft_line<P, +1, 1>(v, m, sm, C, twA, twN);
@@ -214,14 +221,15 @@ __device__ __forceinline__ double wavenumber(int mi, int n, double d) {     // r
     return 6.283185307179586476925286766559 * (double)mt / ((double)n * d);
 }
 
-__global__ void k_build_vdd(double* __restrict__ vdd, int ndim, int plane, int nx, int ny, int nz, int nxhp, double dx,
-                            double dy, double dz, double d_perp, double cutoff, double invP) {
-    const long long total = (long long)nz * ny * nxhp;
+// Folded: rows m_y = 0..ny/2 and m_z = 0..nz/2 only (the table is even in both; dbec_internal.hpp).
+__global__ void k_build_vdd(double* __restrict__ vdd, int ndim, int plane, int nx, int ny, int nz, int nxhp, int nyf, int nzf,
+                            double dx, double dy, double dz, double d_perp, double cutoff, double invP) {
+    const long long total = (long long)nzf * nyf * nxhp;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
          i += (long long)gridDim.x * blockDim.x) {
         const int mx = (int)(i % nxhp);
-        const int my = (int)((i / nxhp) % ny);
-        const int mz = (int)(i / ((long long)nxhp * ny));
+        const int my = (int)((i / nxhp) % nyf);
+        const int mz = (int)(i / ((long long)nxhp * nyf));
         double v = 0.0;
         if (mx <= nx / 2) {
             const double kx = wavenumber(mx, nx, dx), ky = wavenumber(my, ny, dy);
@@ -302,20 +310,23 @@ template <int N, int MODE> static int launch_fft_strided(dbec_handle_s* h, int a
     constexpr int C = DBEC_SPEC_COLS;
     constexpr int TILES = (P::T * C >= 128) ? 1 : 128 / (P::T * C);
     long long line_stride, outer_stride, ntiles;
-    int ntx, vmod;
+    int ntx;
     if (axis == 1) {        // y lines: for each plane (z, member), columns = kx
         line_stride = h->nxhp; outer_stride = (long long)h->ny * h->nxhp; ntx = h->nxhp / C;
-        ntiles = (long long)ntx * h->nplanes; vmod = h->nz;
+        ntiles = (long long)ntx * h->nplanes;
     } else {                // z lines: columns = (ky, kx) flattened; outer = batch member
         line_stride = (long long)h->ny * h->nxhp; outer_stride = h->SP; ntx = (int)(line_stride / C);
-        ntiles = (long long)ntx * h->nb; vmod = 1;
+        ntiles = (long long)ntx * h->nb;
     }
+    // the multiply by V_dd rides on the last axis only: y in 2-D (table [nyf][nxhp]), z in 3-D ([nzf][nyf][nxhp])
+    const int ny3 = axis == 2 ? h->ny : 0;
+    const long long vls = axis == 2 ? (long long)h->nyf * h->nxhp : h->nxhp;
     const size_t sm = (size_t)TILES * P::SMEM * C * sizeof(cd);
     auto k = k_fft_strided<P, MODE, TILES>;
     int rc = set_smem(k, sm);
     if (rc) return rc;
     cudaError_t e = launch_pdl(k, dim3((unsigned)((ntiles + TILES - 1) / TILES)), dim3(P::T * C * TILES), sm, h->stream, h->use_pdl,
-                               h->spec, (const double*)h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles, vmod);
+                               h->spec, (const double*)h->vdd, h->ax[axis].twA, h->ax[axis].twN, line_stride, outer_stride, ntx, ntiles, N, h->nxhp, ny3, vls);
     h->launches++;
     return (int)e;
 }
@@ -371,7 +382,7 @@ int dbec_launch_phi_out(dbec_handle_s* h, double* phi) {
 }
 
 int dbec_launch_build_vdd(dbec_handle_s* h) {
-    k_build_vdd<<<h->num_sms * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->p.plane, h->nx, h->ny, h->nz, h->nxhp, h->p.dx, h->p.dy,
+    k_build_vdd<<<h->num_sms * 8, 256, 0, h->stream>>>(h->vdd, h->p.ndim, h->p.plane, h->nx, h->ny, h->nz, h->nxhp, h->nyf, h->nzf, h->p.dx, h->p.dy,
                                                  h->p.dz, h->p.d_perp, h->p.cutoff, 1.0 / (double)h->P);
     h->launches++;
     return (int)cudaGetLastError();

@@ -26,8 +26,10 @@ struct TileGeom {
     int box_rows;    // rows of one TMA box (<= 256)
     int nbox;        // boxes per tile (N / box_rows)
     int outer0;      // first outer coordinate (slab offset; axis 1 only)
-    int vmod;        // planes of the V_dd table (nz): the outer coordinate of its tile wraps, because a batch of
-                     // 2-D grids is a stack of planes that share one table
+    int vfold;       // fused z pass: NY (the tile's outer coordinate k_y folds to min(k_y, NY - k_y) in the V_dd table);
+                     // fused y pass of a 2-D grid: 0 (the table has one plane, shared by the members of a batch)
+    int vrows;       // rows of one V_dd box, boxes per tile
+    int vnbox;
     int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
     float pol_ld, pol_st;   // L2 eviction policy codes of the tile loads / stores (tma_pipe.cuh: l2_policy_code)
 };
@@ -60,7 +62,8 @@ __device__ __forceinline__ void tile_coords(const TileGeom& tg, int t, int b, in
 
 // Loader: stage i % NST receives tile blockIdx.x + i * gridDim.x.  `extra` (optional) is a second
 // tensor map whose box lands EXTRA_OFF bytes into the stage (the V_dd tile of the fused z pass).
-template <int NST, int STAGE_BYTES, int MAIN_BYTES, int EXTRA_BYTES>
+// EXTRA_TX: the bytes the V_dd boxes really carry (EXTRA_BYTES includes the padding between them)
+template <int NST, int STAGE_BYTES, int MAIN_BYTES, int EXTRA_BYTES, int EXTRA_TX = EXTRA_BYTES>
 __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
                                             const CUtensorMap* extra, const TileGeom& tg, int nmine) {
     const uint64_t pol = l2_policy_code(tg.pol_ld);
@@ -68,18 +71,27 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
         const int s = i % NST;
         if (i >= NST) mbar_wait(pb.empty + s, ((i / NST) - 1) & 1);
         st_release_shared(pb.issued, i + 1);
-        mbar_expect_tx(pb.full + s, MAIN_BYTES + EXTRA_BYTES);
+        mbar_expect_tx(pb.full + s, MAIN_BYTES + EXTRA_TX);
         const int t = blockIdx.x + i * gridDim.x;
         unsigned char* dst = stages + (size_t)s * STAGE_BYTES;
         for (int b = 0; b < tg.nbox; ++b) {
             int c0, c1, c2;
             tile_coords(tg, t, b, 2 * TCOLS, c0, c1, c2);
             tma_load_3d_hint(dst + (size_t)b * (MAIN_BYTES / tg.nbox), map, c0, c1, c2, pb.full + s, pol);
-            if (EXTRA_BYTES) {
-                tile_coords(tg, t, b, TCOLS, c0, c1, c2);
-                if (tg.axis == 1) c2 %= tg.vmod;
-                tma_load_3d_hint(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.nbox), extra, c0, c1, c2, pb.full + s,
-                                 l2_policy_evict_first());      // the V_dd table is read once per step
+        }
+        if (EXTRA_BYTES) {
+            // rows 0 .. N/2 of the folded V_dd table under this tile (table [nzf][nyf][nxhp]; 2-D: [1][nyf][nxhp]).
+            // Evict-first: measured at C4, keeping the 17 MiB table in L2 (evict-last) makes this pass no faster
+            // and costs the next one 3 us of the spectrum lines it would otherwise find there.
+            int c0, c1, c2;
+            tile_coords(tg, t, 0, TCOLS, c0, c1, c2);
+            const int o = tg.axis == 1 ? c2 : c1;
+            const uint64_t polv = l2_policy_evict_first();
+            for (int b = 0; b < tg.vnbox; ++b) {
+                if (tg.vfold) tma_load_3d_hint(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.vnbox), extra, c0,
+                                               o < tg.vfold - o ? o : tg.vfold - o, b * tg.vrows, pb.full + s, polv);
+                else tma_load_3d_hint(dst + MAIN_BYTES + (size_t)b * (EXTRA_BYTES / tg.vnbox), extra, c0, b * tg.vrows, 0,
+                                      pb.full + s, polv);
             }
         }
     }
@@ -237,13 +249,22 @@ __device__ __forceinline__ void fft_line_nb(cd (&v)[16], int m, cd* sm, const cd
     }
 }
 
+// Bytes of the V_dd part of a stage of the fused pass: rows 0 .. N/2 (N/2 + 1 rows of 8 doubles) in one box, or in
+// two boxes of N/4 + 1 rows when that exceeds the 256 rows a box may have; rounded up to the 128 bytes a TMA
+// destination must be aligned to.
+__host__ __device__ constexpr int fmi_vrows(int n) { return n / 2 + 1 <= 256 ? n / 2 + 1 : n / 4 + 1; }
+__host__ __device__ constexpr int fmi_vnbox(int n) { return n / 2 + 1 <= 256 ? 1 : 2; }
+__host__ __device__ constexpr int fmi_extra_bytes(int n) {
+    return fmi_vnbox(n) * ((fmi_vrows(n) * TCOLS * (int)sizeof(double) + 127) / 128 * 128);
+}
+
 template <class P, int MODE, int NG, int NST>
 __global__ void __launch_bounds__(NG* P::T* TCOLS + 96, 1)
 k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap map_vdd,
           const cd* twA, const cd* twN, TileGeom tg) {
     constexpr int T = P::T, N = P::N, GT = T * TCOLS;
     constexpr int MAIN_BYTES = N * TCOLS * (int)sizeof(cd);
-    constexpr int EXTRA_BYTES = (MODE == 2) ? N * TCOLS * (int)sizeof(double) : 0;
+    constexpr int EXTRA_BYTES = (MODE == 2) ? fmi_extra_bytes(N) : 0;     // rows 0 .. N/2 of the folded V_dd table
     constexpr int STAGE_BYTES = MAIN_BYTES + EXTRA_BYTES;
     extern __shared__ __align__(1024) unsigned char smraw[];
     unsigned char* base = smraw;     // (no integer round trip: the compiler must see shared-memory pointers)
@@ -269,7 +290,12 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
             if (MODE == 2) {
                 const double* w = (const double*)(base + (size_t)s * STAGE_BYTES + MAIN_BYTES) + col;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) v[j] = cmul(w[(j * T + m) * TCOLS], v[j]);
+                for (int j = 0; j < 16; ++j) {
+                    const int r = j * T + m, rf = r < N - r ? r : N - r;            // V_dd is even along the line
+                    // (two boxes: the second one starts after the first one's padding)
+                    constexpr int VR = fmi_vrows(N), PADR = fmi_extra_bytes(N) / fmi_vnbox(N) / (TCOLS * (int)sizeof(double)) - VR;
+                    v[j] = cmul(w[(rf + (fmi_vnbox(N) > 1 && rf >= VR ? PADR : 0)) * TCOLS], v[j]);
+                }
             }
             if (MODE == 2 && T > 1) named_bar_sync(1 + g, GT);      // stage-2/3 reads of the forward pass are over
             if (MODE == 1 || MODE == 2) fft_line_nb<P, +1>(v, m, sm, twA, twN, 1 + g, GT);
@@ -281,7 +307,8 @@ k_fft_tma(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUten
             if ((tid & 31) == 0) mbar_arrive(pb.done + s);
         }
     } else if (tid == NG * GT) {
-        pipe_loader<NST, STAGE_BYTES, MAIN_BYTES, EXTRA_BYTES>(pb, base, &map, &map_vdd, tg, nmine);
+        pipe_loader<NST, STAGE_BYTES, MAIN_BYTES, EXTRA_BYTES, (MODE == 2 ? fmi_vnbox(N) * fmi_vrows(N) * TCOLS * (int)sizeof(double) : 0)>(
+            pb, base, &map, &map_vdd, tg, nmine);
     } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
         pipe_storer<NST, STAGE_BYTES, MAIN_BYTES>(pb, base, &map, tg, nmine, (tid - NG * GT) / 32 - 1);
     }
@@ -335,8 +362,13 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
     rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Z], h->psi, 2LL * h->nx, h->ny, np, 2 * TCOLS, 1, bz);
     rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Y], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, by, 1);
     rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Z], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, 1, bz);
-    rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Y], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, by, 1);
-    rc |= make_map((CUtensorMap*)h->tmap[TM_VDD_Z], h->vdd, h->nxhp, h->ny, h->nz, TCOLS, 1, bz);
+    {   // the folded V_dd table, boxes along the last axis (rows 0 .. N/2; fmi_vrows)
+        const int nl = h->p.ndim == 3 ? h->nz : h->ny;
+        if (nl == 128 || nl == 256 || nl == 512) {
+            if (h->p.ndim == 3) rc |= make_map((CUtensorMap*)h->tmap[TM_VDD], h->vdd, h->nxhp, h->nyf, h->nzf, TCOLS, 1, fmi_vrows(nl));
+            else rc |= make_map((CUtensorMap*)h->tmap[TM_VDD], h->vdd, h->nxhp, h->nyf, 1, TCOLS, fmi_vrows(nl), 1);
+        }
+    }
     if (h->nx == 128 || h->nx == 256) {
         // kernels_xwarp.cu: an x-line as NX/8 rows of 128 bytes (8 complex), a box = all rows of 2 (NX = 256) or
         // 4 (NX = 128) lines, 16-byte units of a row rotated by the row index (SWIZZLE_128B)
@@ -356,7 +388,9 @@ static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int n
     tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
     tg.pol_st = h->pol[sp ? POL_FFT_ST : POL_CN_ST];
     tg.axis = axis;
-    tg.vmod = h->nz;
+    tg.vfold = axis == 2 ? h->ny : 0;
+    tg.vrows = fmi_vrows(axis == 1 ? h->ny : h->nz);
+    tg.vnbox = fmi_vnbox(axis == 1 ? h->ny : h->nz);
     tg.ntiles_x = row_elems / TCOLS;
     const int n = axis == 1 ? h->ny : h->nz;
     tg.box_rows = box_rows_of(n);
@@ -415,14 +449,14 @@ template <> struct PlanS<512> { typedef FftPlan<16, 2, false> P; };
 template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
     typedef typename PlanS<N>::P P;
     constexpr int GT = P::T * TCOLS;
-    constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? N * TCOLS * (int)sizeof(double) : 0);
+    constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? fmi_extra_bytes(N) : 0);
     const TileGeom tg = geom_of(h, axis, true, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
     const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 4) * sizeof(uint64_t) + 2 * N * sizeof(cd);
     auto k = k_fft_tma<P, MODE, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_SPEC_Y : TM_SPEC_Z];
-    const CUtensorMap* mv = (const CUtensorMap*)h->tmap[axis == 1 ? TM_VDD_Y : TM_VDD_Z];
+    const CUtensorMap* mv = (const CUtensorMap*)h->tmap[TM_VDD];
     CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, *map, *mv, h->ax[axis].twA, h->ax[axis].twN, tg));
     h->launches++;
     return (int)cudaGetLastError();
@@ -430,8 +464,8 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
 
 template <int MODE> static int launch_fft_tma_n(dbec_handle_s* h, int axis, int z0, int nzs) {
     switch (h->ax[axis].n) {
-        case 128: return launch_fft_tma<128, MODE, 4, (MODE == 2 ? 8 : 12)>(h, axis, z0, nzs);
-        case 256: return launch_fft_tma<256, MODE, 2, (MODE == 2 ? 4 : 6)>(h, axis, z0, nzs);
+        case 128: return launch_fft_tma<128, MODE, 4, (MODE == 2 ? 10 : 12)>(h, axis, z0, nzs);
+        case 256: return launch_fft_tma<256, MODE, 2, (MODE == 2 ? 5 : 6)>(h, axis, z0, nzs);
         case 512: return launch_fft_tma<512, MODE, 1, (MODE == 2 ? 2 : 3)>(h, axis, z0, nzs);
         default: return (int)cudaErrorInvalidValue;
     }

@@ -37,10 +37,10 @@ def test_workspace_bytes_validation_is_host_only(gp):
     n = C.c_size_t()
     ok = gp.params(3, 256, 256, 256, .1, .1, .1, .005, 1, 1.2, .8, 200, 150, 1)
     assert L.dbec_workspace_bytes(C.byref(ok), C.byref(n)) == gp.DBEC_OK
-    # psi + half spectrum + V_dd table + phi
-    P, SP = 256 ** 3, 256 * 256 * 136
-    assert n.value >= 16 * P + 16 * SP + 8 * SP + 8 * P
-    assert n.value < 16 * P + 16 * SP + 8 * SP + 8 * P + (4 << 20)
+    # psi + half spectrum + V_dd table (folded by its even symmetry in k_y, k_z: 129 x 129 rows) + phi
+    P, SP, VP = 256 ** 3, 256 * 256 * 136, 129 * 129 * 136
+    assert n.value >= 16 * P + 16 * SP + 8 * VP + 8 * P
+    assert n.value < 16 * P + 16 * SP + 8 * VP + 8 * P + (4 << 20)
     xz = gp.params(2, 32, 32, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=1)
     assert L.dbec_workspace_bytes(C.byref(xz), C.byref(n)) == gp.DBEC_OK
     assert L.dbec_workspace_bytes(None, C.byref(n)) == gp.DBEC_EINVAL
