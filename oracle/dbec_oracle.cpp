@@ -12,8 +12,10 @@
 // What each function follows:
 //   * oracle_fft_*            PAPER.md:63 "Fourier transformation to momentum space" — the DFT by
 //                             its definition (S7, S8), evaluated by a textbook iterative radix-2
-//                             FFT whose twiddles come from cos/sin of the exact angle; a separate
-//                             O(N^2) sum (oracle_dft_naive_*) pins it.
+//                             FFT whose twiddles come from cos/sin of the exact angle (powers of two)
+//                             or by a textbook recursive Cooley-Tukey over the prime factors (any other
+//                             length); a separate O(N^2) sum (oracle_dft_naive_*)
+//                             pins both.
 //   * oracle_vdd3d / _vdd2d   PAPER.md:63, :75 (`potdd`) under readings S3, S4, S5, S6, S21; _vdd2d_xz:
 //                             the in-plane-dipole kernel of the 2dXZ programs, reading S25.
 //   * oracle_phi_dd           PAPER.md:63, :71 (`calcpsidd2`): n -> DFT -> x V_dd -> inverse DFT.
@@ -133,6 +135,44 @@ static void fft_radix2_line(cplx* a, int n, const cplx* tw) {
 
 static bool is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 
+// Textbook recursive Cooley-Tukey for ANY length (the paper's grids are mostly not
+// powers of two): n = p m with p the smallest prime factor of n,
+//   X[k + q m] = sum_{r < p} W_n^{r (k + q m)} Y_r[k],   Y_r = DFT_m of the samples r, r + p, r + 2p, ...
+// and a prime length straight from the definition.  root[j] = exp(sign 2 pi i j / nroot), nroot a multiple of n,
+// each entry from cos/sin of its own angle.  `in` is read with the given stride, `out` is contiguous.
+static void fft_any_rec(const cplx* in, long long stride, cplx* out, int n, const cplx* root, int nroot, cplx* work) {
+    if (n == 1) { out[0] = in[0]; return; }
+    int p = n;
+    for (int f = 2; (long long)f * f <= n; ++f) if (n % f == 0) { p = f; break; }
+    const int step = nroot / n;                    // W_n^j = root[j * step]
+    if (p == n) {                                  // prime: the definition
+        for (int k = 0; k < n; ++k) {
+            cplx acc(0.0, 0.0);
+            for (int j = 0; j < n; ++j) acc += in[j * stride] * root[(((long long)j * k) % n) * step];
+            out[k] = acc;
+        }
+        return;
+    }
+    const int m = n / p;
+    // Y_r into work[r*m .. r*m + m), recursion scratch behind it
+    for (int r = 0; r < p; ++r) fft_any_rec(in + r * stride, stride * p, work + (long long)r * m, m, root, nroot, work + n);
+    for (int k = 0; k < m; ++k)
+        for (int q = 0; q < p; ++q) {
+            cplx acc(0.0, 0.0);
+            for (int r = 0; r < p; ++r) acc += work[(long long)r * m + k] * root[(((long long)r * (k + q * m)) % n) * step];
+            out[k + q * m] = acc;
+        }
+}
+
+static std::vector<cplx> make_roots(int n, int sign) {
+    std::vector<cplx> root(n);
+    for (int j = 0; j < n; ++j) {
+        double ang = sign * 2.0 * PI * (double)j / (double)n;
+        root[j] = cplx(std::cos(ang), std::sin(ang));
+    }
+    return root;
+}
+
 static std::vector<cplx> make_twiddles(int n, int sign) {
     std::vector<cplx> tw(n / 2 > 0 ? n / 2 : 1);
     for (int k = 0; k < n / 2; ++k) {
@@ -147,16 +187,17 @@ static std::vector<cplx> make_twiddles(int n, int sign) {
 static int transform_axis(cplx* a, int nx, int ny, int nz, int axis, int sign, int naive) {
     int n = axis == 0 ? nx : axis == 1 ? ny : nz;
     if (n == 1) return 0;
-    if (!naive && !is_pow2(n)) return -1;
+    const bool mixed = !naive && !is_pow2(n);      // lengths with other factors: fft_any_rec
     long long stride = axis == 0 ? 1 : axis == 1 ? nx : (long long)nx * ny;
     int n1 = axis == 0 ? ny : nx;             // inner count of lines
     int n2 = axis == 2 ? ny : nz;             // outer count of lines
     long long s1 = axis == 0 ? nx : 1;        // stride between lines (inner)
     long long s2 = axis == 2 ? nx : (long long)nx * ny; // stride between lines (outer)
     std::vector<cplx> tw = make_twiddles(n, sign);
+    std::vector<cplx> root = mixed ? make_roots(n, sign) : std::vector<cplx>();
 #pragma omp parallel
     {
-        std::vector<cplx> buf(n), out(n);
+        std::vector<cplx> buf(n), out(n), work(mixed ? 2 * (size_t)n + 64 : 1);
 #pragma omp for collapse(2) schedule(static)
         for (int o = 0; o < n2; ++o) {
             for (int i = 0; i < n1; ++i) {
@@ -164,6 +205,9 @@ static int transform_axis(cplx* a, int nx, int ny, int nz, int axis, int sign, i
                 for (int j = 0; j < n; ++j) buf[j] = base[j * stride];
                 if (naive) {
                     dft_naive_line(buf.data(), out.data(), n, sign);
+                    for (int j = 0; j < n; ++j) base[j * stride] = out[j];
+                } else if (mixed) {
+                    fft_any_rec(buf.data(), 1, out.data(), n, root.data(), n, work.data());
                     for (int j = 0; j < n; ++j) base[j * stride] = out[j];
                 } else {
                     fft_radix2_line(buf.data(), n, tw.data());
@@ -249,7 +293,6 @@ static int check_params(const oracle_params* p) {
     if (p->nx < 2 || p->ny < 2 || p->nz < 1) return -1;
     if (p->ndim == 2 && p->nz != 1) return -1;
     if (p->ndim == 3 && p->nz < 2) return -1;
-    if (!is_pow2(p->nx) || !is_pow2(p->ny) || !is_pow2(p->nz)) return -2;
     if (!(p->dx > 0) || !(p->dy > 0) || !(p->dt > 0)) return -1;
     if (p->ndim == 3 && !(p->dz > 0)) return -1;
     if (p->time_mode != 0 && p->time_mode != 1) return -1;

@@ -711,3 +711,40 @@ def test_integrated_densities_closed_form_and_numpy(ob):
         o3.density_1d(2)
     with pytest.raises(RuntimeError):
         o3.density_2d(2)
+
+
+# ------------------------------------------------------------------ f2: lengths that are not powers of two
+@pytest.mark.parametrize("shape", [(1, 1, 6), (1, 1, 7), (1, 1, 15), (1, 1, 21), (1, 1, 35), (1, 1, 49), (1, 1, 50), (1, 1, 96),
+                                   (1, 1, 210), (1, 1, 97), (3, 5, 7), (6, 10, 12), (12, 20, 48)])
+def test_fft_any_length_matches_definition_and_library(ob, shape):
+    rng = np.random.default_rng(sum(shape))
+    a = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    out = ob.fft(a, -1)
+    assert np.max(np.abs(out - scipy.fft.fftn(a))) / np.max(np.abs(out)) < 2e-14
+    assert np.max(np.abs(ob.fft(a, +1) - scipy.fft.ifftn(a) * a.size)) / np.max(np.abs(out)) < 2e-14
+    if a.size <= 5000:                                            # the O(N^2) definition (long double accumulation)
+        assert np.max(np.abs(out - ob.fft(a, -1, naive=True))) / np.max(np.abs(out)) < 2e-14
+    back = ob.fft(out, +1) / a.size
+    assert np.max(np.abs(back - a)) < 1e-13
+
+
+@pytest.mark.parametrize("mode", [IMAG, REAL])
+def test_full_step_on_a_non_power_of_two_grid_against_numpy(ob, mode):
+    w = Workload("t", 3, 12, 10, 6, 0.4, 0.3, 0.8, 0.01, 1.0, 1.2, 0.8, 50.0, 40.0, 50.0, 45.0, mode, 1, 4, 1)
+    p = ob.params_of(w)
+    o = ob.Oracle(p)
+    psi = random_psi(w, 21) if mode == REAL else initial_psi(w)
+    o.set_psi(psi)
+    o.set_coupling(w.G_run, w.D_run)
+    ref = psi
+    for _ in range(2):
+        ref = _numpy_step(w, ref, w.G_run, w.D_run, _numpy_vdd(w))
+    o.step(2)
+    assert np.max(np.abs(o.get_psi() - ref)) / np.max(np.abs(ref)) < 1e-13
+    w2 = Workload("t", 2, 50, 14, 1, 0.2, 0.3, 1.0, 0.004, 1.0, 1.5, 0.0, 20.0, 15.0, 25.0, 15.0, mode, 1, 2, 1, plane=1)
+    o2 = ob.Oracle(ob.params_of(w2))
+    psi2 = random_psi(w2, 5)
+    o2.set_psi(psi2)
+    o2.set_coupling(w2.G_run, w2.D_run)
+    o2.step(1)
+    assert np.max(np.abs(o2.get_psi() - _numpy_step(w2, psi2, w2.G_run, w2.D_run, _numpy_vdd(w2)))) < 1e-13
