@@ -15,7 +15,13 @@
 #define DBEC_VERSION 200
 #define DBEC_MAX_BATCH 65536
 
-static bool fft_len_ok(int n) { return n == 16 || n == 32 || n == 64 || n == 128 || n == 256 || n == 512; }
+// Powers of two 16..512 run in the register-resident kernels, every other length 4..1024 with prime factors
+// 2, 3, 5, 7 only in the run-time-length kernels (kernels_gen.cu).
+static bool len_pow2_fast(int n) { return n == 16 || n == 32 || n == 64 || n == 128 || n == 256 || n == 512; }
+static bool fft_len_ok(int n) {
+    int fac[12];
+    return n >= 4 && n <= DBEC_MAX_N && dbec_gen_factor(n, fac) > 0;
+}
 
 static int check_params(const dbec_params* p) {
     if (!p) return DBEC_EINVAL;
@@ -30,24 +36,27 @@ static int check_params(const dbec_params* p) {
     if (p->ndim == 2 && p->nz != 1) return DBEC_EINVAL;
     if (!fft_len_ok(p->nx) || !fft_len_ok(p->ny)) return DBEC_ESIZE;
     if (p->ndim == 3 && !fft_len_ok(p->nz)) return DBEC_ESIZE;
+    // two real x-lines ride one complex transform: the lines pair up, and NX/2 is the Nyquist index
+    if (p->nx % 2 || ((long long)p->ny * p->nz) % 2) return DBEC_ESIZE;
     return DBEC_OK;
 }
 
 // ---- workspace layout: one pass computes the offsets, used by both sizing and create ----
 struct Layout {
     size_t psi, spec, vdd, phi, scal, partial, ticket, obs, tables, total;
-    size_t tab_bytes;
+    size_t tab_bytes, npartial;
 };
 static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-static size_t axis_table_bytes(int n) {
+static size_t axis_table_bytes(int n_) {
+    const int n = (n_ + 15) / 16 * 16;          // tables are zero-padded to whole Crank-Nicolson chunks
     // twA, twN (cd n each); vtrap, x2 (double n each); h, pf, pb (cd n each) + pfe, pbs (cd 32 each);
     // the same five as doubles; pf, pb for chunks of 8 (cd n each) + their pfe, pbs (cd 128 each), and as doubles
     size_t b = 0;
     b += up256(sizeof(cd) * n) * 2;
     b += up256(sizeof(double) * n) * 2;
-    b += up256(sizeof(cd) * n) * 3 + up256(sizeof(cd) * 32) * 2;
-    b += up256(sizeof(double) * n) * 3 + up256(sizeof(double) * 32) * 2;
+    b += up256(sizeof(cd) * n) * 3 + up256(sizeof(cd) * 64) * 2;
+    b += up256(sizeof(double) * n) * 3 + up256(sizeof(double) * 64) * 2;
     b += up256(sizeof(cd) * n) * 2 + up256(sizeof(cd) * 128) * 2;
     b += up256(sizeof(double) * n) * 2 + up256(sizeof(double) * 128) * 2;
     return b;
@@ -68,9 +77,11 @@ static int carry_terms(const std::vector<dbec_host::zc>& f, int nchunks) {
 
 // Reduction partials: one per block of the last Crank-Nicolson sweep (<= one per 256 points), ten per block
 // of the observables pass.
-static size_t npartial_of(size_t P, size_t nb) {
-    size_t n = 32768, a = nb * P / 256 + nb, b = nb * 10 * 8;
+static size_t npartial_of(size_t P, size_t nb, size_t last_sweep_columns = 0) {
+    // last_sweep_columns: lines of the last sweep per member when it runs in kernels_gen.cu (one block per 8)
+    size_t n = 32768, a = nb * P / 256 + nb, b = nb * 10 * 8, c = nb * (last_sweep_columns / 8 + 1);
     if (a > n) n = a;
+    if (c > n) n = c;
     if (b > n) n = b;
     return n;
 }
@@ -85,7 +96,8 @@ static void make_layout(const dbec_params* p, int nbatch, Layout* L) {
     L->vdd = o;     o += up256((nz / 2 + 1) * (ny / 2 + 1) * nxhp * sizeof(double));      // folded (dbec_internal.hpp)
     L->phi = o;     o += up256(nb * P * sizeof(double));
     L->scal = o;    o += up256(nb * SC_COUNT * sizeof(double));
-    L->partial = o; o += up256(npartial_of(P, nb) * sizeof(double));
+    L->npartial = npartial_of(P, nb, p->ndim == 3 ? nx * ny : nx);
+    L->partial = o; o += up256(L->npartial * sizeof(double));
     L->ticket = o;  o += 256;
     L->obs = o;     o += up256(nb * 16 * sizeof(double));
     L->tables = o;
@@ -110,8 +122,8 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     A.n = n;
     std::vector<zc> twN, twA, hh, pf, pb;
     std::vector<double> vtrap(n), x2(n);
-    if (n >= 16) { make_twN(n, twN); make_twA(n, twN, twA); }
-    else { twN.assign(n, zc(1.0, 0.0)); twA = twN; }
+    if (n >= 2) make_twN(n, twN); else twN.assign(1, zc(1.0, 0.0));
+    if (len_pow2_fast(n)) make_twA(n, twN, twA); else twA = twN;
     for (int i = 0; i < n; ++i) {
         const double x = (double)(i - n / 2) * d;           // reading S17
         x2[i] = (n > 1) ? x * x : 0.0;
@@ -119,10 +131,13 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     }
     const double ar = h->p.dt / (4.0 * d * d);              // a = c dt / (4 h^2), c = 1 or i
     const zc a = h->p.time_mode == 0 ? zc(ar, 0.0) : zc(0.0, ar);
-    if (n >= 16) make_cn(n, CN_L, a, hh, pf, pb);
-    else { hh.assign(n, zc(0, 0)); pf = hh; pb = hh; }
-    std::vector<zc> pfe(32, zc(0, 0)), pbs(32, zc(0, 0));
-    for (int c = 0; c < n / CN_L; ++c) { pfe[c] = pf[c * CN_L + CN_L - 1]; pbs[c] = pb[c * CN_L]; }
+    // any n >= 3; padded with zeros to whole chunks of CN_L points (kernels_gen.cu reads whole chunks: a padded
+    // point has h = 0, solves to 0 and feeds nothing back)
+    const int npad = (n + CN_L - 1) / CN_L * CN_L;
+    if (n >= 3) make_cn(n, CN_L, a, hh, pf, pb);
+    hh.resize(npad, zc(0, 0)); pf.resize(npad, zc(0, 0)); pb.resize(npad, zc(0, 0));
+    std::vector<zc> pfe(64, zc(0, 0)), pbs(64, zc(0, 0));
+    for (int c = 0; c < npad / CN_L; ++c) { pfe[c] = pf[c * CN_L + CN_L - 1]; pbs[c] = pb[c * CN_L]; }
     const zc kap = (1.0 - 2.0 * a) / a;
     A.kap = cmake(kap.real(), kap.imag());
 
@@ -139,16 +154,16 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     CU(h, put(twN.data(), sizeof(zc) * n, (const void**)&A.twN));
     CU(h, put(vtrap.data(), sizeof(double) * n, (const void**)&A.vtrap));
     CU(h, put(x2.data(), sizeof(double) * n, (const void**)&A.x2));
-    CU(h, put(hh.data(), sizeof(zc) * n, (const void**)&A.h));
-    CU(h, put(pf.data(), sizeof(zc) * n, (const void**)&A.pf));
-    CU(h, put(pb.data(), sizeof(zc) * n, (const void**)&A.pb));
-    CU(h, put(pfe.data(), sizeof(zc) * 32, (const void**)&A.pfe));
-    CU(h, put(pbs.data(), sizeof(zc) * 32, (const void**)&A.pbs));
-    CU(h, put(h_re.data(), sizeof(double) * n, (const void**)&A.h_re));
-    CU(h, put(pf_re.data(), sizeof(double) * n, (const void**)&A.pf_re));
-    CU(h, put(pb_re.data(), sizeof(double) * n, (const void**)&A.pb_re));
-    CU(h, put(pfe_re.data(), sizeof(double) * 32, (const void**)&A.pfe_re));
-    CU(h, put(pbs_re.data(), sizeof(double) * 32, (const void**)&A.pbs_re));
+    CU(h, put(hh.data(), sizeof(zc) * npad, (const void**)&A.h));
+    CU(h, put(pf.data(), sizeof(zc) * npad, (const void**)&A.pf));
+    CU(h, put(pb.data(), sizeof(zc) * npad, (const void**)&A.pb));
+    CU(h, put(pfe.data(), sizeof(zc) * 64, (const void**)&A.pfe));
+    CU(h, put(pbs.data(), sizeof(zc) * 64, (const void**)&A.pbs));
+    CU(h, put(h_re.data(), sizeof(double) * npad, (const void**)&A.h_re));
+    CU(h, put(pf_re.data(), sizeof(double) * npad, (const void**)&A.pf_re));
+    CU(h, put(pb_re.data(), sizeof(double) * npad, (const void**)&A.pb_re));
+    CU(h, put(pfe_re.data(), sizeof(double) * 64, (const void**)&A.pfe_re));
+    CU(h, put(pbs_re.data(), sizeof(double) * 64, (const void**)&A.pbs_re));
     A.K8 = 0;
     if (axis == 0 && n >= 16 && n % 8 == 0 && n / 8 <= 128) {
         // the x axis again with chunks of 8 points (one 128-byte row of psi per lane, kernels_xwarp.cu)
@@ -215,10 +230,12 @@ static const char* const kernel_names[DBEC_MAX_KERNELS] = {
 // previous pass has just left (dirty) in the 126 MB L2.
 static int launch_fft_pass(dbec_handle h, int axis, int mode, int rev = 0) {
     h->rev_next = rev && h->use_rev;
+    if (h->gen[axis]) return dbec_launch_gen_fft(h, axis, mode);
     return dbec_tma_supported(h, axis) ? dbec_launch_fft_tma(h, axis, mode, 0, h->nplanes) : dbec_launch_fft_strided(h, axis, mode);
 }
 static int launch_cn_pass(dbec_handle h, int axis, int with_norm, int rev = 0) {
     h->rev_next = rev && h->use_rev;
+    if (h->gen[axis]) return dbec_launch_gen_cn(h, axis, with_norm);
     if (axis > 0 && dbec_tma_supported(h, axis)) {
         // a batch: the tiles of one CTA of the persistent sweep span several members, so calcnorm takes a
         // pass of its own (the fields of a batch are small: it runs out of L2)
@@ -235,7 +252,8 @@ static int launch_cn_pass(dbec_handle h, int axis, int with_norm, int rev = 0) {
 // advance: 1 inside a step (the density pass also moves the NSTP ramp on, reading S26).
 static int enqueue_dipolar_spectrum(dbec_handle h, int advance) {
     h->rev_next = 0;
-    if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nplanes, advance));
+    if (h->gen[0]) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_gen_density_fftx(h, advance));
+    else if (dbec_xline_supported(h)) KLAUNCH(h, KS_DENS_FFTX, dbec_launch_xline_density(h, 0, h->nplanes, advance));
     else KLAUNCH(h, KS_DENS_FFTX, dbec_launch_density_fftx(h, advance));
     if (h->p.ndim == 3) {
         KLAUNCH(h, KS_FFT_Y_FWD, launch_fft_pass(h, 1, 0, 1));      // density pass went up in z: come back down
@@ -254,7 +272,8 @@ static int enqueue_step(dbec_handle h) {
     int rc = enqueue_dipolar_spectrum(h, 1);
     if (rc) return rc;
     h->rev_next = h->use_rev;                                       // inverse y pass went up: come back down
-    if (dbec_xwarp_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xwarp_nonlin(h));
+    if (h->gen[0]) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_gen_nonlinear(h));
+    else if (dbec_xwarp_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xwarp_nonlin(h));
     else if (h->fuse_cnx && dbec_xline_supported(h)) KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_xline_nonlin(h, 0, h->nplanes));
     else KLAUNCH(h, KS_IFFTX_NONLIN, dbec_launch_nonlinear(h, h->fuse_cnx));
     if (!h->fuse_cnx) KLAUNCH(h, KS_CN_X, launch_cn_pass(h, 0, 0));
@@ -271,7 +290,7 @@ const char* dbec_strerror(int code) {
     switch (code) {
         case DBEC_OK: return "ok";
         case DBEC_EINVAL: return "invalid argument";
-        case DBEC_ESIZE: return "unsupported grid length (powers of two 16..512 only)";
+        case DBEC_ESIZE: return "unsupported grid length (4..1024 with prime factors 2, 3, 5, 7; NX and NY*NZ even)";
         case DBEC_EWORKSPACE: return "workspace missing, misaligned or too small";
         case DBEC_ECUDA: return "CUDA error (see dbec_last_cuda_error)";
         case DBEC_ENODEVICE: return "no sm_100 CUDA device";
@@ -335,7 +354,7 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     h->partial = (double*)(w + L.partial);
     h->ticket = (unsigned int*)(w + L.ticket);
     h->obs_dev = (double*)(w + L.obs);
-    h->npartial = (int)npartial_of((size_t)h->P, (size_t)nbatch);
+    h->npartial = (int)L.npartial;
     // the only two switches (both exercised by tests/test_gpu_parity.py): the CUDA graph of a step and the
     // x sweep fused into the nonlinear kernel
     const char* fe = getenv("DBEC_FUSE_CNX");
@@ -363,6 +382,11 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     const double om[3] = {p->nu, p->lambda, p->kappa};
     const double dd[3] = {p->dx, p->dy, p->ndim == 3 ? p->dz : 1.0};
     const int nn[3] = {p->nx, p->ny, p->nz};
+    for (int ax = 0; ax < 3; ++ax) {
+        h->gen[ax] = nn[ax] > 1 && !len_pow2_fast(nn[ax]);
+        h->gnfac[ax] = h->gen[ax] ? dbec_gen_factor(nn[ax], h->gfac[ax]) : 0;
+    }
+    if (h->gen[0]) h->fuse_cnx = 0;               // the run-time-length nonlinear kernel carries no x sweep
     for (int ax = 0; ax < 3; ++ax) {
         size_t used = 0;
         rc = upload_axis(h, ax, nn[ax], dd[ax], (p->ndim == 2 && ax == 2) ? 0.0 : om[ax], t, &used);
@@ -486,7 +510,7 @@ int dbec_step(dbec_handle h, int nsteps) {
 int dbec_phi_dd(dbec_handle h, void* phi_f64_dev) {
     if (!h || !phi_f64_dev) return DBEC_EINVAL;
     { int rc = enqueue_dipolar_spectrum(h, 0); if (rc) return rc; }
-    LAUNCH(h, dbec_launch_phi_out(h, (double*)phi_f64_dev));
+    LAUNCH(h, h->gen[0] ? dbec_launch_gen_phi_out(h, (double*)phi_f64_dev) : dbec_launch_phi_out(h, (double*)phi_f64_dev));
     return DBEC_OK;
 }
 
@@ -502,7 +526,7 @@ int dbec_nonlinear(dbec_handle h) {
     // last sweep rewrites it): bring the stored field to s = 1 first, or every later consumer applies s again
     LAUNCH(h, dbec_launch_apply_scale(h));
     { int rc = enqueue_dipolar_spectrum(h, 0); if (rc) return rc; }
-    LAUNCH(h, dbec_launch_nonlinear(h, 0));
+    LAUNCH(h, h->gen[0] ? dbec_launch_gen_nonlinear(h) : dbec_launch_nonlinear(h, 0));
     return DBEC_OK;
 }
 
@@ -518,7 +542,7 @@ int dbec_normalize(dbec_handle h) {
 int dbec_observables_batch(dbec_handle h, dbec_obs* out) {
     if (!h || !out) return DBEC_EINVAL;
     { int rc = enqueue_dipolar_spectrum(h, 0); if (rc) return rc; }
-    LAUNCH(h, dbec_launch_phi_out(h, h->phi));
+    LAUNCH(h, h->gen[0] ? dbec_launch_gen_phi_out(h, h->phi) : dbec_launch_phi_out(h, h->phi));
     LAUNCH(h, dbec_launch_observables(h));
     std::vector<double> v((size_t)h->nb * 16);
     CU(h, cudaMemcpyAsync(v.data(), h->obs_dev, v.size() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -598,16 +622,16 @@ const char* dbec_pass_kernel(dbec_handle h, int slot) {
     if (!h || slot < 0 || slot >= DBEC_MAX_KERNELS) return "";
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
     switch (slot) {
-        case KS_DENS_FFTX: return dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
+        case KS_DENS_FFTX: return h->gen[0] ? "k_gen_density_fftx" : dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
         case KS_FFT_Y_FWD: case KS_FFT_Y_INV:
-            return h->p.ndim == 3 ? (dbec_tma_supported(h, 1) ? "k_fft_tma" : "k_fft_strided") : "";
+            return h->p.ndim == 3 ? (h->gen[1] ? "k_gen_fft_strided" : dbec_tma_supported(h, 1) ? "k_fft_tma" : "k_fft_strided") : "";
         case KS_FFT_LAST_FMI:
-            return dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
-        case KS_IFFTX_NONLIN: return dbec_xwarp_supported(h) ? "k_xwarp_nonlin"
+            return h->gen[last_axis] ? "k_gen_fft_strided" : dbec_tma_supported(h, last_axis) ? "k_fft_tma" : "k_fft_strided";
+        case KS_IFFTX_NONLIN: return h->gen[0] ? "k_gen_ifftx_nonlin" : dbec_xwarp_supported(h) ? "k_xwarp_nonlin"
                                      : (h->fuse_cnx && dbec_xline_supported(h)) ? "k_xline_nonlin" : "k_ifftx_nonlin";
-        case KS_CN_X: return h->fuse_cnx ? "" : "k_cn_x";
-        case KS_CN_Y: return dbec_tma_supported(h, 1) ? "k_cn_tma" : "k_cn_strided";
-        case KS_CN_Z: return h->p.ndim == 3 ? (dbec_tma_supported(h, 2) ? "k_cn_tma" : "k_cn_strided") : "";
+        case KS_CN_X: return h->fuse_cnx ? "" : h->gen[0] ? "k_gen_cn" : "k_cn_x";
+        case KS_CN_Y: return h->gen[1] ? "k_gen_cn" : dbec_tma_supported(h, 1) ? "k_cn_tma" : "k_cn_strided";
+        case KS_CN_Z: return h->p.ndim == 3 ? (h->gen[2] ? "k_gen_cn" : dbec_tma_supported(h, 2) ? "k_cn_tma" : "k_cn_strided") : "";
     }
     return "";
 }

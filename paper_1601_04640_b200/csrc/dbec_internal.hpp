@@ -7,7 +7,7 @@
 #include "../../include/dbec.h"
 #include "cplx.cuh"
 
-#define DBEC_MAX_N 512          // longest supported grid line (16 values per thread x 32 lanes)
+#define DBEC_MAX_N 1024         // longest supported grid line
 #define DBEC_MAX_KERNELS 8      // kernel slots of one step (dbec_step_profile)
 #define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
 #define DBEC_TMAP_BYTES 128     // sizeof(CUtensorMap)
@@ -94,6 +94,9 @@ struct dbec_handle_s {
     unsigned int* ticket;           // last-block tickets
     double* obs_dev;                // nb x 16 doubles
     AxisTables ax[3];
+    // axes whose length is not one of the powers of two 16..512 run in the run-time-length kernels of
+    // kernels_gen.cu: gen[axis] = 1, radices of the Stockham passes in gfac[axis][0..gnfac)
+    int gen[3], gnfac[3], gfac[3][12];
     int npartial;
     // CUDA graph of one step
     cudaGraphExec_t graph_exec;
@@ -130,6 +133,13 @@ int dbec_launch_observables(dbec_handle_s* h);             // a9 (expects h->phi
 int dbec_launch_density_2d(dbec_handle_s* h, int member, int axis, double* out);   // reading S27 (3-D grids)
 int dbec_launch_density_1d(dbec_handle_s* h, int member, int axis, double* out, double* scratch);
 int dbec_launch_build_vdd(dbec_handle_s* h);               // potdd table
+// run-time line lengths 2^a 3^b 5^c 7^d (kernels_gen.cu)
+int dbec_gen_factor(int n, int* fac);
+int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance);
+int dbec_launch_gen_fft(dbec_handle_s* h, int axis, int mode);
+int dbec_launch_gen_nonlinear(dbec_handle_s* h);                // a3 (x) + a4, no sweep
+int dbec_launch_gen_phi_out(dbec_handle_s* h, double* phi);
+int dbec_launch_gen_cn(dbec_handle_s* h, int axis, int with_norm);
 // persistent TMA-fed versions of the strided passes (kernels_tma.cu); z0, nzs: slab of planes (y passes)
 int dbec_make_tensor_maps(dbec_handle_s* h);
 int dbec_tma_supported(const dbec_handle_s* h, int axis);

@@ -1,0 +1,381 @@
+// kernels_gen.cu — every pass of the step for grid lines whose length is NOT one of the powers of two the
+// register-resident kernels are built for: any N = 2^a 3^b 5^c 7^d, 4 <= N <= 1024 (the paper's own
+// experiment sweeps 50^3 .. 600^3 and 1000^2 .. 15000^2 and advises "experimenting with different grid sizes",
+// PAPER.md:81, :89, :93).  Same arithmetic as kernels_fft.cu / kernels_cn.cu (calcpsidd2, calcnu, calclux/y/z,
+// calcnorm — PAPER.md:63, :67, :71, :79); what changes is that the line length is a run-time number:
+//   * the line FFT is a Stockham autosort transform in shared memory, one radix-r pass (r = 4, 2, 3, 5, 7) per
+//     factor of N, twiddles from the axis' table exp(-2 pi i j / N);
+//   * the Crank-Nicolson solve is the chunked Thomas scheme of cn_chunk.cuh with ceil(N / 16) chunks, the last
+//     one padded with h = 0 (a padded point solves to 0 and feeds nothing back).
+// A handle may mix: an axis of 96 points runs here, an axis of 256 points in the persistent kernels.
+#include "dbec_internal.hpp"
+#include "fft_line.cuh"
+#include "cn_chunk.cuh"
+#include "cn_line_smem.cuh"
+#include "tma_pipe.cuh"
+#include "norm_finish.cuh"
+
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
+
+struct GenPlan {
+    int n, nfac;
+    int fac[12];        // radices in the order they are applied
+};
+
+// One radix-R Stockham butterfly.  in / out: element e of the line at e*SE.  Ns = product of the radices already
+// applied, nb = n / R, j < nb.  twN[j] = exp(-2 pi i j / n); S = -1 forward, +1 inverse.
+template <int R, int S>
+__device__ __forceinline__ void gen_butterfly(const cd* in, cd* out, int SE, int j, int Ns, int nb, int n, const cd* __restrict__ twN) {
+    const int k = j % Ns;
+    cd v[R];
+    const int tstep = (n / (Ns * R)) * k;                    // W_{Ns R}^{k t} = twN[t * tstep]
+#pragma unroll
+    for (int t = 0; t < R; ++t) {
+        v[t] = in[(j + t * nb) * SE];
+        if (t > 0) v[t] = cmul(v[t], tw_dir<S>(twN[(t * tstep) % n]));
+    }
+    if (R == 2) dft2<S>(v[0], v[1]);
+    else if (R == 4) dft4<S>(v[0], v[1], v[2], v[3]);
+    else {                                                   // 3, 5, 7: the definition, roots W_R^q = twN[q n / R]
+        cd w[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            cd acc = v[0];
+#pragma unroll
+            for (int t = 1; t < R; ++t) acc = cfma(v[t], tw_dir<S>(twN[((q * t) % R) * (n / R)]), acc);
+            w[q] = acc;
+        }
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = w[q];
+    }
+    const int j0 = (j - k) * R + k;
+#pragma unroll
+    for (int t = 0; t < R; ++t) out[(j0 + t * Ns) * SE] = v[t];
+}
+
+// Transform L lines held in shared memory (line l starts at l*SL, element stride SE) with all threads of the
+// block; a and b are the two Stockham buffers.  LFAST: the line index runs fastest over the threads (tiles of
+// neighbouring columns) or the butterfly index does (contiguous lines).  Returns the buffer holding the result.
+template <int S, bool LFAST>
+__device__ __forceinline__ cd* gen_fft_lines(cd* a, cd* b, int L, int SL, int SE, const GenPlan& pl, const cd* __restrict__ twN) {
+    int Ns = 1;
+    for (int s = 0; s < pl.nfac; ++s) {
+        const int r = pl.fac[s], nb = pl.n / r;
+        for (int idx = threadIdx.x; idx < L * nb; idx += blockDim.x) {
+            const int l = LFAST ? idx % L : idx / nb, j = LFAST ? idx / L : idx % nb;
+            const cd* in = a + l * SL;
+            cd* out = b + l * SL;
+            switch (r) {
+                case 2: gen_butterfly<2, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
+                case 3: gen_butterfly<3, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
+                case 4: gen_butterfly<4, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
+                case 5: gen_butterfly<5, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
+                default: gen_butterfly<7, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
+            }
+        }
+        __syncthreads();
+        cd* t = a; a = b; b = t;
+        Ns *= r;
+    }
+    return a;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1, x axis: n = |s psi|^2 -> half spectrum, two real lines per complex transform
+// ------------------------------------------------------------------------------------------------
+// Block = LP line pairs; shared memory: two buffers of LP lines of n complex values.
+__global__ void __launch_bounds__(256)
+k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twN, double* __restrict__ scal,
+                   GenPlan pl, int LP, int npairs, int nxhp, int pairs_per_member, int nb, int advance) {
+    extern __shared__ cd gsm[];
+    pdl_launch_dependents(); pdl_wait();
+    const int n = pl.n;
+    cd* a = gsm; cd* b = gsm + (size_t)LP * n;
+    const long long pair0 = (long long)blockIdx.x * LP;
+    for (int idx = threadIdx.x; idx < LP * n; idx += blockDim.x) {
+        const int l = idx / n, x = idx % n;
+        const long long pair = pair0 + l;
+        cd v = cmake(0.0, 0.0);
+        if (pair < npairs) {
+            const double s2 = scal[(pair / pairs_per_member) * SC_COUNT + SC_S2];
+            v = cmake(s2 * cnorm2(psi[pair * 2 * n + x]), s2 * cnorm2(psi[(pair * 2 + 1) * n + x]));
+        }
+        a[idx] = v;
+    }
+    if (advance && blockIdx.x == 0)            // first kernel of a step: move the NSTP ramp on (reads neither G nor D)
+        for (int m = threadIdx.x; m < nb; m += blockDim.x) ramp_advance(scal + (size_t)m * SC_COUNT);
+    __syncthreads();
+    const cd* z = gen_fft_lines<-1, false>(a, b, LP, n, 1, pl, twN);
+    for (int idx = threadIdx.x; idx < LP * nxhp; idx += blockDim.x) {
+        const int l = idx / nxhp, k = idx % nxhp;
+        const long long pair = pair0 + l;
+        if (pair >= npairs) continue;
+        cd xa = cmake(0.0, 0.0), xb = xa;
+        if (k <= n / 2) {
+            const cd zk = z[l * n + k], zp = z[l * n + (k ? n - k : 0)];
+            // X_a = (Z[k] + conj Z[N-k])/2,  X_b = (Z[k] - conj Z[N-k])/(2i)
+            xa = cmake(0.5 * (zk.x + zp.x), 0.5 * (zk.y - zp.y));
+            xb = cmake(0.5 * (zk.y + zp.y), -0.5 * (zk.x - zp.x));
+        }
+        spec[pair * 2 * nxhp + k] = xa;
+        spec[(pair * 2 + 1) * nxhp + k] = xb;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 / a3 along y or z on the half spectrum; MODE 2 = forward * V_dd(k)/P * inverse (a2 fused)
+// ------------------------------------------------------------------------------------------------
+// A tile is `cols` neighbouring columns (8: one 128-byte row per line point; 4 for lines longer than 512 points,
+// so that two buffers of n x cols values fit), element (j, col) at j*cols + col in shared memory.
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twN, GenPlan pl, int cols,
+                  long long line_stride, long long outer_stride, int ntiles_x, long long ntiles, int nxhp, int ny3,
+                  long long vdd_line_stride) {
+    extern __shared__ cd gsm[];
+    pdl_launch_dependents(); pdl_wait();
+    const int n = pl.n;
+    cd* a = gsm; cd* b = gsm + (size_t)n * cols;
+    const long long tile = blockIdx.x;
+    if (tile >= ntiles) return;
+    const long long outer = tile / ntiles_x, tx = tile % ntiles_x;
+    cd* g = spec + outer * outer_stride + tx * cols;
+    for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) a[idx] = g[(long long)(idx / cols) * line_stride + idx % cols];
+    __syncthreads();
+    cd* r = a; cd* o = b;
+    if (MODE == 0 || MODE == 2) { r = gen_fft_lines<-1, true>(a, b, cols, 1, cols, pl, twN); o = (r == a) ? b : a; }
+    if (MODE == 2) {
+        // folded V_dd table (kernels_fft.cu: k_fft_strided): row j -> min(j, n - j); 3-D: k_y of the column folds too
+        for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) {
+            const int j = idx / cols;
+            const long long cix = tx * cols + idx % cols;
+            long long voff = cix;
+            if (ny3) { const int ky = (int)(cix / nxhp), kx = (int)(cix % nxhp); voff = (long long)(ky < ny3 - ky ? ky : ny3 - ky) * nxhp + kx; }
+            r[idx] = cmul(vdd[voff + (long long)(j < n - j ? j : n - j) * vdd_line_stride], r[idx]);
+        }
+        __syncthreads();
+    }
+    if (MODE == 1 || MODE == 2) r = gen_fft_lines<+1, true>(r, o, cols, 1, cols, pl, twN);
+    for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) g[(long long)(idx / cols) * line_stride + idx % cols] = r[idx];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3 (x axis, complex-to-real, two lines per transform) + a4 calcnu, or Phi_dd written out
+// ------------------------------------------------------------------------------------------------
+template <bool RT, bool PHI>
+__global__ void __launch_bounds__(256)
+k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out, const cd* __restrict__ twN,
+                   const double* __restrict__ scal, const double* __restrict__ vx, const double* __restrict__ vy,
+                   const double* __restrict__ vz, double dt, GenPlan pl, int LP, int npairs, int nxhp, int ny, int nz) {
+    extern __shared__ cd gsm[];
+    pdl_launch_dependents(); pdl_wait();
+    const int n = pl.n;
+    cd* a = gsm; cd* b = gsm + (size_t)LP * n;
+    const long long pair0 = (long long)blockIdx.x * LP;
+    for (int idx = threadIdx.x; idx < LP * n; idx += blockDim.x) {
+        const int l = idx / n, k = idx % n;
+        const long long pair = pair0 + l;
+        cd v = cmake(0.0, 0.0);
+        if (pair < npairs) {
+            const cd* sa = spec + pair * 2 * nxhp;
+            const cd* sb = sa + nxhp;
+            if (k <= n / 2) { const cd p = sa[k], q = sb[k]; v = cmake(p.x - q.y, p.y + q.x); }            // X_a + i X_b
+            else { const cd p = sa[n - k], q = sb[n - k]; v = cmake(p.x + q.y, q.x - p.y); }               // conj X_a + i conj X_b
+        }
+        a[idx] = v;
+    }
+    __syncthreads();
+    const cd* f = gen_fft_lines<+1, false>(a, b, LP, n, 1, pl, twN);      // (Phi on line a, Phi on line b); 1/P is in the table
+    for (int idx = threadIdx.x; idx < 2 * LP * n; idx += blockDim.x) {
+        const int ll = idx / n, x = idx % n;                              // line ll of the block: pair ll / 2, component ll & 1
+        const long long row = (pair0 + ll / 2) * 2 + (ll & 1);
+        if (row >= 2LL * npairs) continue;
+        const cd pp = f[(ll / 2) * n + x];
+        const double phi = (ll & 1) ? pp.y : pp.x;
+        if (PHI) { phi_out[row * n + x] = phi; continue; }
+        const int y = (int)(row % ny), zz = (int)(row / ny), z = zz % nz;
+        const double* sc = scal + (size_t)(zz / nz) * SC_COUNT;           // this row's batch member
+        const double s = sc[SC_S], s2 = sc[SC_S2];
+        const cd q = psi[row * n + x];
+        const double u = dt * (vx[x] + vy[y] + vz[z] + sc[SC_G] * (s2 * cnorm2(q)) + sc[SC_D] * phi);
+        cd r;
+        if (RT) { double sn, cs; sincos(u, &sn, &cs); r = cmul(s, cmul(q, cmake(cs, -sn))); }
+        else r = cmul(s * exp(-u), q);
+        psi[row * n + x] = r;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5..a7 (+ a8): Crank-Nicolson sweep along any axis, ceil(n / 16) chunks per line
+// ------------------------------------------------------------------------------------------------
+// Thread (chunk c, column col) of a tile of GC columns; point j of column q sits at q*col_stride + j*elem_stride
+// (x sweep: columns are lines, elem_stride 1; y / z sweeps: columns are neighbouring x, elem_stride = line stride).
+// blockIdx.y = outer index (plane or batch member).  Points j >= n of the last chunk are padding: psi = 0, h = 0.
+constexpr int GC = 8;
+template <bool RT, bool NORM>
+__global__ void __launch_bounds__(512)
+k_gen_cn(cd* __restrict__ psi, CnTab<RT> cn, int n, int nch, long long elem_stride, long long col_stride, long long outer_stride,
+         long long ncols, double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV, int nb) {
+    typedef typename CnCoef<RT>::type CT;
+    extern __shared__ cd gsm[];                // [2][chunk slots][GC] zero-start chunk ends
+    // (the block is rounded up to whole warps: chunk slots c >= nch hold padding only and solve to zero)
+    const int nslot = blockDim.x / GC;
+    __shared__ double red[32];
+    pdl_launch_dependents(); pdl_wait();
+    const int col = threadIdx.x % GC, c = threadIdx.x / GC, j0 = c * CN_L;
+    long long q = (long long)blockIdx.x * GC + col;
+    const bool active = q < ncols;
+    if (!active) q = 0;
+    cd* g = psi + (long long)blockIdx.y * outer_stride + q * col_stride;
+    const cd zero = cmake(0.0, 0.0);
+    cd u[CN_L];
+#pragma unroll
+    for (int i = 0; i < CN_L; ++i) u[i] = (j0 + i < n) ? g[(j0 + i) * elem_stride] : zero;
+    // the tables are zero-padded to whole chunks (dbec_api.cu: upload_axis); chunk slots beyond them read chunk 0
+    const int jt = j0 < n ? j0 : 0;
+    const bool pad = j0 >= n;
+    const cd lo = (j0 > 0 && j0 - 1 < n) ? g[(j0 - 1) * elem_stride] : zero;
+    const cd hi = (j0 + CN_L < n) ? g[(j0 + CN_L) * elem_stride] : zero;
+    cn_chunk_forward<CT>(u, lo, hi, cn.kap, cn.h + jt);
+    if (pad) {
+#pragma unroll
+        for (int i = 0; i < CN_L; ++i) u[i] = zero;
+    }
+    cd* e0 = gsm; cd* e1 = gsm + nslot * GC;
+    e0[c * GC + col] = u[CN_L - 1];
+    __syncthreads();
+    // carries over ALL earlier / later chunks; chunk-end products from the per-element tables
+    cd din = zero;
+    for (int i = 0; i < c && i < nch; ++i) din = cn_fma(cn.pf[i * CN_L + CN_L - 1], din, e0[i * GC + col]);
+    cn_chunk_backward<CT>(u, din, cn.h + jt, cn.pf + jt);
+    if (pad) {
+#pragma unroll
+        for (int i = 0; i < CN_L; ++i) u[i] = zero;
+    }
+    e1[c * GC + col] = u[0];
+    __syncthreads();
+    cd uin = zero;
+    for (int i = nch - 1; i > c; --i) uin = cn_fma(cn.pb[i * CN_L], uin, e1[i * GC + col]);
+    cn_chunk_fix<CT>(u, uin, cn.pb + jt);
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < CN_L; ++i) {
+        if (active && j0 + i < n) { g[(j0 + i) * elem_stride] = u[i]; if (NORM) acc += cnorm2(u[i]); }
+    }
+    if (NORM) {
+        // block sum in a fixed order, then the last block's per-member finish (kernels_cn.cu)
+        double x = acc;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+        __syncthreads();
+        if (l == 0) red[w] = x;
+        __syncthreads();
+        double part = 0.0;
+        if (threadIdx.x == 0) for (int i = 0; i < nw; ++i) part += red[i];
+        __syncthreads();
+        norm_finish(part, partial, ticket, scal, dV, red, nb);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+// Radices of a length with factors 2, 3, 5, 7 only: 4s first, then one 2, then the odd ones.  Returns the number
+// of radices, 0 if n has another prime factor.
+int dbec_gen_factor(int n, int* fac) {
+    int k = 0;
+    while (n % 4 == 0) { fac[k++] = 4; n /= 4; }
+    if (n % 2 == 0) { fac[k++] = 2; n /= 2; }
+    for (int p = 3; p <= 7; p += 2) while (n % p == 0) { fac[k++] = p; n /= p; }
+    return n == 1 ? k : 0;
+}
+
+static GenPlan plan_of(const dbec_handle_s* h, int axis) {
+    GenPlan pl;
+    pl.n = h->ax[axis].n;
+    pl.nfac = h->gnfac[axis];
+    for (int i = 0; i < 12; ++i) pl.fac[i] = h->gfac[axis][i];
+    return pl;
+}
+
+template <class K> static int gen_smem(K kernel, size_t bytes) {
+    if (bytes > 48 * 1024) CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return 0;
+}
+
+// line pairs per block of the x kernels: two buffers of LP lines within 64 KiB
+static int gen_lp(int n) { int lp = 2048 / n; return lp < 1 ? 1 : (lp > 8 ? 8 : lp); }
+
+int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance) {
+    const GenPlan pl = plan_of(h, 0);
+    const int LP = gen_lp(pl.n), ppm = h->ny * h->nz / 2, npairs = ppm * h->nb;
+    const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
+    CK((cudaError_t)gen_smem(k_gen_density_fftx, sm));
+    CK(launch_pdl(k_gen_density_fftx, dim3((npairs + LP - 1) / LP), dim3(256), sm, h->stream, h->use_pdl, (const cd*)h->psi, h->spec,
+                  h->ax[0].twN, h->scal, pl, LP, npairs, h->nxhp, ppm, h->nb, advance));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+template <int MODE> static int launch_gen_fft(dbec_handle_s* h, int axis) {
+    const GenPlan pl = plan_of(h, axis);
+    const int cols = pl.n <= 512 ? 8 : 4;
+    long long line_stride, outer_stride, ntiles;
+    int ntx;
+    if (axis == 1) { line_stride = h->nxhp; outer_stride = (long long)h->ny * h->nxhp; ntx = h->nxhp / cols; ntiles = (long long)ntx * h->nplanes; }
+    else { line_stride = (long long)h->ny * h->nxhp; outer_stride = h->SP; ntx = (int)(line_stride / cols); ntiles = (long long)ntx * h->nb; }
+    const int ny3 = axis == 2 ? h->ny : 0;
+    const long long vls = axis == 2 ? (long long)h->nyf * h->nxhp : h->nxhp;
+    const size_t sm = 2 * (size_t)pl.n * cols * sizeof(cd);
+    auto k = k_gen_fft_strided<MODE>;
+    CK((cudaError_t)gen_smem(k, sm));
+    CK(launch_pdl(k, dim3((unsigned)ntiles), dim3(256), sm, h->stream, h->use_pdl, h->spec, (const double*)h->vdd, h->ax[axis].twN, pl,
+                  cols, line_stride, outer_stride, ntx, ntiles, h->nxhp, ny3, vls));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_gen_fft(dbec_handle_s* h, int axis, int mode) {
+    return mode == 0 ? launch_gen_fft<0>(h, axis) : mode == 1 ? launch_gen_fft<1>(h, axis) : launch_gen_fft<2>(h, axis);
+}
+
+template <bool RT, bool PHI> static int launch_gen_nonlin(dbec_handle_s* h, double* phi) {
+    const GenPlan pl = plan_of(h, 0);
+    const int LP = gen_lp(pl.n), npairs = h->ny * h->nz / 2 * h->nb;
+    const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
+    auto k = k_gen_ifftx_nonlin<RT, PHI>;
+    CK((cudaError_t)gen_smem(k, sm));
+    CK(launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(256), sm, h->stream, h->use_pdl, (const cd*)h->spec, h->psi, phi, h->ax[0].twN,
+                  (const double*)h->scal, h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, pl, LP, npairs, h->nxhp, h->ny, h->nz));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_gen_nonlinear(dbec_handle_s* h) {
+    return h->p.time_mode == 1 ? launch_gen_nonlin<true, false>(h, nullptr) : launch_gen_nonlin<false, false>(h, nullptr);
+}
+int dbec_launch_gen_phi_out(dbec_handle_s* h, double* phi) { return launch_gen_nonlin<false, true>(h, phi); }
+
+template <bool RT, bool NORM> static int launch_gen_cn(dbec_handle_s* h, int axis) {
+    const int n = h->ax[axis].n, nch = (n + CN_L - 1) / CN_L;
+    const int threads = (nch * GC + 31) / 32 * 32;
+    long long es, cs, os, ncols;
+    int nouter;
+    if (axis == 0) { es = 1; cs = h->nx; os = 0; ncols = (long long)h->ny * h->nplanes; nouter = 1; }
+    else if (axis == 1) { es = h->nx; cs = 1; os = (long long)h->nx * h->ny; ncols = h->nx; nouter = h->nplanes; }
+    else { es = (long long)h->nx * h->ny; cs = 1; os = h->P; ncols = es; nouter = h->nb; }
+    dim3 grid((unsigned)((ncols + GC - 1) / GC), (unsigned)nouter);
+    if (NORM && (long long)grid.x * grid.y > h->npartial) return (int)cudaErrorInvalidValue;
+    const size_t sm = 2 * (size_t)(threads / GC) * GC * sizeof(cd);
+    CK(launch_pdl(k_gen_cn<RT, NORM>, grid, dim3(threads), sm, h->stream, h->use_pdl, h->psi, make_cntab<RT>(h->ax[axis]), n, nch, es, cs, os,
+                  ncols, h->partial, h->ticket, h->scal, h->dV, h->nb));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
+int dbec_launch_gen_cn(dbec_handle_s* h, int axis, int with_norm) {
+    if (axis == 0 && with_norm) return (int)cudaErrorInvalidValue;
+    if (h->p.time_mode == 1) return with_norm ? launch_gen_cn<true, true>(h, axis) : launch_gen_cn<true, false>(h, axis);
+    return with_norm ? launch_gen_cn<false, true>(h, axis) : launch_gen_cn<false, false>(h, axis);
+}

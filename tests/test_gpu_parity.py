@@ -308,10 +308,76 @@ def test_real_time_norm_conserved_on_gpu(gp):
     sim.close()
 
 
+# ------------------------------------------------------------------ f2: line lengths that are not powers of two
+GEN3 = [(96, 80, 48), (48, 20, 12), (50, 14, 6), (1024, 8, 4), (12, 1024, 4), (6, 10, 600), (256, 96, 40), (80, 128, 256),
+        (16, 24, 32)]
+GEN2 = [(96, 80), (1000, 12), (50, 70), (512, 48), (48, 512), (1024, 1024)]
+
+
+def gen_workloads():
+    out = []
+    for mode in (IMAG, REAL):
+        for s in GEN3:
+            out.append(grid3(*s, mode, d=(0.4, 0.3, 0.6)))
+        for s in GEN2:
+            out.append(grid2(*s, mode, dx=0.2, dy=0.25, plane=(s[0] // 2) % 2))
+    return out
+
+
+@pytest.mark.parametrize("w", gen_workloads(), ids=wid)
+def test_non_power_of_two_lengths(gp, ob, w):
+    """Every part and one full step on grids whose lines run in the run-time-length kernels (kernels_gen.cu), mixed
+    with axes the register-resident / persistent kernels serve."""
+    psi0 = random_psi(w, 9)
+    p = ob.params_of(w)
+    sim = gp.Dbec(gp.params_of(w))
+    for axis in range(w.ndim):
+        sim.set_psi(psi0)
+        sim.cn_sweep(axis)
+        assert relerr(sim.get_psi(), ob.cn_sweep(p, psi0, axis)) < PSI_TOL, f"cn axis {axis}"
+    sim.set_psi(psi0)
+    phi = ob.phi_dd(p, np.abs(psi0) ** 2)
+    assert relerr(sim.phi_dd().cpu().numpy(), phi) < PSI_TOL
+    sim.nonlinear()
+    assert relerr(sim.get_psi(), ob.nonlinear(p, psi0, phi)) < PSI_TOL
+    sim.set_psi(psi0)
+    sim.step(2)
+    o = ob.Oracle(p)
+    o.set_psi(psi0)
+    o.step(2)
+    assert relerr(sim.get_psi(), o.get_psi()) < PSI_TOL
+    a, b = sim.observables(), o.observables()
+    for k in b:
+        if w.ndim == 2 and k == "rms_z":
+            continue
+        assert abs(a[k] - b[k]) <= OBS_TOL * max(abs(b[k]), 1e-300), k
+    sim.close()
+    o.close()
+
+
+def test_non_power_of_two_batch_and_ramp(gp, ob):
+    w = grid3(48, 20, 12, IMAG, d=(0.4, 0.3, 0.6))
+    nb = 3
+    psis = np.stack([initial_psi(w, noise=1e-3 * (m + 1)) for m in range(nb)])
+    sim = gp.Dbec(gp.params_of(w), nbatch=nb)
+    sim.set_psi(psis)
+    sim.set_ramp(3, 0.0, 0.0, w.G, w.D)
+    sim.step(4)
+    got = sim.get_psi()
+    for m in range(nb):
+        o = ob.Oracle(ob.params_of(w))
+        o.set_psi(psis[m])
+        o.set_ramp(3, 0.0, 0.0, w.G, w.D)
+        o.step(4)
+        assert relerr(got[m], o.get_psi()) < PSI_TOL, m
+        o.close()
+    sim.close()
+
+
 def test_errors_and_edge_cases(gp):
     import ctypes as C
     L = gp.lib()
-    p = gp.params(3, 48, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0)
+    p = gp.params(3, 44, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0)
     n = C.c_size_t()
     assert L.dbec_workspace_bytes(C.byref(p), C.byref(n)) == gp.DBEC_ESIZE
     p = gp.params(3, 32, 32, 32, .5, .5, .5, -1.0, 1, 1, .5, 1, 1, 0)

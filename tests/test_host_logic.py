@@ -43,12 +43,18 @@ def test_workspace_bytes_validation_is_host_only(gp):
     assert n.value < 16 * P + 16 * SP + 8 * VP + 8 * P + (4 << 20)
     xz = gp.params(2, 32, 32, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0, plane=1)
     assert L.dbec_workspace_bytes(C.byref(xz), C.byref(n)) == gp.DBEC_OK
+    # lengths 4..1024 with prime factors 2, 3, 5, 7 (the paper's grids are mostly not powers of two)
+    for shape in ((48, 32, 32), (96, 80, 48), (1024, 32, 8), (50, 70, 6), (600, 4, 4)):
+        ok2 = gp.params(3, *shape, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0)
+        assert L.dbec_workspace_bytes(C.byref(ok2), C.byref(n)) == gp.DBEC_OK, shape
     assert L.dbec_workspace_bytes(None, C.byref(n)) == gp.DBEC_EINVAL
     assert L.dbec_workspace_bytes(C.byref(ok), None) == gp.DBEC_EINVAL
     for bad, code in [
-        (gp.params(3, 48, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # not 2^k
-        (gp.params(3, 1024, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),    # too long
-        (gp.params(3, 32, 32, 8, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # too short
+        (gp.params(3, 44, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # prime factor 11
+        (gp.params(3, 2048, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),    # too long
+        (gp.params(3, 32, 32, 2, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # too short
+        (gp.params(3, 45, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),       # NX odd
+        (gp.params(2, 32, 15, 1, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_ESIZE),        # NY*NZ odd: lines do not pair
         (gp.params(2, 32, 32, 2, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),      # 2-D with nz != 1
         (gp.params(4, 32, 32, 32, .5, .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
         (gp.params(3, 32, 32, 32, 0., .5, .5, .025, 1, 1, .5, 1, 1, 0), gp.DBEC_EINVAL),
