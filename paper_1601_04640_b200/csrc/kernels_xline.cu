@@ -157,7 +157,7 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
                             sincos_cw(u[jj], &sn, &cs_);          // branch-free: the evaluations interleave
                             q[jj] = cmul(s, cmul(q[jj], cmake(cs_, -sn)));
                         } else {
-                            q[jj] = cmul(s * exp(-u[jj]), q[jj]);
+                            q[jj] = cmul(s * exp_cw(-u[jj]), q[jj]);
                         }
                     }
 #pragma unroll

@@ -27,9 +27,9 @@
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
 constexpr int WL = 8;              // Crank-Nicolson chunk: 8 points = one 128-byte row of psi
-// calcnu: points evaluated side by side (same reason as NLU_C in kernels_xline.cu); the library exp of imaginary
-// time needs more registers per evaluation than the branch-free sin/cos
-template <bool RT> struct NlwBatch { static constexpr int C = RT ? 4 : 2; };
+// calcnu: points evaluated side by side (same reason as NLU_C in kernels_xline.cu); both time modes use the
+// branch-free functions of trig.cuh, whose evaluations interleave
+template <bool RT> struct NlwBatch { static constexpr int C = 4; };
 
 template <int N> struct WPlan;
 template <> struct WPlan<256> { typedef FftPlanV<8, 8, 4> P; };     // one pair per warp (32 lanes)
@@ -196,7 +196,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
                                 sincos_cw(a[kk], &sn, &cs_);          // branch-free: the evaluations interleave
                                 u[k0 + kk] = cmul(s, cmul(u[k0 + kk], cmake(cs_, -sn)));
                             } else {
-                                u[k0 + kk] = cmul(s * exp(-a[kk]), u[k0 + kk]);
+                                u[k0 + kk] = cmul(s * exp_cw(-a[kk]), u[k0 + kk]);
                             }
                         }
                     }
