@@ -56,6 +56,10 @@ ALG_BYTES_PER_POINT = {
     "cn_x": 32,
     "cn_y": 32,
     "cn_z": 32,
+    # the whole step of a small grid in one launch (kernels_small.cu): the fused pipeline's bytes per point,
+    # filled in per workload by alg_bytes() — the data never leaves L2, so its HBM fraction only says how far
+    # from a streaming grid the small one runs
+    "sscn_step<cluster>": None,
 }
 MODEL_BYTES_PER_POINT = {3: 208, 2: 144}    # SURVEY.md §8(d) "Model M": fixed reference accounting
 # What this repository's fused pipeline itself has to stream (x sweep inside the nonlinear kernel): the honest
@@ -65,6 +69,11 @@ FUSED_BYTES_PER_POINT = {3: 176, 2: 112}
 # multiply as in a step, the last inverse writing Phi (8 + 8), the reduction pass reading psi and Phi (16 + 8).
 OBS_BYTES_PER_POINT = {3: 24 + 16 + 16 + 16 + 16 + 24, 2: 24 + 16 + 16 + 24}
 REF_BUDGET_S = 240.0                        # --impl reference: whole run (K + W oracle steps)
+
+
+def alg_bytes(name, w):
+    b = ALG_BYTES_PER_POINT[name]
+    return FUSED_BYTES_PER_POINT[w.ndim] if b is None else b
 
 
 def measured_peaks():
@@ -247,7 +256,7 @@ def kernel_profile(sim, w, steps, peak):
     per_kernel = {}
     for name, (tot_ms, cnt) in prof.items():
         avg_ms = tot_ms / cnt
-        gbs = ALG_BYTES_PER_POINT[name] * w.npoints / (avg_ms * 1e-3) / 1e9
+        gbs = alg_bytes(name, w) * w.npoints / (avg_ms * 1e-3) / 1e9
         per_kernel[name] = {"kernel": kernels.get(name, ""), "ms": avg_ms, "alg_GBps": gbs, "frac": gbs / peak}
     return per_kernel
 
@@ -402,7 +411,7 @@ def run_ours(args, w):
         roofline = {"bound": "hbm", "kernel": per_kernel[top]["kernel"], "pass": top, "achieved": per_kernel[top]["alg_GBps"],
                     "peak": peak, "unit": "GB/s", "frac": per_kernel[top]["frac"], "traffic": None, "peak_source": peak_src,
                     "kernel_ms": per_kernel[top]["ms"], "kernel_share_of_step": per_kernel[top]["ms"] / step_ms_prof,
-                    "alg_bytes_per_launch": ALG_BYTES_PER_POINT[top] * w.npoints,
+                    "alg_bytes_per_launch": alg_bytes(top, w) * w.npoints,
                     "per_kernel": per_kernel,
                     "step_model": {"bytes_per_point": model, "achieved_GBps": model * pts_per_ns, "frac": model * pts_per_ns / peak,
                                    "note": "SURVEY 8(d) fixed accounting M (counts an x sweep pass the fused kernels never make)"},

@@ -40,7 +40,8 @@ extern "C" {
 #define DBEC_OK           0
 #define DBEC_EINVAL      -1   /* NULL pointer, bad ndim / time_mode / spacing, nsteps < 0 ...        */
 #define DBEC_ESIZE       -2   /* grid length not a supported FFT length (never silently adjusted,
-                                 contrast PAPER.md:93); supported: powers of two 16..512, NY even   */
+                                 contrast PAPER.md:93); supported: 4..1024 with prime factors 2, 3,
+                                 5, 7 only, NX even, NY*NZ even                                     */
 #define DBEC_EWORKSPACE  -3   /* workspace NULL, misaligned or smaller than dbec_workspace_bytes    */
 #define DBEC_ECUDA       -4   /* a CUDA call failed; dbec_last_cuda_error gives the CUDA code       */
 #define DBEC_ENODEVICE   -5   /* no CUDA device / not an sm_100 device                              */
@@ -97,7 +98,10 @@ int dbec_set_coupling(dbec_handle h, double G, double D);
  * CUDA graph of a step sees it; dbec_observables / dbec_phi_dd do not advance it. */
 int dbec_set_ramp(dbec_handle h, int nstp, double G0, double D0, double G1, double D1);
 
-/* nsteps SSCN steps, asynchronous on the handle's stream, no host sync. */
+/* nsteps SSCN steps, asynchronous on the handle's stream, no host sync.  Grids of up to
+ * 65536 points (per batch member) run all nsteps steps in ONE launch by one thread-block cluster per member
+ * (PAPER.md:79 on launch overhead; environment DBEC_CLUSTER=0 at dbec_create switches that off);
+ * larger grids replay a CUDA graph of the step's seven launches. */
 int dbec_step(dbec_handle h, int nsteps);
 
 /* calcmuen + calcrms on the current psi.  host_out: HOST pointer.  Synchronises
@@ -161,12 +165,13 @@ int dbec_launch_count(dbec_handle h, long long* launches);
  * around every kernel.  ms_per_slot: HOST pointer to DBEC_KERNEL_SLOTS doubles receiving the total
  * milliseconds spent in each kernel slot over the nsteps steps; launches_per_slot: HOST pointer to
  * DBEC_KERNEL_SLOTS counts.  Synchronises the stream.  Slot names from dbec_kernel_name. */
-#define DBEC_KERNEL_SLOTS 8
+#define DBEC_KERNEL_SLOTS 9
 int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long* launches_per_slot);
 const char* dbec_kernel_name(int slot);
 /* Name of the __global__ function that serves pass `slot` on this handle ("" if the pass is not part
- * of this handle's step): grid lines of 128..512 points run in the persistent TMA-fed kernels,
- * shorter ones in the one-tile-per-block kernels. */
+ * of this handle's dbec_step): grid lines of 128..512 points run in the persistent TMA-fed kernels,
+ * shorter ones in the one-tile-per-block kernels; on a small grid the only slot is the last one,
+ * "sscn_step<cluster>" (k_small_step). */
 const char* dbec_pass_kernel(dbec_handle h, int slot);
 
 int dbec_version(void);

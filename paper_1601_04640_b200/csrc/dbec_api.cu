@@ -210,10 +210,11 @@ static int write_member_scalars(dbec_handle h, int first, int count, const doubl
 }
 
 // Kernel slots of one step (dbec_step_profile / dbec_kernel_name).
-enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z };
+enum { KS_DENS_FFTX = 0, KS_FFT_Y_FWD, KS_FFT_LAST_FMI, KS_FFT_Y_INV, KS_IFFTX_NONLIN, KS_CN_X, KS_CN_Y, KS_CN_Z, KS_SMALL_STEP };
 static const char* const kernel_names[DBEC_MAX_KERNELS] = {
     "density+fft_x", "fft_y<fwd>", "fft_last<fwd*Vdd*inv>", "fft_y<inv>",
-    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z"};
+    "ifft_x+calcnu+cn_x", "cn_x", "cn_y", "cn_z", "sscn_step<cluster>"};
+static_assert(DBEC_MAX_KERNELS == DBEC_KERNEL_SLOTS, "include/dbec.h and dbec_internal.hpp disagree on the slot count");
 
 #define KLAUNCH(h, slot, x)                                                                      \
     do {                                                                                         \
@@ -355,8 +356,8 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     h->ticket = (unsigned int*)(w + L.ticket);
     h->obs_dev = (double*)(w + L.obs);
     h->npartial = (int)L.npartial;
-    // the only two switches (both exercised by tests/test_gpu_parity.py): the CUDA graph of a step and the
-    // x sweep fused into the nonlinear kernel
+    // the only three switches (all exercised by tests/test_gpu_parity.py): the CUDA graph of a step, the x sweep
+    // fused into the nonlinear kernel, and the one-launch step of small grids (CTAs per cluster; 0 = off)
     const char* fe = getenv("DBEC_FUSE_CNX");
     h->fuse_cnx = fe ? atoi(fe) : 1;
     const char* ge = getenv("DBEC_GRAPH");
@@ -392,6 +393,13 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
         rc = upload_axis(h, ax, nn[ax], dd[ax], (p->ndim == 2 && ax == 2) ? 0.0 : om[ax], t, &used);
         if (rc) FAIL(rc);
         t += used;
+    }
+    {
+        const char* ce = getenv("DBEC_CLUSTER");
+        int req = ce ? atoi(ce) : -1;
+        if (req > 0 && req != 1 && req != 2 && req != 4 && req != 8 && req != 16) req = -1;
+        h->use_cluster = dbec_small_choose(h, req);
+        h->use_small = h->use_cluster > 0;
     }
     if (h->use_tma) TRY((cudaError_t)dbec_make_tensor_maps(h));
     if (init_scalars(h)) FAIL(DBEC_ECUDA);
@@ -480,6 +488,11 @@ int dbec_batch_size(dbec_handle h, int* nbatch) {
 
 int dbec_step(dbec_handle h, int nsteps) {
     if (!h || nsteps < 0) return DBEC_EINVAL;
+    if (h->use_small) {
+        // a small grid: one launch runs all nsteps steps inside one thread-block cluster (kernels_small.cu)
+        if (nsteps > 0) LAUNCH(h, dbec_launch_small_step(h, nsteps));
+        return DBEC_OK;
+    }
     if (!h->use_graph) {
         for (int i = 0; i < nsteps; ++i) { int rc = enqueue_step(h); if (rc) return rc; }
         return DBEC_OK;
@@ -597,7 +610,11 @@ int dbec_step_profile(dbec_handle h, int nsteps, double* ms_per_slot, long long*
     int rc = DBEC_OK;
     for (int s = 0; s < nsteps && rc == DBEC_OK; ++s) {
         h->prof_on = 1; h->prof_n = 0;
-        rc = enqueue_step(h);
+        if (h->use_small) {
+            rc = [&]() -> int { KLAUNCH(h, KS_SMALL_STEP, dbec_launch_small_step(h, 1)); return DBEC_OK; }();
+        } else {
+            rc = enqueue_step(h);
+        }
         h->prof_on = 0;
         if (rc) break;
         if (cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = DBEC_ECUDA; break; }
@@ -616,11 +633,13 @@ const char* dbec_kernel_name(int slot) {
     return (slot >= 0 && slot < DBEC_MAX_KERNELS) ? kernel_names[slot] : "";
 }
 
-// Which __global__ function serves a pass on this handle (lines of 128..512 points go to the
-// persistent TMA / bulk-copy kernels, shorter ones to the one-tile-per-block kernels).
+// Which __global__ function serves a pass of dbec_step on this handle (lines of 128..512 points go to the
+// persistent TMA / bulk-copy kernels, shorter ones to the one-tile-per-block kernels; a small grid's whole step
+// is one launch of k_small_step).
 const char* dbec_pass_kernel(dbec_handle h, int slot) {
     if (!h || slot < 0 || slot >= DBEC_MAX_KERNELS) return "";
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
+    if (h->use_small) return slot == KS_SMALL_STEP ? "k_small_step" : "";      // dbec_step launches nothing else
     switch (slot) {
         case KS_DENS_FFTX: return h->gen[0] ? "k_gen_density_fftx" : dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
         case KS_FFT_Y_FWD: case KS_FFT_Y_INV:

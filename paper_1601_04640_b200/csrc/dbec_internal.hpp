@@ -8,7 +8,7 @@
 #include "cplx.cuh"
 
 #define DBEC_MAX_N 1024         // longest supported grid line
-#define DBEC_MAX_KERNELS 8      // kernel slots of one step (dbec_step_profile)
+#define DBEC_MAX_KERNELS 9      // kernel slots of one step (dbec_step_profile); the last one is the one-launch small-grid step
 #define DBEC_SPEC_COLS 8        // columns per tile of the strided FFT passes (8 x 16 B = one 128 B line)
 #define DBEC_TMAP_BYTES 128     // sizeof(CUtensorMap)
 
@@ -109,6 +109,10 @@ struct dbec_handle_s {
     int fuse_cnx;                   // env DBEC_FUSE_CNX (default 1): x sweep inside the nonlinear kernel
     int use_tma;                    // 1: persistent TMA-fed kernels for lines of 128..512 points
     int num_sms;
+    int use_cluster;                // CTAs per cluster of the one-launch small-grid step, 0 = not used (dbec_small_choose;
+                                    // env DBEC_CLUSTER = 0 / 1 / 2 / 4 / 8 / 16 overrides the choice)
+    int use_small;                  // 1: dbec_step runs k_small_step (use_cluster > 0)
+    int small_max_clusters;         // clusters of k_small_step that can be resident at once (0: not asked yet)
     int use_pdl;                    // 1: programmatic dependent launch of every kernel of a step
     int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
     int use_rev;                    // 1: consecutive plane-ordered passes walk their tiles in opposite directions
@@ -149,6 +153,9 @@ int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nz
 int dbec_xline_supported(const dbec_handle_s* h);
 int dbec_launch_xline_nonlin(dbec_handle_s* h, int z0, int nzs);          // a3 (x) + a4 + a5
 int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance);   // a1 (x)
+// the whole step of a small grid in one launch by one thread-block cluster (kernels_small.cu)
+int dbec_small_choose(dbec_handle_s* h, int request);     // CTAs per cluster (0: multi-launch path); request < 0: auto
+int dbec_launch_small_step(dbec_handle_s* h, int nsteps);
 // one warp per line pair (kernels_xwarp.cu): a3 (x) + a4 + a5 for lines of 128 / 256 points
 int dbec_xwarp_supported(const dbec_handle_s* h);
 int dbec_launch_xwarp_nonlin(dbec_handle_s* h);

@@ -10,75 +10,13 @@
 // A handle may mix: an axis of 96 points runs here, an axis of 256 points in the persistent kernels.
 #include "dbec_internal.hpp"
 #include "fft_line.cuh"
+#include "fft_gen.cuh"
 #include "cn_chunk.cuh"
 #include "cn_line_smem.cuh"
 #include "tma_pipe.cuh"
 #include "norm_finish.cuh"
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
-
-struct GenPlan {
-    int n, nfac;
-    int fac[12];        // radices in the order they are applied
-};
-
-// One radix-R Stockham butterfly.  in / out: element e of the line at e*SE.  Ns = product of the radices already
-// applied, nb = n / R, j < nb.  twN[j] = exp(-2 pi i j / n); S = -1 forward, +1 inverse.
-template <int R, int S>
-__device__ __forceinline__ void gen_butterfly(const cd* in, cd* out, int SE, int j, int Ns, int nb, int n, const cd* __restrict__ twN) {
-    const int k = j % Ns;
-    cd v[R];
-    const int tstep = (n / (Ns * R)) * k;                    // W_{Ns R}^{k t} = twN[t * tstep]
-#pragma unroll
-    for (int t = 0; t < R; ++t) {
-        v[t] = in[(j + t * nb) * SE];
-        if (t > 0) v[t] = cmul(v[t], tw_dir<S>(twN[(t * tstep) % n]));
-    }
-    if (R == 2) dft2<S>(v[0], v[1]);
-    else if (R == 4) dft4<S>(v[0], v[1], v[2], v[3]);
-    else {                                                   // 3, 5, 7: the definition, roots W_R^q = twN[q n / R]
-        cd w[R];
-#pragma unroll
-        for (int q = 0; q < R; ++q) {
-            cd acc = v[0];
-#pragma unroll
-            for (int t = 1; t < R; ++t) acc = cfma(v[t], tw_dir<S>(twN[((q * t) % R) * (n / R)]), acc);
-            w[q] = acc;
-        }
-#pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = w[q];
-    }
-    const int j0 = (j - k) * R + k;
-#pragma unroll
-    for (int t = 0; t < R; ++t) out[(j0 + t * Ns) * SE] = v[t];
-}
-
-// Transform L lines held in shared memory (line l starts at l*SL, element stride SE) with all threads of the
-// block; a and b are the two Stockham buffers.  LFAST: the line index runs fastest over the threads (tiles of
-// neighbouring columns) or the butterfly index does (contiguous lines).  Returns the buffer holding the result.
-template <int S, bool LFAST>
-__device__ __forceinline__ cd* gen_fft_lines(cd* a, cd* b, int L, int SL, int SE, const GenPlan& pl, const cd* __restrict__ twN) {
-    int Ns = 1;
-    for (int s = 0; s < pl.nfac; ++s) {
-        const int r = pl.fac[s], nb = pl.n / r;
-        for (int idx = threadIdx.x; idx < L * nb; idx += blockDim.x) {
-            const int l = LFAST ? idx % L : idx / nb, j = LFAST ? idx / L : idx % nb;
-            const cd* in = a + l * SL;
-            cd* out = b + l * SL;
-            switch (r) {
-                case 2: gen_butterfly<2, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
-                case 3: gen_butterfly<3, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
-                case 4: gen_butterfly<4, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
-                case 5: gen_butterfly<5, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
-                default: gen_butterfly<7, S>(in, out, SE, j, Ns, nb, pl.n, twN); break;
-            }
-        }
-        __syncthreads();
-        cd* t = a; a = b; b = t;
-        Ns *= r;
-    }
-    return a;
-}
 
 // ------------------------------------------------------------------------------------------------
 // a1, x axis: n = |s psi|^2 -> half spectrum, two real lines per complex transform

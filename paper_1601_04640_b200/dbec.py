@@ -24,7 +24,7 @@ EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi"
            "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel", "dbec_build_id",
            "dbec_set_ramp", "dbec_workspace_bytes_batch", "dbec_create_batch", "dbec_batch_size",
            "dbec_set_coupling_batch", "dbec_observables_batch", "dbec_density_1d", "dbec_density_2d"]
-KERNEL_SLOTS = 8
+KERNEL_SLOTS = 9
 
 
 class DbecParams(C.Structure):

@@ -208,8 +208,21 @@ def one_step_pair(gp, ob, w, psi0, steps=1):
     return sim, o, got, ref
 
 
-@pytest.mark.parametrize("w", all_small_workloads(), ids=wid)
-def test_one_step_small_grids(gp, ob, w):
+def small_step_cases():
+    """(workload, cluster): "auto" = small 3-D grids take the one-launch cluster step (kernels_small.cu), everything
+    else the multi-launch path; "0" = the multi-launch path also on the grids "auto" gives to the cluster step."""
+    out = []
+    for w in all_small_workloads():
+        out.append((w, "auto"))
+        if w.ndim == 3 and w.npoints <= 65536:
+            out.append((w, "0"))
+    return out
+
+
+@pytest.mark.parametrize("w,cluster", small_step_cases(), ids=lambda v: wid(v) if isinstance(v, Workload) else f"cluster-{v}")
+def test_one_step_small_grids(gp, ob, w, cluster, monkeypatch):
+    if cluster == "0":
+        monkeypatch.setenv("DBEC_CLUSTER", "0")
     psi0 = random_psi(w, 9) if w.time_mode == REAL else initial_psi(w)
     sim, o, got, ref = one_step_pair(gp, ob, w, psi0)
     assert relerr(got, ref) < PSI_TOL
@@ -242,6 +255,7 @@ def test_fused_and_unfused_x_sweep_agree(gp, monkeypatch):
     w = workload("C1")
     psi0 = initial_psi(w)
     outs = []
+    monkeypatch.setenv("DBEC_CLUSTER", "0")            # the multi-launch path (C1 would take the one-launch step)
     for fuse in ("1", "0"):
         monkeypatch.setenv("DBEC_FUSE_CNX", fuse)
         sim = gp.Dbec(gp.params_of(w))
@@ -256,6 +270,7 @@ def test_graph_and_plain_launches_agree_bitwise(gp, monkeypatch):
     w = workload("C1")
     psi0 = initial_psi(w)
     outs = []
+    monkeypatch.setenv("DBEC_CLUSTER", "0")
     for g in ("1", "0"):
         monkeypatch.setenv("DBEC_GRAPH", g)
         sim = gp.Dbec(gp.params_of(w))
@@ -264,6 +279,79 @@ def test_graph_and_plain_launches_agree_bitwise(gp, monkeypatch):
         outs.append(sim.get_psi())
         sim.close()
     assert np.array_equal(outs[0], outs[1])
+
+
+CLUSTER_CASES = [grid3(32, 32, 32, IMAG), grid3(32, 32, 32, REAL), grid3(16, 16, 16, REAL), grid3(64, 16, 32, IMAG, d=(0.4, 0.3, 0.6)),
+                 grid3(48, 20, 12, IMAG, d=(0.4, 0.3, 0.6)), grid3(50, 14, 6, REAL), grid3(12, 10, 6, IMAG), grid3(128, 32, 16, REAL),
+                 grid3(16, 64, 64, IMAG), grid2(64, 32, REAL, dx=0.2, dy=0.3), grid2(256, 256, IMAG), grid2(96, 80, REAL, plane=1),
+                 grid2(16, 1024, IMAG)]
+
+
+@pytest.mark.parametrize("cs", ["1", "2", "8", "16"])
+@pytest.mark.parametrize("w", CLUSTER_CASES, ids=wid)
+def test_cluster_step_matches_oracle_and_multi_launch(gp, ob, w, cs, monkeypatch):
+    """kernels_small.cu: the whole step in one launch by one thread-block cluster, several steps per
+    launch, against the oracle and against the multi-launch path, for cluster sizes from 1 CTA (everything in one
+    SM, ragged tiles) to 16; 2-D grids and run-time line lengths are forced onto it here."""
+    psi0 = random_psi(w, 31)
+    monkeypatch.setenv("DBEC_CLUSTER", cs)
+    sim = gp.Dbec(gp.params_of(w))
+    assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_step"}
+    sim.set_psi(psi0)
+    sim.step(3)
+    got = sim.get_psi()
+    obs = sim.observables()
+    n0 = sim.launch_count()
+    sim.step(5)
+    assert sim.launch_count() - n0 == 1            # five steps, one launch
+    sim.close()
+    o = ob.Oracle(ob.params_of(w))
+    o.set_psi(psi0)
+    o.step(3)
+    assert relerr(got, o.get_psi()) < PSI_TOL
+    b = o.observables()
+    for k in b:
+        if w.ndim == 2 and k == "rms_z":
+            continue
+        assert abs(obs[k] - b[k]) <= OBS_TOL * max(abs(b[k]), 1e-300), k
+    o.close()
+    monkeypatch.setenv("DBEC_CLUSTER", "0")
+    ml = gp.Dbec(gp.params_of(w))
+    assert "sscn_step<cluster>" not in ml.pass_kernels()
+    ml.set_psi(psi0)
+    ml.step(3)
+    assert relerr(got, ml.get_psi()) < PSI_TOL
+    ml.close()
+
+
+def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch):
+    """A batch on the cluster step (one cluster per member, per-member couplings, the NSTP ramp advancing inside a
+    launch) and the automatic choice: small 3-D grids only, and only while every member gets a resident cluster."""
+    monkeypatch.delenv("DBEC_CLUSTER", raising=False)
+    w = grid3(32, 32, 32, IMAG, G=0.0, D=0.0)
+    nb = 3
+    psis = np.stack([random_psi(w, 50 + m) for m in range(nb)])
+    sim = gp.Dbec(gp.params_of(w), nbatch=nb)
+    assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_step"}
+    sim.set_psi(psis)
+    sim.set_ramp(4, 0.0, 0.0, 40.0, 25.0)
+    sim.step(6)                                       # the ramp ends inside the launch
+    got = sim.get_psi()
+    sim.close()
+    for m in range(nb):
+        o = ob.Oracle(ob.params_of(w))
+        o.set_psi(psis[m])
+        for k in range(1, 7):
+            f = min(k, 4) / 4.0
+            o.set_coupling(40.0 * f, 25.0 * f)
+            o.step(1)
+        assert relerr(got[m], o.get_psi()) < PSI_TOL, m
+        o.close()
+    for wl, nbatch, small in ((grid3(32, 32, 32, REAL), 1, True), (grid3(32, 32, 32, REAL), 200, False),
+                              (grid2(128, 128, REAL), 1, False), (grid3(64, 64, 32, IMAG), 1, False)):
+        h = gp.Dbec(gp.params_of(wl), nbatch=nbatch)
+        assert ("sscn_step<cluster>" in h.pass_kernels()) == small, (wid(wl), nbatch)
+        h.close()
 
 
 @pytest.mark.parametrize("shape,mode", [((256, 128, 256), REAL), ((128, 128, 128), IMAG), ((256, 256, 64), IMAG)])
