@@ -363,6 +363,7 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     const char* ge = getenv("DBEC_GRAPH");
     h->use_graph = ge ? atoi(ge) : 1;
     h->use_rev = 1; h->use_pdl = 1; h->use_tma = 1;
+    h->zpair_min_stride = 2LL << 20;
     {   // L2 eviction policy per access site: the outputs of the two x-line kernels are kept evict-last (the
         // passes after them find part of the spectrum / of psi in L2), their dead inputs evict-first,
         // everything else a neutral hint (measured alternatives: profiles/r1d_step_ncu_full.md)

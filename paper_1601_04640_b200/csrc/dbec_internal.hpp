@@ -19,7 +19,8 @@ enum { POL_CN_LD = 0, POL_CN_ST, POL_NL_LD, POL_NL_ST, POL_NL_SPEC, POL_D_PSI, P
 // Tensor maps of the handle (kernels_tma.cu): field x direction of the box rows.
 // TM_PSI_XW: psi as [line][NX/8][8 complex] with the 128-byte swizzle (kernels_xwarp.cu).
 // TM_VDD: the folded V_dd table, boxes along the last axis of the grid.
-enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD, TM_PSI_XW, TM_COUNT };
+// TM_PSI_Z2: psi with boxes of 8 columns x 2 rows of y x N rows of z (k_cn_tma with TC = 16).
+enum { TM_PSI_Y = 0, TM_PSI_Z, TM_SPEC_Y, TM_SPEC_Z, TM_VDD, TM_PSI_XW, TM_PSI_Z2, TM_COUNT };
 
 // Device scalars every kernel reads (so that a captured CUDA graph never bakes them in), one block of
 // SC_COUNT doubles per batch member (dbec_create_batch; a plain handle has one member).
@@ -113,6 +114,7 @@ struct dbec_handle_s {
                                     // env DBEC_CLUSTER = 0 / 1 / 2 / 4 / 8 / 16 overrides the choice)
     int use_small;                  // 1: dbec_step runs k_small_step (use_cluster > 0)
     int small_max_clusters;         // clusters of k_small_step that can be resident at once (0: not asked yet)
+    long long zpair_min_stride;     // z sweeps pair two rows of y per tile when the xy plane is at least this many bytes
     int use_pdl;                    // 1: programmatic dependent launch of every kernel of a step
     int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
     int use_rev;                    // 1: consecutive plane-ordered passes walk their tiles in opposite directions
@@ -147,6 +149,7 @@ int dbec_launch_gen_cn(dbec_handle_s* h, int axis, int with_norm);
 // persistent TMA-fed versions of the strided passes (kernels_tma.cu); z0, nzs: slab of planes (y passes)
 int dbec_make_tensor_maps(dbec_handle_s* h);
 int dbec_tma_supported(const dbec_handle_s* h, int axis);
+int dbec_zpair_tiles(const dbec_handle_s* h);
 int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs);
 int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nzs);
 // persistent bulk-copy-fed versions of the x passes (kernels_xline.cu)

@@ -30,6 +30,7 @@ struct TileGeom {
                      // fused y pass of a 2-D grid: 0 (the table has one plane, shared by the members of a batch)
     int vrows;       // rows of one V_dd box, boxes per tile
     int vnbox;
+    int ystep;       // z passes: rows of y per tile (1, or 2 when a tile is 8 columns x 2 rows of y: k_cn_tma with TC = 16)
     int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
     float pol_ld, pol_st;   // L2 eviction policy codes of the tile loads / stores (tma_pipe.cuh: l2_policy_code)
 };
@@ -56,7 +57,7 @@ __device__ __forceinline__ void tile_coords(const TileGeom& tg, int t, int b, in
     if (tg.rev) t = tg.ntiles - 1 - t;
     const int tx = t % tg.ntiles_x, o = t / tg.ntiles_x + tg.outer0;
     c0 = tx * inner;
-    c1 = tg.axis == 1 ? b * tg.box_rows : o;
+    c1 = tg.axis == 1 ? b * tg.box_rows : o * tg.ystep;
     c2 = tg.axis == 1 ? o : b * tg.box_rows;
 }
 
@@ -142,12 +143,15 @@ template <int NT> __device__ __forceinline__ double block_sum_t(double x, double
 // ------------------------------------------------------------------------------------------------
 // Crank-Nicolson sweep along y or z (calcluy / calcluz)
 // ------------------------------------------------------------------------------------------------
-template <bool RT, int NCH, int NG, int NST, bool NORM>
-__global__ void __launch_bounds__(NG* NCH* TCOLS + 96, 1)
+// TC: lines per tile — 8 neighbouring columns, or 16 = 8 columns x 2 neighbouring rows of y (z sweeps whose planes are
+// 2 MiB or more apart: the two rows of a plane share a memory page, so a tile touches half as many pages per byte;
+// measured at 512 x 512 x 256, plane stride 4 MiB: 473 -> 415 us; no change at 256^3, plane stride 1 MiB).
+template <bool RT, int NCH, int NG, int NST, bool NORM, int TC>
+__global__ void __launch_bounds__(NG* NCH* TC + 96, 1)
 k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, double* __restrict__ partial,
          unsigned int* ticket, double* __restrict__ scal, double dV) {
     typedef typename CnCoef<RT>::type CT;
-    constexpr int N = NCH * CN_L, GT = NCH * TCOLS, TILE = N * TCOLS, STAGE_BYTES = TILE * (int)sizeof(cd);
+    constexpr int N = NCH * CN_L, GT = NCH * TC, TILE = N * TC, STAGE_BYTES = TILE * (int)sizeof(cd);
     constexpr int NT = NG * GT + 96;
     extern __shared__ __align__(1024) unsigned char smraw[];
     __shared__ double red[32];
@@ -168,7 +172,7 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
     const int nmine = (tg.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     double acc = 0.0;
     if (tid < NG * GT) {
-        const int g = tid / GT, r = tid % GT, col = r % TCOLS, c = r / TCOLS, j0 = c * CN_L;
+        const int g = tid / GT, r = tid % GT, col = r % TC, c = r / TC, j0 = c * CN_L;
         const int t0 = j0 + c;      // chunk c of the padded tables
         cd* myends = ends + g * 2 * GT;
         for (int i = g; i < nmine; i += NG) {
@@ -178,21 +182,21 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
             cd* t = (cd*)(base + (size_t)s * STAGE_BYTES) + col;
             cd u[CN_L];
 #pragma unroll
-            for (int k = 0; k < CN_L; ++k) u[k] = t[(j0 + k) * TCOLS];
-            const cd lo = (c > 0) ? t[(j0 - 1) * TCOLS] : cmake(0.0, 0.0);
-            const cd hi = (c < NCH - 1) ? t[(j0 + CN_L) * TCOLS] : cmake(0.0, 0.0);
+            for (int k = 0; k < CN_L; ++k) u[k] = t[(j0 + k) * TC];
+            const cd lo = (c > 0) ? t[(j0 - 1) * TC] : cmake(0.0, 0.0);
+            const cd hi = (c < NCH - 1) ? t[(j0 + CN_L) * TC] : cmake(0.0, 0.0);
             cn_chunk_forward<CT>(u, lo, hi, cs.kap, cs.h + t0);
-            myends[c * TCOLS + col] = u[CN_L - 1];
+            myends[c * TC + col] = u[CN_L - 1];
             named_bar_sync(1 + g, GT);
-            const cd din = cn_carry_forward<CT>(c, myends + col, TCOLS, cs.pfe);
+            const cd din = cn_carry_forward<CT>(c, myends + col, TC, cs.pfe);
             cn_chunk_backward<CT>(u, din, cs.h + t0, cs.pf + t0);
-            myends[GT + c * TCOLS + col] = u[0];
+            myends[GT + c * TC + col] = u[0];
             named_bar_sync(1 + g, GT);
-            const cd uin = cn_carry_backward<CT>(c, NCH, myends + GT + col, TCOLS, cs.pbs);
+            const cd uin = cn_carry_backward<CT>(c, NCH, myends + GT + col, TC, cs.pbs);
             cn_chunk_fix<CT>(u, uin, cs.pb + t0);
 #pragma unroll
             for (int k = 0; k < CN_L; ++k) {
-                t[(j0 + k) * TCOLS] = u[k];
+                t[(j0 + k) * TC] = u[k];
                 if (NORM) acc += cnorm2(u[k]);
             }
             fence_proxy_async();
@@ -360,6 +364,7 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
     const int np = h->nplanes;
     rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Y], h->psi, 2LL * h->nx, h->ny, np, 2 * TCOLS, by, 1);
     rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Z], h->psi, 2LL * h->nx, h->ny, np, 2 * TCOLS, 1, bz);
+    if (h->ny % 2 == 0) rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_Z2], h->psi, 2LL * h->nx, h->ny, np, 2 * TCOLS, 2, bz);
     rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Y], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, by, 1);
     rc |= make_map((CUtensorMap*)h->tmap[TM_SPEC_Z], h->spec, 2LL * h->nxhp, h->ny, np, 2 * TCOLS, 1, bz);
     {   // the folded V_dd table, boxes along the last axis (rows 0 .. N/2; fmi_vrows)
@@ -384,6 +389,7 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
 static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int nzs) {
     TileGeom tg;
     tg.rev = h->rev_next;
+    tg.ystep = 1;
     const int row_elems = sp ? h->nxhp : h->nx;          // a pass over the half spectrum or over psi
     tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
     tg.pol_st = h->pol[sp ? POL_FFT_ST : POL_CN_ST];
@@ -402,16 +408,17 @@ static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int n
 
 static int grid_of(const dbec_handle_s* h, int ntiles) { return ntiles < h->num_sms ? ntiles : h->num_sms; }
 
-template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
-    constexpr int GT = NCH * TCOLS, STAGE = NCH * CN_L * TCOLS * (int)sizeof(cd);
-    const TileGeom tg = geom_of(h, axis, false, z0, nzs);
+template <bool RT, int NCH, int NG, int NST, bool NORM, int TC = TCOLS> static int launch_cn_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
+    constexpr int GT = NCH * TC, STAGE = NCH * CN_L * TC * (int)sizeof(cd);
+    TileGeom tg = geom_of(h, axis, false, z0, nzs);
+    if (TC == 2 * TCOLS) { tg.ystep = 2; tg.ntiles = tg.ntiles_x * (h->ny / 2); }
     const int grid = grid_of(h, tg.ntiles);
     if (NORM && (grid > h->npartial || h->nb > 1)) return (int)cudaErrorInvalidValue;   // a CTA's tiles span members
     const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 4) * sizeof(uint64_t) +
                       (3 * cn_tab_elems(NCH * CN_L) + 2 * NCH) * sizeof(typename CnCoef<RT>::type);
-    auto k = k_cn_tma<RT, NCH, NG, NST, NORM>;
+    auto k = k_cn_tma<RT, NCH, NG, NST, NORM, TC>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_PSI_Y : TM_PSI_Z];
+    const CUtensorMap* map = (const CUtensorMap*)h->tmap[axis == 1 ? TM_PSI_Y : TC == 2 * TCOLS ? TM_PSI_Z2 : TM_PSI_Z];
     CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, *map, make_cntab<RT>(h->ax[axis]), tg, h->partial,
                   h->ticket, h->scal, h->dV));
     h->launches++;
@@ -420,11 +427,20 @@ template <bool RT, int NCH, int NG, int NST, bool NORM> static int launch_cn_tma
 
 template <bool RT, bool NORM> static int launch_cn_tma_n(dbec_handle_s* h, int axis, int z0, int nzs) {
     switch (h->ax[axis].n) {
-        case 128: return launch_cn_tma<RT, 8, 4, 12, NORM>(h, axis, z0, nzs);     // 16 KiB tiles
-        case 256: return launch_cn_tma<RT, 16, 3, 6, NORM>(h, axis, z0, nzs);     // 32 KiB tiles
+        case 128:
+            if (axis == 2 && dbec_zpair_tiles(h)) return launch_cn_tma<RT, 8, 3, 6, NORM, 2 * TCOLS>(h, axis, z0, nzs);    // 32 KiB tiles
+            return launch_cn_tma<RT, 8, 4, 12, NORM>(h, axis, z0, nzs);     // 16 KiB tiles
+        case 256:
+            if (axis == 2 && dbec_zpair_tiles(h)) return launch_cn_tma<RT, 16, 1, 3, NORM, 2 * TCOLS>(h, axis, z0, nzs);   // 64 KiB tiles
+            return launch_cn_tma<RT, 16, 3, 6, NORM>(h, axis, z0, nzs);     // 32 KiB tiles
         case 512: return launch_cn_tma<RT, 32, 1, 3, NORM>(h, axis, z0, nzs);     // 64 KiB tiles
         default: return (int)cudaErrorInvalidValue;
     }
+}
+
+// z sweeps on tiles of 8 columns x 2 rows of y: planes at least 2 MiB apart
+int dbec_zpair_tiles(const dbec_handle_s* h) {
+    return h->p.ndim == 3 && h->nb == 1 && h->ny % 2 == 0 && (long long)h->nx * h->ny * (long long)sizeof(cd) >= h->zpair_min_stride;
 }
 
 int dbec_tma_supported(const dbec_handle_s* h, int axis) {

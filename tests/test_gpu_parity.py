@@ -281,6 +281,26 @@ def test_graph_and_plain_launches_agree_bitwise(gp, monkeypatch):
     assert np.array_equal(outs[0], outs[1])
 
 
+@pytest.mark.parametrize("w", [grid3(512, 256, 128, REAL), grid3(512, 256, 128, IMAG, d=(0.4, 0.3, 0.6)), grid3(256, 512, 256, REAL)], ids=wid)
+def test_z_sweep_on_paired_row_tiles(gp, ob, w):
+    """xy planes of 2 MiB or more: the z sweep works on tiles of 8 columns x 2 rows of y (k_cn_tma with TC = 16;
+    C5 is the only BASELINE.json config that gets there, in imaginary time with 256 points along z)."""
+    psi0 = random_psi(w, 17)
+    p = ob.params_of(w)
+    sim = gp.Dbec(gp.params_of(w))
+    sim.set_psi(psi0)
+    sim.cn_sweep(2)
+    assert relerr(sim.get_psi(), ob.cn_sweep(p, psi0, 2)) < PSI_TOL
+    sim.set_psi(psi0)
+    sim.step(1)
+    o = ob.Oracle(p)
+    o.set_psi(psi0)
+    o.step(1)
+    assert relerr(sim.get_psi(), o.get_psi()) < PSI_TOL
+    sim.close()
+    o.close()
+
+
 CLUSTER_CASES = [grid3(32, 32, 32, IMAG), grid3(32, 32, 32, REAL), grid3(16, 16, 16, REAL), grid3(64, 16, 32, IMAG, d=(0.4, 0.3, 0.6)),
                  grid3(48, 20, 12, IMAG, d=(0.4, 0.3, 0.6)), grid3(50, 14, 6, REAL), grid3(12, 10, 6, IMAG), grid3(128, 32, 16, REAL),
                  grid3(16, 64, 64, IMAG), grid2(64, 32, REAL, dx=0.2, dy=0.3), grid2(256, 256, IMAG), grid2(96, 80, REAL, plane=1),
