@@ -374,10 +374,10 @@ int dbec_make_tensor_maps(dbec_handle_s* h) {
             else rc |= make_map((CUtensorMap*)h->tmap[TM_VDD], h->vdd, h->nxhp, h->nyf, 1, TCOLS, fmi_vrows(nl), 1);
         }
     }
-    if (h->nx == 128 || h->nx == 256) {
-        // kernels_xwarp.cu: an x-line as NX/8 rows of 128 bytes (8 complex), a box = all rows of 2 (NX = 256) or
+    if (h->nx == 128 || h->nx == 256 || h->nx == 512) {
+        // kernels_xwarp.cu: an x-line as NX/8 rows of 128 bytes (8 complex), a box = all rows of 2 (NX = 256, 512) or
         // 4 (NX = 128) lines, 16-byte units of a row rotated by the row index (SWIZZLE_128B)
-        const int lpt = h->nx == 256 ? 2 : 4;
+        const int lpt = h->nx == 128 ? 4 : 2;
         rc |= make_map((CUtensorMap*)h->tmap[TM_PSI_XW], h->psi, 16, h->nx / 8, (long long)h->ny * np, 16, h->nx / 8, lpt, true);
     }
     return rc ? (int)cudaErrorInvalidValue : 0;

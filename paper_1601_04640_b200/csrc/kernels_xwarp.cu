@@ -262,6 +262,222 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
 }
 
 // ------------------------------------------------------------------------------------------------
+// lines of 512 points: TWO warps per line pair
+// ------------------------------------------------------------------------------------------------
+// A pair of 512-point lines is 16 KiB of psi plus 9 KiB of spectrum / exchange: with one warp per pair only seven
+// warps' worth of stages fit.  Here the two warps of a group share the pair: the 64 threads run the pair's inverse
+// transform together (V = 8, T = 64: the exchanges are 64-thread named barriers), then each warp takes ONE line:
+// a lane holds chunks `lane` and `lane + 32` of it (8 points each), calcnu and calclux as in k_xwarp_nonlin, the
+// neighbours, chunk ends and carries crossing between the two halves by rotating shuffles.
+typedef FftPlanV<8, 8, 8> WPlan512;
+
+__device__ __forceinline__ cd shfl_rot_cd(cd v, int src) {
+    return cmake(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+
+template <bool RT, int NG, int NST>
+__global__ void __launch_bounds__((2 * NG + 3) * 32, 1)
+k_xwarp2_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict__ spec, const cd* __restrict__ twN_g,
+                const double* __restrict__ scal, const double* __restrict__ vx_g, const double* __restrict__ vy,
+                const double* __restrict__ vz, double dt, int ntiles, int ny, int nz, int nb, CnTabW<RT> cn, int rev,
+                float pol_ld, float pol_st, float pol_spec) {
+    typedef typename CnCoef<RT>::type CT;
+    typedef WPlan512 P;
+    constexpr int N = 512, NLW_C = NlwBatch<RT>::C;
+    constexpr int T = P::T;                                          // 64 threads per pair
+    constexpr int CPL = N / WL;                                      // 64 chunks per line: two per lane
+    constexpr int NXHP = w_nxhp(N);
+    constexpr int NTAB = N + N / 8;
+    constexpr int PAIR_EL = w_pair_el(P::SMEM, NXHP, NTAB);
+    constexpr int NPD = N + N / 4;
+    constexpr int PSI_BYTES = 2 * N * (int)sizeof(cd), SLOT_BYTES = PAIR_EL * (int)sizeof(cd);
+    static_assert(PSI_BYTES % 1024 == 0, "the swizzle pattern needs 1024-byte aligned psi tiles");
+    constexpr int NW = 2 * NG, NT = (NW + 3) * 32;
+    extern __shared__ __align__(1024) unsigned char smraw[];
+    unsigned char* base = smraw;
+    unsigned char* slots = base + (size_t)NST * PSI_BYTES;
+    cd* tw = (cd*)(slots + (size_t)NST * SLOT_BYTES);            // twA [N], tw2 [T]
+    CT* tab = (CT*)(tw + N + T);                                 // h, PF, PB (padded), PFE, PBS
+    double* vxs = (double*)(tab + 3 * NTAB + 2 * CPL);
+    uint64_t* bars = (uint64_t*)(vxs + NPD);
+    uint64_t* full = bars; uint64_t* empty = bars + NST; uint64_t* done = bars + 2 * NST;
+    int* issued = (int*)(bars + 3 * NST);
+    const int tid = threadIdx.x;
+    for (int k = tid; k < N; k += NT) {
+        tw[k] = twN_g[((k % T) * (k / T)) % N];                  // twA[k1*T + m] = W_N^{m k1}
+        if (k < T) tw[N + k] = twN_g[(P::V * (k % P::R3) * (k / P::R3)) % N];   // tw2[k2*R3 + n3] = W_N^{V n3 k2}
+        vxs[padd(k)] = dt * vx_g[k];
+        tab[padt(k)] = cn.h[k]; tab[NTAB + padt(k)] = cn.pf[k]; tab[2 * NTAB + padt(k)] = cn.pb[k];
+    }
+    for (int k = tid; k < CPL; k += NT) { tab[3 * NTAB + k] = cn.pfe[k]; tab[3 * NTAB + CPL + k] = cn.pbs[k]; }
+    if (tid == 0) {
+        *issued = 0;
+        for (int s = 0; s < NST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); mbar_init(done + s, 2); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    pdl_launch_dependents();
+    pdl_wait();
+    const int nmine = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto tile_of = [&](int i) {
+        const long long t = (long long)blockIdx.x + (long long)i * gridDim.x;
+        return rev ? (long long)ntiles - 1 - t : t;
+    };
+    const int warp = tid >> 5, lane = tid & 31;
+    if (warp < NW) {
+        const cd* twA = tw; const cd* tw2 = tw + N;
+        const CT* th = tab; const CT* tpf = tab + NTAB; const CT* tpb = tab + 2 * NTAB;
+        const CT* pfe = tab + 3 * NTAB; const CT* pbs = pfe + CPL;
+        const CT kap = cn.kap;
+        const int K = cn.K;
+        const int g = warp >> 1, sub = warp & 1;                     // group, and this warp's line of the pair
+        const int m = tid - g * 64;                                  // FFT thread of the pair
+        const int c0 = lane, c1 = lane + 32;                         // this lane's two chunks of the line
+        double s = scal[SC_S];
+        double dtG = dt * (scal[SC_G] * scal[SC_S2]), dtD = dt * scal[SC_D];
+        for (int i = g; i < nmine; i += NG) {
+            const int st = i % NST;
+            const int row = (int)(tile_of(i) * 2) + sub;
+            const double vr = dt * (vy[row % ny] + vz[(row / ny) % nz]);
+            if (nb > 1) {
+                const double* sc = scal + (size_t)(row / (ny * nz)) * SC_COUNT;
+                s = sc[SC_S]; dtG = dt * (sc[SC_G] * sc[SC_S2]); dtD = dt * sc[SC_D];
+            }
+            wait_issued(issued, i);
+            mbar_wait(full + st, (i / NST) & 1);
+            cd* ps = (cd*)(base + (size_t)st * PSI_BYTES);
+            cd* sa = (cd*)(slots + (size_t)st * SLOT_BYTES);
+            // ---- inverse transform of the pair's spectrum by the group's 64 threads
+            {
+                const cd* sb = sa + NXHP;
+                cd v[P::V];
+#pragma unroll
+                for (int j = 0; j < P::V; ++j) {
+                    const int k = j * T + m;
+                    if (k <= N / 2) {
+                        const cd a = sa[k], b = sb[k];
+                        v[j] = cmake(a.x - b.y, a.y + b.x);          // X_a + i X_b
+                    } else {
+                        const cd a = sa[N - k], b = sb[N - k];
+                        v[j] = cmake(a.x + b.y, b.x - a.y);          // conj X_a + i conj X_b
+                    }
+                }
+                named_bar_sync(1 + g, 64);                           // the rows are in registers: reuse their area
+                fftv_stage1<P, +1>(v, m, twA);
+                fftv_x1_write<P>(v, m, sa);
+                named_bar_sync(1 + g, 64);
+                fftv_stage2<P, +1>(v, m, sa, tw2);
+                named_bar_sync(1 + g, 64);
+                fftv_x2_write<P>(v, m, sa);
+                named_bar_sync(1 + g, 64);
+                fftv_stage3<P, +1>(v, m, sa);
+                named_bar_sync(1 + g, 64);
+#pragma unroll
+                for (int j = 0; j < P::V; ++j) sa[padt(j * T + m)] = v[j];       // (Phi line a, Phi line b) at x
+            }
+            named_bar_sync(1 + g, 64);
+            // ---- calcnu on this warp's line: chunks c0 and c1 in registers u0, u1
+            cd u0[WL], u1[WL];
+            cd* p0 = ps + sub * N + c0 * WL;
+            cd* p1 = ps + sub * N + c1 * WL;
+            const int sw = lane & 7;                                 // (c0 & 7 == c1 & 7)
+#pragma unroll
+            for (int k = 0; k < WL; ++k) { u0[k] = p0[k ^ sw]; u1[k] = p1[k ^ sw]; }
+            {
+                const cd* ph0 = sa + padt(c0 * WL);
+                const cd* ph1 = sa + padt(c1 * WL);
+                const double* vx0 = vxs + padd(c0 * WL);
+                const double* vx1 = vxs + padd(c1 * WL);
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+#pragma unroll
+                    for (int k0 = 0; k0 < WL; k0 += NLW_C) {
+                        cd* u = half ? u1 : u0;
+                        const cd* ph = half ? ph1 : ph0;
+                        const double* vxc = half ? vx1 : vx0;
+                        double a[NLW_C];
+#pragma unroll
+                        for (int kk = 0; kk < NLW_C; ++kk) {
+                            const cd f = ph[k0 + kk];
+                            a[kk] = fma(dtD, sub ? f.y : f.x, vxc[k0 + kk] + vr);
+                            a[kk] = fma(dtG, cnorm2(u[k0 + kk]), a[kk]);
+                        }
+#pragma unroll
+                        for (int kk = 0; kk < NLW_C; ++kk) {
+                            if (RT) {
+                                double sn, cs_;
+                                sincos_cw(a[kk], &sn, &cs_);
+                                u[k0 + kk] = cmul(s, cmul(u[k0 + kk], cmake(cs_, -sn)));
+                            } else {
+                                u[k0 + kk] = cmul(s * exp_cw(-a[kk]), u[k0 + kk]);
+                            }
+                        }
+                    }
+                }
+            }
+            // ---- calclux on 64 chunks: chunk lane (u0) and chunk lane + 32 (u1)
+            const cd zero = cmake(0.0, 0.0);
+            const int up = (lane + 31) & 31, dn = (lane + 1) & 31;
+            {
+                const cd a = shfl_rot_cd(u0[WL - 1], up), b = shfl_rot_cd(u1[WL - 1], up);
+                const cd c = shfl_rot_cd(u1[0], dn), d = shfl_rot_cd(u0[0], dn);
+                const cd lo0 = lane > 0 ? a : zero, lo1 = lane > 0 ? b : a;      // chunk 32 follows chunk 31 (lane 31's u0)
+                const cd hi0 = lane < 31 ? d : c, hi1 = lane < 31 ? c : zero;    // chunk 31 precedes chunk 32 (lane 0's u1)
+                cn_chunk_forward<CT>(u0, lo0, hi0, kap, th + padt(c0 * WL));
+                cn_chunk_forward<CT>(u1, lo1, hi1, kap, th + padt(c1 * WL));
+            }
+            cd d0 = zero, d1 = zero;
+            for (int q = K; q >= 1; --q) {                           // D_in = e[c-1] + pfe[c-1] (e[c-2] + pfe[c-2] (...))
+                const int src = (lane - q) & 31;
+                const cd r0 = shfl_rot_cd(u0[WL - 1], src), r1 = shfl_rot_cd(u1[WL - 1], src);
+                if (lane >= q) d0 = cn_fma(pfe[c0 - q], d0, r0);
+                d1 = cn_fma(pfe[c1 - q], d1, lane >= q ? r1 : r0);
+            }
+            cn_chunk_backward<CT>(u0, d0, th + padt(c0 * WL), tpf + padt(c0 * WL));
+            cn_chunk_backward<CT>(u1, d1, th + padt(c1 * WL), tpf + padt(c1 * WL));
+            cd w0 = zero, w1 = zero;
+            for (int q = K; q >= 1; --q) {                           // U_in = e[c+1] + pbs[c+1] (e[c+2] + ...)
+                const int src = (lane + q) & 31;
+                const cd r0 = shfl_rot_cd(u0[0], src), r1 = shfl_rot_cd(u1[0], src);
+                w0 = cn_fma(pbs[c0 + q], w0, lane + q < 32 ? r0 : r1);
+                if (lane + q < 32) w1 = cn_fma(pbs[c1 + q], w1, r1);
+            }
+            cn_chunk_fix<CT>(u0, w0, tpb + padt(c0 * WL));
+            cn_chunk_fix<CT>(u1, w1, tpb + padt(c1 * WL));
+#pragma unroll
+            for (int k = 0; k < WL; ++k) { p0[k ^ sw] = u0[k]; p1[k ^ sw] = u1[k]; }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(done + st);
+        }
+    } else if (tid == NW * 32) {
+        const uint64_t pol = l2_policy_code(pol_spec), polp = l2_policy_code(pol_ld);
+        for (int i = 0; i < nmine; ++i) {
+            const int st = i % NST;
+            if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            st_release_shared(issued, i + 1);
+            mbar_expect_tx(full + st, PSI_BYTES + 2 * NXHP * (int)sizeof(cd));
+            const long long tile = tile_of(i);
+            tma_load_3d_hint(base + (size_t)st * PSI_BYTES, &map_psi, 0, 0, (int)(tile * 2), full + st, polp);
+            bulk_load_hint(slots + (size_t)st * SLOT_BYTES, spec + tile * 2 * NXHP, 2 * NXHP * (int)sizeof(cd), full + st, pol);
+        }
+    } else if (tid == (NW + 1) * 32 || tid == (NW + 2) * 32) {
+        const int which = warp - NW - 1;
+        const uint64_t polp = l2_policy_code(pol_st);
+        for (int i = 0; i < nmine; ++i) {
+            const int st = i % NST;
+            if ((st & 1) != which) continue;
+            mbar_wait(done + st, (i / NST) & 1);
+            tma_store_3d_hint(&map_psi, 0, 0, (int)(tile_of(i) * 2), base + (size_t)st * PSI_BYTES, polp);
+            bulk_commit();
+            bulk_wait_read<0>();
+            mbar_arrive(empty + st);
+        }
+        bulk_wait<0>();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
 template <bool RT> static CnTabW<RT> make_cntabw(const AxisTables& a);
@@ -274,8 +490,11 @@ template <> CnTabW<false> make_cntabw<false>(const AxisTables& a) {
 }
 
 int dbec_xwarp_supported(const dbec_handle_s* h) {
-    const int lpt = h->nx == 256 ? 2 : 4;
-    return h->use_tma && h->fuse_cnx && (h->nx == 128 || h->nx == 256) && ((h->ny * h->nz) % lpt == 0) &&
+    const int lpt = h->nx == 128 ? 4 : 2;
+    // 512-point lines: the two-warps-per-pair kernel stages 45 KB of tables per CTA before its first tile; a grid
+    // with only a tile or two per SM (BASELINE.json's 512^2 config: 256 pairs) is served faster by k_xline_nonlin
+    if (h->nx == 512 && (long long)h->ny * h->nplanes / 2 < 8LL * h->num_sms) return 0;
+    return h->use_tma && h->fuse_cnx && (h->nx == 128 || h->nx == 256 || h->nx == 512) && ((h->ny * h->nz) % lpt == 0) &&
            h->ax[0].K8 >= 1 && h->ax[0].K8 <= 31;
 }
 
@@ -300,9 +519,31 @@ template <int N, bool RT, int NW, int NST> static int launch_xwarp(dbec_handle_s
     return (int)cudaGetLastError();
 }
 
+template <bool RT, int NG, int NST> static int launch_xwarp2(dbec_handle_s* h) {
+    typedef typename CnCoef<RT>::type CT;
+    typedef WPlan512 P;
+    constexpr int N = 512, NXHP = w_nxhp(N), CPL = N / WL;
+    constexpr int PAIR_EL = w_pair_el(P::SMEM, NXHP, N + N / 8);
+    constexpr int STAGE = 2 * N * (int)sizeof(cd) + PAIR_EL * (int)sizeof(cd);
+    if (h->nxhp != NXHP) return (int)cudaErrorInvalidValue;
+    const int ntiles = (int)((long long)h->ny * h->nplanes / 2);
+    const int grid = ntiles < h->num_sms ? ntiles : h->num_sms;
+    const size_t sm = (size_t)NST * STAGE + (N + P::T) * sizeof(cd) + (3 * (N + N / 8) + 2 * CPL) * sizeof(CT) +
+                      (N + N / 4) * sizeof(double) + (3 * NST + 1) * sizeof(uint64_t);
+    auto k = k_xwarp2_nonlin<RT, NG, NST>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const CUtensorMap* map = (const CUtensorMap*)h->tmap[TM_PSI_XW];
+    CK(launch_pdl(k, dim3(grid), dim3((2 * NG + 3) * 32), sm, h->stream, h->use_pdl, *map, (const cd*)h->spec, h->ax[0].twN,
+                  (const double*)h->scal, h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, h->nz, h->nb,
+                  make_cntabw<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]));
+    h->launches++;
+    return (int)cudaGetLastError();
+}
+
 int dbec_launch_xwarp_nonlin(dbec_handle_s* h) {
     const bool rt = h->p.time_mode == 1;
     switch (h->nx) {
+        case 512: return rt ? launch_xwarp2<true, 6, 7>(h) : launch_xwarp2<false, 6, 7>(h);
         case 128: return rt ? launch_xwarp<128, true, 12, 15>(h) : launch_xwarp<128, false, 12, 15>(h);
         case 256: return rt ? launch_xwarp<256, true, 12, 16>(h) : launch_xwarp<256, false, 12, 16>(h);
         default: return (int)cudaErrorInvalidValue;

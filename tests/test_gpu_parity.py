@@ -374,7 +374,8 @@ def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch):
         h.close()
 
 
-@pytest.mark.parametrize("shape,mode", [((256, 128, 256), REAL), ((128, 128, 128), IMAG), ((256, 256, 64), IMAG)])
+@pytest.mark.parametrize("shape,mode", [((256, 128, 256), REAL), ((128, 128, 128), IMAG), ((256, 256, 64), IMAG),
+                                        ((512, 64, 64), REAL), ((512, 256, 32), IMAG)])
 def test_persistent_kernels_are_bit_reproducible(gp, shape, mode):
     """The persistent loader / worker / storer kernels (kernels_tma.cu, kernels_xline.cu) hand stages over
     through mbarrier phase parities; a worker that ran a whole ring ahead once read a stage that was
