@@ -719,3 +719,25 @@ def test_full_run_observables_against_oracle_golden(gp, key):
             assert abs(a[k] - row[k]) <= OBS_TOL * abs(row[k]), (key, row["step"], k, a[k], row[k])
     assert done == w.steps
     sim.close()
+
+
+@pytest.mark.gpu
+def test_fp64_pipe_probe(tmp_path):
+    """Builds and runs tests/fp64_probe.cu: dependent-DFMA latency and DFMA throughput per SM, the two numbers
+    DESIGN.md section 6 sets beside the HBM roofline (profiles/r2_fp64_probe.md keeps one run's line)."""
+    import json
+    import shutil
+    import subprocess
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("no nvcc on this box")
+    exe = str(tmp_path / "fp64_probe")
+    src = os.path.join(os.path.dirname(__file__), "fp64_probe.cu")
+    subprocess.run([nvcc, "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, r.stdout + r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    print("fp64_probe", json.dumps(line))
+    assert line["cuda_error"] == 0
+    assert 4.0 <= line["dependent_dfma_latency_cycles"] <= 16.0
+    assert 16.0 <= line["dfma_per_clk_per_sm"] <= 130.0
