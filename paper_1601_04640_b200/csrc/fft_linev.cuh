@@ -28,9 +28,12 @@ template <int V_, int R2_, int R3_> struct FftPlanV {
 
 // Stage-2 exchange position of entry (p, n3).  R3 = 4: rows of 4 x 16 bytes; rotating the entry index by
 // bits 1..2 of the row puts the 8 rows a quarter warp touches (writes: 2 rows x 4 entries; reads: 8 rows, same
-// entry) into 8 different 16-byte bank groups.  R3 = 2: rows of 2, rotation by bit 2 of the row.
+// entry) into 8 different 16-byte bank groups.  R3 = 2: rows of 2, rotation by bit 2 of the row.  R3 = 8: rows of
+// 8 x 16 bytes = all bank groups; rotating by the row index keeps a row's writes a permutation of the row and sends
+// the 8 rows a quarter warp reads (same entry) to 8 different groups (plain: an 8-way conflict).
 template <class P> DBEC_HD int x2_pos(int p, int n3) {
-    return P::R3 == 4 ? p * 4 + (n3 ^ ((p >> 1) & 3)) : P::R3 == 2 ? p * 2 + (n3 ^ ((p >> 2) & 1)) : p * P::R3 + n3;
+    return P::R3 == 8 ? p * 8 + ((n3 + p) & 7)
+         : P::R3 == 4 ? p * 4 + (n3 ^ ((p >> 1) & 3)) : P::R3 == 2 ? p * 2 + (n3 ^ ((p >> 2) & 1)) : p * P::R3 + n3;
 }
 
 template <int V, int S> DBEC_HD void dft_regs(cd (&v)[V]) { dft_small<V, S>(v); }
