@@ -131,7 +131,7 @@ inline bool make_plan_p(const GenPlan& g, GenPlanP* p) {
 }
 
 // One pass of the transform below: L lines, nb butterflies each.
-template <int R, int S, bool LFAST, bool FIRST>
+template <int R, int S, bool LFAST>
 __device__ __forceinline__ void gen_fft_pass(const cd* a, cd* b, int L, const FastDiv& fL, const FastDiv& fL0, int S0, int S1, int SE,
                                              int n, const GenPass& ps, const cd* __restrict__ twN) {
     const int nb = ps.nb, Ns = ps.Ns, tunit = ps.tunit;
@@ -141,36 +141,34 @@ __device__ __forceinline__ void gen_fft_pass(const cd* a, cd* b, int L, const Fa
         if (LFAST) fL.divmod(idx, j, l); else fnb.divmod(idx, l, j);
         fL0.divmod(l, lq, lr);
         const int off = lq * S1 + lr * S0;
-        if (FIRST) { k = 0; } else { fNs.divmod(j, jq, k); }
-        gen_butterfly_k<R, S, FIRST>(a + off, b + off, SE, j, k, Ns, nb, n, tunit * k, twN);
+        fNs.divmod(j, jq, k);
+        gen_butterfly_k<R, S, false>(a + off, b + off, SE, j, k, Ns, nb, n, tunit * k, twN);
     }
+}
+// the odd radices are rare: one out-of-line copy each keeps the calling kernel inside the instruction cache
+template <int R, int S, bool LFAST>
+__device__ __noinline__ void gen_fft_pass_odd(const cd* a, cd* b, int L, FastDiv fL, FastDiv fL0, int S0, int S1, int SE, int n,
+                                              GenPass ps, const cd* __restrict__ twN) {
+    gen_fft_pass<R, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, n, ps, twN);
 }
 
 // The same transform over L lines whose starts follow a two-level pattern: line l begins at
 // (l / L0) * S1 + (l % L0) * S0 (stacked planes of strided columns, or stacked rows), element stride SE.  Every
-// division is a multiply-high with constants from the host; twN may sit in shared memory.
+// division is a multiply-high with constants from the host.  Inlined into the caller, so that a, b and twN keep
+// their shared-memory address space (LDS / STS, not generic accesses) and the plan is read straight from the
+// kernel's parameter bank: through an out-of-line call with generic pointers a pass on a handful of lines took
+// ~900 cycles, most of it address-space and parameter overhead.
 template <int S, bool LFAST>
-__device__ __noinline__ cd* gen_fft_lines2(cd* a, cd* b, int L, FastDiv fL, FastDiv fL0, int S0, int S1, int SE, const GenPlanP* plp,
-                                           const cd* __restrict__ twN) {
-    const GenPlanP& pl = *plp;                       // (in shared memory: the kernel's own copy)
+__device__ __forceinline__ cd* gen_fft_lines2(cd* a, cd* b, int L, FastDiv fL, FastDiv fL0, int S0, int S1, int SE, const GenPlanP& pl,
+                                              const cd* __restrict__ twN) {
     for (int s = 0; s < pl.nfac; ++s) {
         const GenPass ps = pl.pass[s];
-        if (s == 0) {
-            switch (ps.r) {
-                case 2: gen_fft_pass<2, S, LFAST, true>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                case 3: gen_fft_pass<3, S, LFAST, true>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                case 4: gen_fft_pass<4, S, LFAST, true>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                case 5: gen_fft_pass<5, S, LFAST, true>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                default: gen_fft_pass<7, S, LFAST, true>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-            }
-        } else {
-            switch (ps.r) {
-                case 2: gen_fft_pass<2, S, LFAST, false>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                case 3: gen_fft_pass<3, S, LFAST, false>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                case 4: gen_fft_pass<4, S, LFAST, false>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                case 5: gen_fft_pass<5, S, LFAST, false>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-                default: gen_fft_pass<7, S, LFAST, false>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
-            }
+        switch (ps.r) {
+            case 2: gen_fft_pass<2, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
+            case 4: gen_fft_pass<4, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
+            case 3: gen_fft_pass_odd<3, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
+            case 5: gen_fft_pass_odd<5, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
+            default: gen_fft_pass_odd<7, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
         }
         __syncthreads();
         cd* t = a; a = b; b = t;

@@ -134,7 +134,6 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
     cd* twx = e1 + SMT; cd* twy = twx + nx; cd* twl = twy + (d3 ? ny : 0);
     CT* tcx = (CT*)(twl + nl); CT* tcy = tcx + 3 * npx; CT* tcl = tcy + (d3 ? 3 * npy : 0);
     double* vxs = (double*)(tcl + 3 * npl); double* vys = vxs + nx; double* vzs = vys + ny;
-    GenPlanP* plans = (GenPlanP*)(vzs + ((a.nz + 1) & ~1));
     for (int k = tid; k < nx; k += SMT) { twx[k] = a.twx[k]; vxs[k] = a.vx[k]; }
     for (int k = tid; k < ny; k += SMT) { if (d3) twy[k] = a.twy[k]; vys[k] = a.vy[k]; }
     for (int k = tid; k < a.nz; k += SMT) vzs[k] = a.vz[k];
@@ -142,16 +141,10 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
     for (int k = tid; k < npx; k += SMT) { tcx[k] = cnx_g.h[k]; tcx[npx + k] = cnx_g.pf[k]; tcx[2 * npx + k] = cnx_g.pb[k]; }
     if (d3) for (int k = tid; k < npy; k += SMT) { tcy[k] = cny_g.h[k]; tcy[npy + k] = cny_g.pf[k]; tcy[2 * npy + k] = cny_g.pb[k]; }
     for (int k = tid; k < npl; k += SMT) { tcl[k] = cnl_g.h[k]; tcl[npl + k] = cnl_g.pf[k]; tcl[2 * npl + k] = cnl_g.pb[k]; }
-    {
-        const int* src[3] = {(const int*)&a.px, (const int*)&a.py, (const int*)&a.pl};
-        constexpr int W = (int)(sizeof(GenPlanP) / sizeof(int));
-        for (int k = tid; k < 3 * W; k += SMT) ((int*)plans)[k] = src[k / W][k % W];
-    }
     CnTab<RT> cnx = cnx_g, cny = cny_g, cnl = cnl_g;
     cnx.h = tcx; cnx.pf = tcx + npx; cnx.pb = tcx + 2 * npx;
     cny.h = tcy; cny.pf = tcy + npy; cny.pb = tcy + 2 * npy;
     cnl.h = tcl; cnl.pf = tcl + npl; cnl.pb = tcl + 2 * npl;
-    const GenPlanP* ppx = plans; const GenPlanP* ppy = plans + 1; const GenPlanP* ppl = plans + 2;
     const FastDiv fnx(nx), fnxh1(nxh1), fny(ny), fone(1);
     const long long ls_spec = a.ndim == 3 ? (long long)ny * nxhp : nxhp;       // last-axis strides
     const long long ls_psi = a.ndim == 3 ? (long long)ny * nx : nx;
@@ -183,7 +176,7 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
                     A[idx] = cmake(s2 * cnorm2(p0), s2 * cnorm2(p1));
                 }
                 __syncthreads();
-                const cd* z = gen_fft_lines2<-1, false>(A, B, np, fone, FastDiv(np), nx, 0, 1, ppx, twx);
+                const cd* z = gen_fft_lines2<-1, false>(A, B, np, fone, FastDiv(np), nx, 0, 1, a.px, twx);
                 cd* o = (z == A) ? B : A;
                 for (int idx = tid; idx < np * nxh1; idx += SMT) {
                     int l, k;
@@ -195,7 +188,7 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
                 }
                 __syncthreads();
                 const cd* r = o;
-                if (a.ndim == 3) r = gen_fft_lines2<-1, true>(o, (cd*)z, nu * nxh1, FastDiv(nu * nxh1), fnxh1, 1, ny * nxh1, nxh1, ppy, twy);
+                if (a.ndim == 3) r = gen_fft_lines2<-1, true>(o, (cd*)z, nu * nxh1, FastDiv(nu * nxh1), fnxh1, 1, ny * nxh1, nxh1, a.py, twy);
                 cd* gs = spec + r0 * nxhp;
                 for (int idx = tid; idx < nrows * nxh1; idx += SMT) {
                     int row, k;
@@ -216,7 +209,7 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
                     A[idx] = ldcg2(spec + (long long)j * ls_spec + y * nxhp + k);
                 }
                 __syncthreads();
-                cd* r = gen_fft_lines2<-1, true>(A, B, w, fw, fw, 1, 0, w, ppl, twl);
+                cd* r = gen_fft_lines2<-1, true>(A, B, w, fw, fw, 1, 0, w, a.pl, twl);
                 cd* o = (r == A) ? B : A;
                 for (int idx = tid; idx < nl * w; idx += SMT) {
                     int j, c, y, k;
@@ -227,7 +220,7 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
                     r[idx] = cmul(a.vdd[base + (long long)(j < nl - j ? j : nl - j) * vls], r[idx]);
                 }
                 __syncthreads();
-                r = gen_fft_lines2<+1, true>(r, o, w, fw, fw, 1, 0, w, ppl, twl);
+                r = gen_fft_lines2<+1, true>(r, o, w, fw, fw, 1, 0, w, a.pl, twl);
                 for (int idx = tid; idx < nl * w; idx += SMT) {
                     int j, c, y, k;
                     fw.divmod(idx, j, c);
@@ -255,7 +248,7 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
                 }
                 __syncthreads();
                 cd* r = A;
-                if (a.ndim == 3) r = gen_fft_lines2<+1, true>(A, B, nu * nxh1, FastDiv(nu * nxh1), fnxh1, 1, ny * nxh1, nxh1, ppy, twy);
+                if (a.ndim == 3) r = gen_fft_lines2<+1, true>(A, B, nu * nxh1, FastDiv(nu * nxh1), fnxh1, 1, ny * nxh1, nxh1, a.py, twy);
                 cd* o = (r == A) ? B : A;
                 for (int idx = tid; idx < np * nx; idx += SMT) {
                     int l, k;
@@ -268,7 +261,7 @@ k_small_step(const __grid_constant__ SmallArgs a, CnTab<RT> cnx_g, CnTab<RT> cny
                     o[idx] = v;
                 }
                 __syncthreads();
-                const cd* f = gen_fft_lines2<+1, false>(o, r, np, fone, FastDiv(np), nx, 0, 1, ppx, twx);   // (Phi line 2l, Phi line 2l+1)
+                const cd* f = gen_fft_lines2<+1, false>(o, r, np, fone, FastDiv(np), nx, 0, 1, a.px, twx);   // (Phi line 2l, Phi line 2l+1)
                 {
                     const double s = sc[SC_S], s2 = sc[SC_S2], G = sc[SC_G], D = sc[SC_D], dt = a.dt;
                     for (int idx = tid; idx < nrows * nx; idx += SMT) {
