@@ -364,11 +364,21 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     h->use_graph = ge ? atoi(ge) : 1;
     h->use_rev = 1; h->use_pdl = 1; h->use_tma = 1;
     h->zpair_min_stride = 2LL << 20;
-    {   // L2 eviction policy per access site: the outputs of the two x-line kernels are kept evict-last (the
-        // passes after them find part of the spectrum / of psi in L2), their dead inputs evict-first,
-        // everything else a neutral hint (measured alternatives: profiles/r1d_step_ncu_full.md)
-        const float def[POL_COUNT] = {0.f, 0.f, 0.f, 1.f, 2.f, 2.f, 1.f, 0.f, 0.f};
-        for (int i = 0; i < POL_COUNT; ++i) h->pol[i] = def[i];
+    {   // Pacing of the streaming passes (tma_pipe.cuh: pace_wait).  The schedule interval is set by the THEORETICAL
+        // DRAM bandwidth (B200: 2 x 3996 MHz x 7680 bit = 7672 GB/s), which no pass reaches: every CTA is then
+        // "late", publishes its lag, and the loaders issue tile i when the slowest CTA of the launch has issued its
+        // own — lockstep at whatever rate the memory delivers, with no tuned constant.  Scanned on B200: 5600 ...
+        // 6600 GB/s has a sharp optimum at 6200 without the shared lag; with it, anything from 6800 up gives the
+        // same step time (C5 2.25 -> 2.00 ms, C4 491 -> 478 us).  DBEC_PACE (GB/s; 0 = off) is the tests' switch.
+        int khz = 0, bits = 0, l2 = 0;
+        cudaDeviceGetAttribute(&khz, cudaDevAttrMemoryClockRate, dev);
+        cudaDeviceGetAttribute(&bits, cudaDevAttrGlobalMemoryBusWidth, dev);
+        cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+        h->l2_bytes = l2;
+        h->pace_gbs = 2.0 * (double)khz * 1e3 * (double)bits / 8.0 / 1e9;
+        h->pace_head_speed = 0.5;
+        const char* pe = getenv("DBEC_PACE");
+        if (pe) h->pace_gbs = atof(pe);
     }
     // the legacy default stream cannot be captured: plain launches there
     if (h->stream == nullptr || h->stream == cudaStreamLegacy) h->use_graph = 0;

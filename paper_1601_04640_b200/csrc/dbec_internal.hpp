@@ -47,6 +47,14 @@ __device__ __forceinline__ void ramp_advance(double* __restrict__ sc) {
 }
 #endif
 
+// Pacing of the streaming passes (tma_pipe.cuh: pace_wait).  PaceState: one word per handle in the ticket block.
+struct PaceState { unsigned long long lag; unsigned int exits; unsigned int pad; };
+struct PaceArgs {
+    int ns;             // interval at which a loader issues its tiles, 0 = no pacing
+    int head, head_ns;  // the first `head` tiles of a CTA (they come out of L2) at this shorter interval
+    PaceState* st;
+};
+
 // Per-axis tables on the device.
 struct AxisTables {
     int n;                  // points along the axis
@@ -114,6 +122,9 @@ struct dbec_handle_s {
                                     // env DBEC_CLUSTER = 0 / 1 / 2 / 4 / 8 / 16 overrides the choice)
     int use_small;                  // 1: dbec_step runs k_small_step (use_cluster > 0)
     int small_max_clusters;         // clusters of k_small_step that can be resident at once (0: not asked yet)
+    double pace_gbs;                // bandwidth the streaming passes are paced to, GB/s (tma_pipe.cuh: pace_wait); 0 = off
+    long long l2_bytes;             // L2 cache size of the device
+    double pace_head_speed;         // time per tile of the L2-resident head of a pass relative to the paced time
     long long zpair_min_stride;     // z sweeps pair two rows of y per tile when the xy plane is at least this many bytes
     int use_pdl;                    // 1: programmatic dependent launch of every kernel of a step
     int rev_next;                   // the next persistent launch walks its tiles last to first (L2 reuse across passes)
@@ -150,6 +161,8 @@ int dbec_launch_gen_cn(dbec_handle_s* h, int axis, int with_norm);
 int dbec_make_tensor_maps(dbec_handle_s* h);
 int dbec_tma_supported(const dbec_handle_s* h, int axis);
 int dbec_zpair_tiles(const dbec_handle_s* h);
+// pacing of a launch of `grid` CTAs over `ntiles` tiles moving tile_bytes each while streaming a field of field_bytes
+PaceArgs dbec_pace_args(const dbec_handle_s* h, int ntiles, int grid, size_t tile_bytes, double field_bytes);
 int dbec_launch_fft_tma(dbec_handle_s* h, int axis, int mode, int z0, int nzs);
 int dbec_launch_cn_tma(dbec_handle_s* h, int axis, int with_norm, int z0, int nzs);
 // persistent bulk-copy-fed versions of the x passes (kernels_xline.cu)

@@ -30,6 +30,9 @@ struct TileGeom {
                      // fused y pass of a 2-D grid: 0 (the table has one plane, shared by the members of a batch)
     int vrows;       // rows of one V_dd box, boxes per tile
     int vnbox;
+    int pace_ns;     // interval at which the loader issues its tiles (tma_pipe.cuh: pace_wait; 0: no pacing)
+    int pace_head, pace_head_ns;   // the first pace_head tiles of a CTA, which come out of L2, at this shorter interval
+    PaceState* pace;               // the launch's shared lag word
     int ystep;       // z passes: rows of y per tile (1, or 2 when a tile is 8 columns x 2 rows of y: k_cn_tma with TC = 16)
     int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
     float pol_ld, pol_st;   // L2 eviction policy codes of the tile loads / stores (tma_pipe.cuh: l2_policy_code)
@@ -68,9 +71,11 @@ template <int NST, int STAGE_BYTES, int MAIN_BYTES, int EXTRA_BYTES, int EXTRA_T
 __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* stages, const CUtensorMap* map,
                                             const CUtensorMap* extra, const TileGeom& tg, int nmine) {
     const uint64_t pol = l2_policy_code(tg.pol_ld);
+    unsigned long long t0 = 0;
     for (int i = 0; i < nmine; ++i) {
         const int s = i % NST;
         if (i >= NST) mbar_wait(pb.empty + s, ((i / NST) - 1) & 1);
+        if (tg.pace_ns) pace_wait(t0, i, tg.pace_head, tg.pace_head_ns, tg.pace_ns, tg.pace);
         st_release_shared(pb.issued, i + 1);
         mbar_expect_tx(pb.full + s, MAIN_BYTES + EXTRA_TX);
         const int t = blockIdx.x + i * gridDim.x;
@@ -95,7 +100,7 @@ __device__ __forceinline__ void pipe_loader(const PipeBars& pb, unsigned char* s
                                       pb.full + s, polv);
             }
         }
-    }
+    }    if (tg.pace_ns) pace_done(tg.pace);
 }
 
 // Two storers, one for the even and one for the odd stages (which = 0 / 1): while one sits in
@@ -390,6 +395,7 @@ static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int n
     TileGeom tg;
     tg.rev = h->rev_next;
     tg.ystep = 1;
+    tg.pace_ns = 0; tg.pace_head = 0; tg.pace_head_ns = 0; tg.pace = nullptr;
     const int row_elems = sp ? h->nxhp : h->nx;          // a pass over the half spectrum or over psi
     tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
     tg.pol_st = h->pol[sp ? POL_FFT_ST : POL_CN_ST];
@@ -408,12 +414,36 @@ static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int n
 
 static int grid_of(const dbec_handle_s* h, int ntiles) { return ntiles < h->num_sms ? ntiles : h->num_sms; }
 
+// Pacing of a streaming pass (tma_pipe.cuh: pace_wait).  tile_bytes: what one tile reads and writes; field_bytes:
+// the field the pass streams.  The share of the field the previous pass left in L2 (about 0.8 of the cache, walked
+// first thanks to the alternating tile order) is scheduled at pace_head_speed of the paced interval; a field that fits
+// there is never paced.
+PaceArgs dbec_pace_args(const dbec_handle_s* h, int ntiles, int grid, size_t tile_bytes, double field_bytes) {
+    PaceArgs pa; pa.ns = 0; pa.head = 0; pa.head_ns = 0; pa.st = nullptr;
+    if (h->pace_gbs <= 0.0 || grid < 1) return pa;
+    const double head = 0.8 * (double)h->l2_bytes / field_bytes;
+    if (head >= 1.0) return pa;
+    const int per_cta = ntiles / grid;
+    if (per_cta < 8) return pa;
+    pa.ns = (int)((double)tile_bytes * grid / h->pace_gbs);
+    if (pa.ns < 1) pa.ns = 1;
+    pa.head = (int)(head * per_cta);
+    pa.head_ns = (int)(h->pace_head_speed * pa.ns);
+    pa.st = (PaceState*)(h->ticket + 16);          // 64 bytes into the ticket block
+    return pa;
+}
+static void set_pace(const dbec_handle_s* h, TileGeom* tg, int grid, size_t tile_bytes, double field_bytes) {
+    const PaceArgs pa = dbec_pace_args(h, tg->ntiles, grid, tile_bytes, field_bytes);
+    tg->pace_ns = pa.ns; tg->pace_head = pa.head; tg->pace_head_ns = pa.head_ns; tg->pace = pa.st;
+}
+
 template <bool RT, int NCH, int NG, int NST, bool NORM, int TC = TCOLS> static int launch_cn_tma(dbec_handle_s* h, int axis, int z0, int nzs) {
     constexpr int GT = NCH * TC, STAGE = NCH * CN_L * TC * (int)sizeof(cd);
     TileGeom tg = geom_of(h, axis, false, z0, nzs);
     if (TC == 2 * TCOLS) { tg.ystep = 2; tg.ntiles = tg.ntiles_x * (h->ny / 2); }
     const int grid = grid_of(h, tg.ntiles);
     if (NORM && (grid > h->npartial || h->nb > 1)) return (int)cudaErrorInvalidValue;   // a CTA's tiles span members
+    set_pace(h, &tg, grid, 2 * (size_t)STAGE, 16.0 * (double)h->P * h->nb);
     const size_t sm = 128 + (size_t)NST * STAGE + (size_t)NG * 2 * GT * sizeof(cd) + (3 * NST + 4) * sizeof(uint64_t) +
                       (3 * cn_tab_elems(NCH * CN_L) + 2 * NCH) * sizeof(typename CnCoef<RT>::type);
     auto k = k_cn_tma<RT, NCH, NG, NST, NORM, TC>;
@@ -466,8 +496,9 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
     typedef typename PlanS<N>::P P;
     constexpr int GT = P::T * TCOLS;
     constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? fmi_extra_bytes(N) : 0);
-    const TileGeom tg = geom_of(h, axis, true, z0, nzs);
+    TileGeom tg = geom_of(h, axis, true, z0, nzs);
     const int grid = grid_of(h, tg.ntiles);
+    set_pace(h, &tg, grid, (size_t)STAGE + N * TCOLS * sizeof(cd), 16.0 * (double)h->SP * h->nb);
     const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 4) * sizeof(uint64_t) + 2 * N * sizeof(cd);
     auto k = k_fft_tma<P, MODE, NG, NST>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));

@@ -244,7 +244,7 @@ template <class P, int XP, int NG, int NST>
 __global__ void __launch_bounds__(NG* XP* P::T + 96, 1)
 k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twA_g,
                 const cd* __restrict__ twN_g, double* __restrict__ scal, int ntiles, int tiles_per_member, int nb,
-                int advance, int rev, float pol_psi, float pol_spec) {
+                int advance, int rev, float pol_psi, float pol_spec, PaceArgs pace) {
     constexpr int XR = 2 * XP;
     constexpr int T = P::T, N = P::N, GT = XP * T, NT = NG * GT + 96;
     constexpr int NXHP = nxhp_of(N);
@@ -322,13 +322,16 @@ k_xline_density(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __r
         if (advance && blockIdx.x == 0)
             for (int b = 0; b < nb; ++b) ramp_advance(scal + (size_t)b * SC_COUNT);
         const uint64_t pol = l2_policy_code(pol_psi);
+        unsigned long long t0 = 0;
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            if (pace.ns) pace_wait(t0, i, pace);
             st_release_shared(issued, i + 1);
             mbar_expect_tx(full + st, STAGE_BYTES);
             bulk_load_hint(base + (size_t)st * STAGE_BYTES, psi + tile_of(i) * XR * N, STAGE_BYTES, full + st, pol);
         }
+        if (pace.ns) pace_done(pace.st);
     } else if (tid == NG * GT + 32 || tid == NG * GT + 64) {
         const int which = (tid - NG * GT) / 32 - 1;      // storer 0: even stages, storer 1: odd stages
         for (int i = 0; i < nmine; ++i) {
@@ -401,7 +404,8 @@ template <int N, int NG, int NST> static int launch_xline_density(dbec_handle_s*
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const long long row0 = (long long)z0 * h->ny;
     CK(launch_pdl(k, dim3(grid), dim3(NG * GT + 96), sm, h->stream, h->use_pdl, h->psi + row0 * N, h->spec + row0 * NXHP, h->ax[0].twA, h->ax[0].twN, h->scal,
-                                             ntiles, h->ny * h->nz / XR, h->nb, advance, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC]));
+                                             ntiles, h->ny * h->nz / XR, h->nb, advance, h->rev_next, h->pol[POL_D_PSI], h->pol[POL_D_SPEC],
+                                             dbec_pace_args(h, ntiles, grid, (size_t)XR * (N + NXHP) * sizeof(cd), 16.0 * (double)h->P * h->nb)));
     h->launches++;
     return (int)cudaGetLastError();
 }

@@ -64,7 +64,7 @@ __global__ void __launch_bounds__((NW + 3) * 32, 1)
 k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict__ spec, const cd* __restrict__ twN_g,
                const double* __restrict__ scal, const double* __restrict__ vx_g, const double* __restrict__ vy,
                const double* __restrict__ vz, double dt, int ntiles, int ny, int nz, int nb, CnTabW<RT> cn, int rev,
-               float pol_ld, float pol_st, float pol_spec) {
+               float pol_ld, float pol_st, float pol_spec, PaceArgs pace) {
     typedef typename CnCoef<RT>::type CT;
     typedef typename WPlan<N>::P P;
     constexpr int NLW_C = NlwBatch<RT>::C;
@@ -232,9 +232,11 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
         }
     } else if (tid == NW * 32) {
         const uint64_t pol = l2_policy_code(pol_spec), polp = l2_policy_code(pol_ld);
+        unsigned long long t0 = 0;
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            if (pace.ns) pace_wait(t0, i, pace);
             st_release_shared(issued, i + 1);
             mbar_expect_tx(full + st, PSI_BYTES + PAIRS * 2 * NXHP * (int)sizeof(cd));
             const long long tile = tile_of(i);
@@ -244,6 +246,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
                 bulk_load_hint(slots + (size_t)st * SLOT_BYTES + (size_t)pp * PAIR_EL * sizeof(cd),
                                spec + (tile * PAIRS + pp) * 2 * NXHP, 2 * NXHP * (int)sizeof(cd), full + st, pol);
         }
+        if (pace.ns) pace_done(pace.st);
     } else if (tid == (NW + 1) * 32 || tid == (NW + 2) * 32) {
         // two storers (even / odd stages): while one sits in wait_group.read, the other drains the next stage
         const int which = warp - NW - 1;
@@ -280,7 +283,7 @@ __global__ void __launch_bounds__((2 * NG + 3) * 32, 1)
 k_xwarp2_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict__ spec, const cd* __restrict__ twN_g,
                 const double* __restrict__ scal, const double* __restrict__ vx_g, const double* __restrict__ vy,
                 const double* __restrict__ vz, double dt, int ntiles, int ny, int nz, int nb, CnTabW<RT> cn, int rev,
-                float pol_ld, float pol_st, float pol_spec) {
+                float pol_ld, float pol_st, float pol_spec, PaceArgs pace) {
     typedef typename CnCoef<RT>::type CT;
     typedef WPlan512 P;
     constexpr int N = 512, NLW_C = NlwBatch<RT>::C;
@@ -452,15 +455,18 @@ k_xwarp2_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restric
         }
     } else if (tid == NW * 32) {
         const uint64_t pol = l2_policy_code(pol_spec), polp = l2_policy_code(pol_ld);
+        unsigned long long t0 = 0;
         for (int i = 0; i < nmine; ++i) {
             const int st = i % NST;
             if (i >= NST) mbar_wait(empty + st, ((i / NST) - 1) & 1);
+            if (pace.ns) pace_wait(t0, i, pace);
             st_release_shared(issued, i + 1);
             mbar_expect_tx(full + st, PSI_BYTES + 2 * NXHP * (int)sizeof(cd));
             const long long tile = tile_of(i);
             tma_load_3d_hint(base + (size_t)st * PSI_BYTES, &map_psi, 0, 0, (int)(tile * 2), full + st, polp);
             bulk_load_hint(slots + (size_t)st * SLOT_BYTES, spec + tile * 2 * NXHP, 2 * NXHP * (int)sizeof(cd), full + st, pol);
         }
+        if (pace.ns) pace_done(pace.st);
     } else if (tid == (NW + 1) * 32 || tid == (NW + 2) * 32) {
         const int which = warp - NW - 1;
         const uint64_t polp = l2_policy_code(pol_st);
@@ -480,6 +486,10 @@ k_xwarp2_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restric
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
+// These kernels are bound by the fp64 pipe, not by memory: paced to the slowest CTA (tma_pipe.cuh: pace_wait) they lose
+// 8 - 30 % (measured at 256^3 and 512 x 512 x 256); the loaders keep the hook, the launchers switch it off.
+static PaceArgs no_pace() { PaceArgs pa; pa.ns = 0; pa.head = 0; pa.head_ns = 0; pa.st = nullptr; return pa; }
+
 template <bool RT> static CnTabW<RT> make_cntabw(const AxisTables& a);
 template <> CnTabW<true> make_cntabw<true>(const AxisTables& a) {
     CnTabW<true> t; t.h = a.h; t.pf = a.pf8; t.pb = a.pb8; t.pfe = a.pfe8; t.pbs = a.pbs8; t.kap = a.kap; t.K = a.K8; return t;
@@ -514,7 +524,7 @@ template <int N, bool RT, int NW, int NST> static int launch_xwarp(dbec_handle_s
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[TM_PSI_XW];
     CK(launch_pdl(k, dim3(grid), dim3((NW + 3) * 32), sm, h->stream, h->use_pdl, *map, (const cd*)h->spec, h->ax[0].twN,
                   (const double*)h->scal, h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, h->nz, h->nb,
-                  make_cntabw<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]));
+                  make_cntabw<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC], no_pace()));
     h->launches++;
     return (int)cudaGetLastError();
 }
@@ -535,7 +545,7 @@ template <bool RT, int NG, int NST> static int launch_xwarp2(dbec_handle_s* h) {
     const CUtensorMap* map = (const CUtensorMap*)h->tmap[TM_PSI_XW];
     CK(launch_pdl(k, dim3(grid), dim3((2 * NG + 3) * 32), sm, h->stream, h->use_pdl, *map, (const cd*)h->spec, h->ax[0].twN,
                   (const double*)h->scal, h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, ntiles, h->ny, h->nz, h->nb,
-                  make_cntabw<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC]));
+                  make_cntabw<RT>(h->ax[0]), h->rev_next, h->pol[POL_NL_LD], h->pol[POL_NL_ST], h->pol[POL_NL_SPEC], no_pace()));
     h->launches++;
     return (int)cudaGetLastError();
 }

@@ -11,6 +11,7 @@
 // so that global loads, arithmetic and global stores of different tiles overlap inside one CTA.
 #pragma once
 #include <cuda.h>
+#include "dbec_internal.hpp"
 #include <stdint.h>
 #include <utility>
 
@@ -139,6 +140,47 @@ template <int N> __device__ __forceinline__ void bulk_wait() {
 // tables, initialising barriers) overlaps that tail, everything after sees the predecessor's memory ----
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// ---- pacing of a loader thread against the wall clock ----
+// A pass that streams a field much larger than L2 runs fastest when the CTAs walk their tiles in lockstep: the
+// tiles neighbouring CTAs work on at the same moment are neighbours in memory (128-byte pieces of the same rows), and
+// DRAM serves them from open pages.  Left alone, CTAs whose workers are quicker than their share of the memory
+// bandwidth drift apart, every piece opens its page again, and the pass drops to 0.77 - 0.85 of the copy bandwidth
+// (measured at 512 x 512 x 256: the imaginary-time y sweep, with LESS arithmetic per tile, took 423 us where the
+// real-time one took 333).  So every loader issues its tile i on a schedule: head_ns apart for the first `head`
+// tiles (what the previous pass left in L2, kernels_tma.cu: set_pace), pace_ns apart after that — the time the whole
+// grid needs for one tile each at a bandwidth just below what DRAM sustains (dbec_handle_s::pace_gbs).  The
+// schedule has to BIND at all times (a slack of two tiles lets the CTAs drift inside it and loses the effect) and it
+// has to be COMMON: a CTA that finds itself late publishes by how much (atomicMax on one word in global memory),
+// and every loader adds that lag to its own schedule, so the pack moves at the pace of its slowest member instead
+// of falling apart when the schedule is too optimistic.  The last loader to finish clears the word for the next
+// launch (launches that use it are ordered by the stream; their loaders start after griddepcontrol.wait).
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void pace_wait(unsigned long long& t0, int i, int head, int head_ns, int pace_ns, PaceState* ps) {
+    if (i == 0) { t0 = global_ns(); return; }
+    const unsigned long long nominal = t0 + (unsigned long long)(i < head ? i : head) * (unsigned long long)head_ns +
+                                       (unsigned long long)(i > head ? i - head : 0) * (unsigned long long)pace_ns;
+    const unsigned long long lag = ld_relaxed_u64(&ps->lag);
+    const unsigned long long now = global_ns();
+    if (now > nominal + lag + (unsigned long long)(pace_ns >> 3)) atomicMax(&ps->lag, now - nominal);     // late: everyone waits for me
+    else while (global_ns() < nominal + lag) __nanosleep(40);
+}
+__device__ __forceinline__ void pace_wait(unsigned long long& t0, int i, const PaceArgs& pa) {
+    pace_wait(t0, i, pa.head, pa.head_ns, pa.ns, pa.st);
+}
+__device__ __forceinline__ void pace_done(PaceState* ps) {
+    __threadfence();
+    if (atomicAdd(&ps->exits, 1u) == gridDim.x - 1) { ps->lag = 0ull; ps->exits = 0u; __threadfence(); }
+}
 
 // barrier over `nthreads` threads (a multiple of 32) with hardware barrier `id` (1..15; 0 is __syncthreads)
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {

@@ -281,6 +281,27 @@ def test_graph_and_plain_launches_agree_bitwise(gp, monkeypatch):
     assert np.array_equal(outs[0], outs[1])
 
 
+@pytest.mark.parametrize("shape,mode", [((256, 256, 128), REAL), ((512, 256, 64), IMAG)])
+def test_paced_and_unpaced_passes_agree_bitwise(gp, monkeypatch, shape, mode):
+    """Fields larger than L2: the loaders of the streaming passes are paced to the slowest CTA of the launch
+    (tma_pipe.cuh: pace_wait; DBEC_PACE=0 switches it off).  Pacing moves no arithmetic: bit-identical psi, and the
+    lag word is back at zero after every launch."""
+    w = grid3(*shape, mode)
+    psi0 = random_psi(w, 23)
+    outs = []
+    for pace in (None, "0"):
+        if pace is None:
+            monkeypatch.delenv("DBEC_PACE", raising=False)
+        else:
+            monkeypatch.setenv("DBEC_PACE", pace)
+        sim = gp.Dbec(gp.params_of(w))
+        sim.set_psi(psi0)
+        sim.step(4)
+        outs.append(sim.get_psi())
+        sim.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
 @pytest.mark.parametrize("w", [grid3(512, 256, 128, REAL), grid3(512, 256, 128, IMAG, d=(0.4, 0.3, 0.6)), grid3(256, 512, 256, REAL)], ids=wid)
 def test_z_sweep_on_paired_row_tiles(gp, ob, w):
     """xy planes of 2 MiB or more: the z sweep works on tiles of 8 columns x 2 rows of y (k_cn_tma with TC = 16;
