@@ -194,7 +194,7 @@ k_xwarp_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restrict
                             if (RT) {
                                 double sn, cs_;
                                 sincos_cw(a[kk], &sn, &cs_);          // branch-free: the evaluations interleave
-                                u[k0 + kk] = cmul(s, cmul(u[k0 + kk], cmake(cs_, -sn)));
+                                u[k0 + kk] = cmul(u[k0 + kk], cmake(cs_, -sn));      // (s = 1 in real time: no calcnorm, dbec_normalize applies its factor at once)
                             } else {
                                 u[k0 + kk] = cmul(s * exp_cw(-a[kk]), u[k0 + kk]);
                             }
@@ -410,7 +410,7 @@ k_xwarp2_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restric
                             if (RT) {
                                 double sn, cs_;
                                 sincos_cw(a[kk], &sn, &cs_);
-                                u[k0 + kk] = cmul(s, cmul(u[k0 + kk], cmake(cs_, -sn)));
+                                u[k0 + kk] = cmul(u[k0 + kk], cmake(cs_, -sn));      // (s = 1 in real time: no calcnorm, dbec_normalize applies its factor at once)
                             } else {
                                 u[k0 + kk] = cmul(s * exp_cw(-a[kk]), u[k0 + kk]);
                             }

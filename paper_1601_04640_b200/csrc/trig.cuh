@@ -4,18 +4,18 @@
 // The CUDA library sincos carries a slow-path branch for huge arguments; sixteen calls in a row then
 // run one after the other.  This version has no branch, so the compiler interleaves the sixteen
 // evaluations of a thread (the fp64 pipe has an 8-cycle dependent latency on sm_100a).
-//   k = nearest integer to u 2/pi;  r = u - k pi/2 with pi/2 as the sum of three doubles and FMAs
-//   (exact to < 1e-19 for |k| < 2^30);  Taylor polynomials of sin r / cos r on |r| <= pi/4 up to
+//   k = nearest integer to u 2/pi;  r = u - k pi/2 with pi/2 as the sum of two doubles and FMAs
+//   (pi/2 to 2^-106: the reduction error stays below 1e-23 for |k| < 2^30);  Taylor polynomials of sin r / cos r on |r| <= pi/4 up to
 //   r^15 / r^16 (truncation < 5e-17);  quadrant from k mod 4.
-// Absolute error <= 1.5e-16 against long-double sin/cos for |u| <= SINCOS_CW_MAX = 1e14 (checked on
-// the host by tests/test_host_logic.py; the reduction is exact while |k| < 2^51).  Beyond that, where
-// one ulp of u is already a sizeable part of a turn and the time step is meaningless anyway, and for
+// Absolute error <= 1.5e-16 against long-double sin/cos for |u| <= SINCOS_CW_MAX = 1e9 (checked on
+// the host by tests/test_host_logic.py).  Beyond that — u = dt (V + G n + D Phi) of a meaningful time step is of
+// order one — and for
 // non-finite u, both results are NaN (a select, not a branch), as loud as the library's behaviour
 // for infinities.
 #pragma once
 #include "cplx.cuh"
 
-#define SINCOS_CW_MAX 1.0e14
+#define SINCOS_CW_MAX 1.0e9
 
 // Coefficients: on the device they sit in constant memory, so that every DFMA takes its coefficient
 // as a constant-bank operand (as 64-bit immediates they cost two uniform-register moves per use).
@@ -56,7 +56,6 @@ DBEC_HD void sincos_cw(double u, double* sn, double* cs) {
 #endif
     double r = fma(-kd, K[1], u);
     r = fma(-kd, K[2], r);
-    r = fma(-kd, K[3], r);
     const double r2 = r * r;
     double ps = K[4];
 #pragma unroll

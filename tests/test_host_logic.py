@@ -134,7 +134,7 @@ def test_reference_arm_prints_one_json_line():
 
 def test_branch_free_sincos_matches_libm(tmp_path):
     """csrc/trig.cuh (used by the real-time calcnu) against numpy's sin/cos in long double: absolute
-    error <= 2e-16 on |u| <= 1e14, exact values at 0, NaN beyond the stated range and for inf/nan."""
+    error <= 2e-16 on |u| <= 1e9, exact values at 0, NaN beyond the stated range and for inf/nan."""
     import ctypes
     import numpy as np
     src = os.path.join(os.path.dirname(__file__), "host_trig_harness.cpp")
@@ -143,7 +143,7 @@ def test_branch_free_sincos_matches_libm(tmp_path):
     L = ctypes.CDLL(so)
     L.sincos_cw_array.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long]
     rng = np.random.default_rng(7)
-    parts = [rng.uniform(-s, s, 200000) for s in (1.0, 10.0, 1e3, 1e6, 1e10, 1e14)]
+    parts = [rng.uniform(-s, s, 200000) for s in (1.0, 10.0, 1e3, 1e6, 1e8, 1e9)]
     parts.append(np.arange(-64, 65) * (np.pi / 4))            # quadrant boundaries
     parts.append(np.array([0.0, -0.0, 1e-300, 5e-324]))
     u = np.ascontiguousarray(np.concatenate(parts))
@@ -153,7 +153,7 @@ def test_branch_free_sincos_matches_libm(tmp_path):
     assert np.max(np.abs(sn - np.sin(ul))) <= 2e-16
     assert np.max(np.abs(cs - np.cos(ul))) <= 2e-16
     assert np.max(np.abs(sn * sn + cs * cs - 1.0)) <= 5e-16
-    bad = np.array([2e14, -1e300, np.inf, -np.inf, np.nan])
+    bad = np.array([2e9, -1e300, np.inf, -np.inf, np.nan])
     sb, cb = np.empty_like(bad), np.empty_like(bad)
     with np.errstate(all="ignore"):
         L.sincos_cw_array(bad.ctypes.data, sb.ctypes.data, cb.ctypes.data, bad.size)
