@@ -2,7 +2,7 @@
 // ("launching of all required kernels would create a sizeable overhead").
 //
 // A grid of up to 64 Ki points (BASELINE.json's 32^3 config: psi is 512 KiB) cannot feed 148 SMs, and seven launches
-// per step cost more than their work.  Here a cluster of CS CTAs (8, one per SM) owns a simulation for as many steps
+// per step cost more than their work.  Here a cluster of CS CTAs (16 or 8, one per SM) owns a simulation for as many steps
 // as dbec_step asks: the data stays in L2, the kernel boundaries of the step become hardware cluster barriers
 // (barrier.cluster, release/acquire), and the passes that share an xy plane run back to back in shared memory:
 //   A  per plane:   n = |s psi|^2 -> FFT-x (two real lines per transform) -> FFT-y -> spectrum
