@@ -302,6 +302,30 @@ def test_paced_and_unpaced_passes_agree_bitwise(gp, monkeypatch, shape, mode):
     assert np.array_equal(outs[0], outs[1])
 
 
+def test_handles_on_concurrent_streams_do_not_disturb_each_other(gp):
+    """Three handles on three streams advance at the same time: a paced 256 x 256 x 128 grid (its persistent kernels
+    want every SM and wait for each other's lag word, which lives in each handle's own workspace), a 128^3 grid and a
+    32^3 grid on its cluster.  Nothing may hang, and each result is bit-identical to the same handle run alone."""
+    ws = [grid3(256, 256, 128, REAL), grid3(128, 128, 128, IMAG), grid3(32, 32, 32, REAL)]
+    psis = [random_psi(w, 60 + i) for i, w in enumerate(ws)]
+    alone = []
+    for w, psi0 in zip(ws, psis):
+        sim = gp.Dbec(gp.params_of(w))
+        sim.set_psi(psi0)
+        sim.step(6)
+        alone.append(sim.get_psi())
+        sim.close()
+    sims = [gp.Dbec(gp.params_of(w)) for w in ws]
+    for sim, psi0 in zip(sims, psis):
+        sim.set_psi(psi0)
+    for _ in range(3):                       # interleave the enqueues: the three streams run side by side
+        for sim in sims:
+            sim.step(2)
+    for sim, ref in zip(sims, alone):
+        assert np.array_equal(sim.get_psi(), ref)
+        sim.close()
+
+
 @pytest.mark.parametrize("w", [grid3(512, 256, 128, REAL), grid3(512, 256, 128, IMAG, d=(0.4, 0.3, 0.6)), grid3(256, 512, 256, REAL)], ids=wid)
 def test_z_sweep_on_paired_row_tiles(gp, ob, w):
     """xy planes of 2 MiB or more: the z sweep works on tiles of 8 columns x 2 rows of y (k_cn_tma with TC = 16;
