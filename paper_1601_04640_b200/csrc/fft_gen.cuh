@@ -94,6 +94,7 @@ __device__ __forceinline__ void gen_butterfly_k(const cd* in, cd* out, int SE, i
     }
     if (R == 2) dft2<S>(v[0], v[1]);
     else if (R == 4) dft4<S>(v[0], v[1], v[2], v[3]);
+    else if (R == 8 || R == 16) dft_small<R, S>(v);
     else {
         cd w[R];
 #pragma unroll
@@ -158,12 +159,16 @@ __device__ __noinline__ void gen_fft_pass_odd(const cd* a, cd* b, int L, FastDiv
 // their shared-memory address space (LDS / STS, not generic accesses) and the plan is read straight from the
 // kernel's parameter bank: through an out-of-line call with generic pointers a pass on a handful of lines took
 // ~900 cycles, most of it address-space and parameter overhead.
-template <int S, bool LFAST>
+// BIG: the plan may also hold passes of radix 8 and 16 (kernels_gen.cu; kernels_small.cu keeps to 2 and 4 for its
+// instruction-cache footprint).
+template <int S, bool LFAST, bool BIG = false>
 __device__ __forceinline__ cd* gen_fft_lines2(cd* a, cd* b, int L, FastDiv fL, FastDiv fL0, int S0, int S1, int SE, const GenPlanP& pl,
                                               const cd* __restrict__ twN) {
     for (int s = 0; s < pl.nfac; ++s) {
         const GenPass ps = pl.pass[s];
-        switch (ps.r) {
+        if (BIG && ps.r == 16) gen_fft_pass<16, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN);
+        else if (BIG && ps.r == 8) gen_fft_pass<8, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN);
+        else switch (ps.r) {
             case 2: gen_fft_pass<2, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
             case 4: gen_fft_pass<4, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;
             case 3: gen_fft_pass_odd<3, S, LFAST>(a, b, L, fL, fL0, S0, S1, SE, pl.n, ps, twN); break;

@@ -24,14 +24,16 @@
 // Block = LP line pairs; shared memory: two buffers of LP lines of n complex values.
 __global__ void __launch_bounds__(256)
 k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twN, double* __restrict__ scal,
-                   GenPlan pl, int LP, int npairs, int nxhp, int pairs_per_member, int nb, int advance) {
+                   const __grid_constant__ GenPlanP pl, int LP, int npairs, int nxhp, int pairs_per_member, int nb, int advance) {
     extern __shared__ cd gsm[];
     pdl_launch_dependents(); pdl_wait();
     const int n = pl.n;
     cd* a = gsm; cd* b = gsm + (size_t)LP * n;
     const long long pair0 = (long long)blockIdx.x * LP;
+    const FastDiv fn(n), fnxhp(nxhp), fone(1), fLP(LP);
     for (int idx = threadIdx.x; idx < LP * n; idx += blockDim.x) {
-        const int l = idx / n, x = idx % n;
+        int l, x;
+        fn.divmod(idx, l, x);
         const long long pair = pair0 + l;
         cd v = cmake(0.0, 0.0);
         if (pair < npairs) {
@@ -43,9 +45,10 @@ k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* 
     if (advance && blockIdx.x == 0)            // first kernel of a step: move the NSTP ramp on (reads neither G nor D)
         for (int m = threadIdx.x; m < nb; m += blockDim.x) ramp_advance(scal + (size_t)m * SC_COUNT);
     __syncthreads();
-    const cd* z = gen_fft_lines<-1, false>(a, b, LP, n, 1, pl, twN);
+    const cd* z = gen_fft_lines2<-1, false, true>(a, b, LP, fone, fLP, n, 0, 1, pl, twN);
     for (int idx = threadIdx.x; idx < LP * nxhp; idx += blockDim.x) {
-        const int l = idx / nxhp, k = idx % nxhp;
+        int l, k;
+        fnxhp.divmod(idx, l, k);
         const long long pair = pair0 + l;
         if (pair >= npairs) continue;
         cd xa = cmake(0.0, 0.0), xb = xa;
@@ -67,7 +70,7 @@ k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* 
 // so that two buffers of n x cols values fit), element (j, col) at j*cols + col in shared memory.
 template <int MODE>
 __global__ void __launch_bounds__(256)
-k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twN, GenPlan pl, int cols,
+k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twN, const __grid_constant__ GenPlanP pl, int cols,
                   long long line_stride, long long outer_stride, int ntiles_x, long long ntiles, int nxhp, int ny3,
                   long long vdd_line_stride) {
     extern __shared__ cd gsm[];
@@ -78,23 +81,25 @@ k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const c
     if (tile >= ntiles) return;
     const long long outer = tile / ntiles_x, tx = tile % ntiles_x;
     cd* g = spec + outer * outer_stride + tx * cols;
-    for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) a[idx] = g[(long long)(idx / cols) * line_stride + idx % cols];
+    const int cs = cols == 8 ? 3 : 2, cm = cols - 1;           // cols is 8 or 4
+    const FastDiv fc(cols), fnxhp(nxhp);
+    for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) a[idx] = g[(long long)(idx >> cs) * line_stride + (idx & cm)];
     __syncthreads();
     cd* r = a; cd* o = b;
-    if (MODE == 0 || MODE == 2) { r = gen_fft_lines<-1, true>(a, b, cols, 1, cols, pl, twN); o = (r == a) ? b : a; }
+    if (MODE == 0 || MODE == 2) { r = gen_fft_lines2<-1, true, true>(a, b, cols, fc, fc, 1, 0, cols, pl, twN); o = (r == a) ? b : a; }
     if (MODE == 2) {
         // folded V_dd table (kernels_fft.cu: k_fft_strided): row j -> min(j, n - j); 3-D: k_y of the column folds too
         for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) {
-            const int j = idx / cols;
-            const long long cix = tx * cols + idx % cols;
+            const int j = idx >> cs;
+            const long long cix = tx * cols + (idx & cm);
             long long voff = cix;
-            if (ny3) { const int ky = (int)(cix / nxhp), kx = (int)(cix % nxhp); voff = (long long)(ky < ny3 - ky ? ky : ny3 - ky) * nxhp + kx; }
+            if (ny3) { int ky, kx; fnxhp.divmod((int)cix, ky, kx); voff = (long long)(ky < ny3 - ky ? ky : ny3 - ky) * nxhp + kx; }
             r[idx] = cmul(vdd[voff + (long long)(j < n - j ? j : n - j) * vdd_line_stride], r[idx]);
         }
         __syncthreads();
     }
-    if (MODE == 1 || MODE == 2) r = gen_fft_lines<+1, true>(r, o, cols, 1, cols, pl, twN);
-    for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) g[(long long)(idx / cols) * line_stride + idx % cols] = r[idx];
+    if (MODE == 1 || MODE == 2) r = gen_fft_lines2<+1, true, true>(r, o, cols, fc, fc, 1, 0, cols, pl, twN);
+    for (int idx = threadIdx.x; idx < n * cols; idx += blockDim.x) g[(long long)(idx >> cs) * line_stride + (idx & cm)] = r[idx];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -104,14 +109,16 @@ template <bool RT, bool PHI>
 __global__ void __launch_bounds__(256)
 k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out, const cd* __restrict__ twN,
                    const double* __restrict__ scal, const double* __restrict__ vx, const double* __restrict__ vy,
-                   const double* __restrict__ vz, double dt, GenPlan pl, int LP, int npairs, int nxhp, int ny, int nz) {
+                   const double* __restrict__ vz, double dt, const __grid_constant__ GenPlanP pl, int LP, int npairs, int nxhp, int ny, int nz) {
     extern __shared__ cd gsm[];
     pdl_launch_dependents(); pdl_wait();
     const int n = pl.n;
     cd* a = gsm; cd* b = gsm + (size_t)LP * n;
     const long long pair0 = (long long)blockIdx.x * LP;
+    const FastDiv fn(n), fone(1), fLP(LP);
     for (int idx = threadIdx.x; idx < LP * n; idx += blockDim.x) {
-        const int l = idx / n, k = idx % n;
+        int l, k;
+        fn.divmod(idx, l, k);
         const long long pair = pair0 + l;
         cd v = cmake(0.0, 0.0);
         if (pair < npairs) {
@@ -123,9 +130,10 @@ k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __
         a[idx] = v;
     }
     __syncthreads();
-    const cd* f = gen_fft_lines<+1, false>(a, b, LP, n, 1, pl, twN);      // (Phi on line a, Phi on line b); 1/P is in the table
+    const cd* f = gen_fft_lines2<+1, false, true>(a, b, LP, fone, fLP, n, 0, 1, pl, twN);      // (Phi on line a, Phi on line b); 1/P is in the table
     for (int idx = threadIdx.x; idx < 2 * LP * n; idx += blockDim.x) {
-        const int ll = idx / n, x = idx % n;                              // line ll of the block: pair ll / 2, component ll & 1
+        int ll, x;
+        fn.divmod(idx, ll, x);                              // line ll of the block: pair ll / 2, component ll & 1
         const long long row = (pair0 + ll / 2) * 2 + (ll & 1);
         if (row >= 2LL * npairs) continue;
         const cd pp = f[(ll / 2) * n + x];
@@ -229,12 +237,20 @@ int dbec_gen_factor(int n, int* fac) {
     return n == 1 ? k : 0;
 }
 
-static GenPlan plan_of(const dbec_handle_s* h, int axis) {
+// The plans of this file take the powers of two in passes of radix 16 and 8 first (384 = 16 x 8 x 3: three passes
+// through shared memory instead of five).
+static GenPlanP plan_of(const dbec_handle_s* h, int axis) {
     GenPlan pl;
-    pl.n = h->ax[axis].n;
-    pl.nfac = h->gnfac[axis];
-    for (int i = 0; i < 12; ++i) pl.fac[i] = h->gfac[axis][i];
-    return pl;
+    int n = h->ax[axis].n, k = 0;
+    pl.n = n;
+    for (int i = 0; i < 12; ++i) pl.fac[i] = 0;
+    while (n % 16 == 0) { pl.fac[k++] = 16; n /= 16; }
+    if (n % 8 == 0) { pl.fac[k++] = 8; n /= 8; }
+    k += dbec_gen_factor(n, pl.fac + k);
+    pl.nfac = k;
+    GenPlanP pp;
+    make_plan_p(pl, &pp);
+    return pp;
 }
 
 template <class K> static int gen_smem(K kernel, size_t bytes) {
@@ -246,7 +262,7 @@ template <class K> static int gen_smem(K kernel, size_t bytes) {
 static int gen_lp(int n) { int lp = 2048 / n; return lp < 1 ? 1 : (lp > 8 ? 8 : lp); }
 
 int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance) {
-    const GenPlan pl = plan_of(h, 0);
+    const GenPlanP pl = plan_of(h, 0);
     const int LP = gen_lp(pl.n), ppm = h->ny * h->nz / 2, npairs = ppm * h->nb;
     const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
     CK((cudaError_t)gen_smem(k_gen_density_fftx, sm));
@@ -257,7 +273,7 @@ int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance) {
 }
 
 template <int MODE> static int launch_gen_fft(dbec_handle_s* h, int axis) {
-    const GenPlan pl = plan_of(h, axis);
+    const GenPlanP pl = plan_of(h, axis);
     const int cols = pl.n <= 512 ? 8 : 4;
     long long line_stride, outer_stride, ntiles;
     int ntx;
@@ -279,7 +295,7 @@ int dbec_launch_gen_fft(dbec_handle_s* h, int axis, int mode) {
 }
 
 template <bool RT, bool PHI> static int launch_gen_nonlin(dbec_handle_s* h, double* phi) {
-    const GenPlan pl = plan_of(h, 0);
+    const GenPlanP pl = plan_of(h, 0);
     const int LP = gen_lp(pl.n), npairs = h->ny * h->nz / 2 * h->nb;
     const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
     auto k = k_gen_ifftx_nonlin<RT, PHI>;
