@@ -165,6 +165,7 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     CU(h, put(pfe_re.data(), sizeof(double) * 64, (const void**)&A.pfe_re));
     CU(h, put(pbs_re.data(), sizeof(double) * 64, (const void**)&A.pbs_re));
     A.K8 = 0;
+    A.K16 = std::max(1, std::max(carry_terms(pfe, npad / CN_L), carry_terms(pbs, npad / CN_L)));
     if (axis == 0 && n >= 16 && n % 8 == 0 && n / 8 <= 128) {
         // the x axis again with chunks of 8 points (one 128-byte row of psi per lane, kernels_xwarp.cu)
         std::vector<zc> h8, pf8, pb8, pfe8(128, zc(0, 0)), pbs8(128, zc(0, 0));

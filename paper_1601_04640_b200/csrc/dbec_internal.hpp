@@ -73,6 +73,7 @@ struct AxisTables {
     const cd* pf8; const cd* pb8; const cd* pfe8; const cd* pbs8;
     const double* pf8_re; const double* pb8_re; const double* pfe8_re; const double* pbs8_re;
     int K8;
+    int K16;                // the same count for the chunks of 16 points (kernels_gen.cu)
 };
 
 struct dbec_handle_s {

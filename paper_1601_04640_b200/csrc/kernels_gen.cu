@@ -15,6 +15,7 @@
 #include "cn_line_smem.cuh"
 #include "tma_pipe.cuh"
 #include "norm_finish.cuh"
+#include "trig.cuh"
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
@@ -145,8 +146,8 @@ k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __
         const cd q = psi[row * n + x];
         const double u = dt * (vx[x] + vy[y] + vz[z] + sc[SC_G] * (s2 * cnorm2(q)) + sc[SC_D] * phi);
         cd r;
-        if (RT) { double sn, cs; sincos(u, &sn, &cs); r = cmul(s, cmul(q, cmake(cs, -sn))); }
-        else r = cmul(s * exp(-u), q);
+        if (RT) { double sn, cs; sincos_cw(u, &sn, &cs); r = cmul(s, cmul(q, cmake(cs, -sn))); }      // (trig.cuh: branch-free)
+        else r = cmul(s * exp_cw(-u), q);
         psi[row * n + x] = r;
     }
 }
@@ -161,7 +162,7 @@ constexpr int GC = 8;
 template <bool RT, bool NORM>
 __global__ void __launch_bounds__(512)
 k_gen_cn(cd* __restrict__ psi, CnTab<RT> cn, int n, int nch, long long elem_stride, long long col_stride, long long outer_stride,
-         long long ncols, double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV, int nb) {
+         long long ncols, double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV, int nb, int K) {
     typedef typename CnCoef<RT>::type CT;
     extern __shared__ cd gsm[];                // [2][chunk slots][GC] zero-start chunk ends
     // (the block is rounded up to whole warps: chunk slots c >= nch hold padding only and solve to zero)
@@ -192,7 +193,9 @@ k_gen_cn(cd* __restrict__ psi, CnTab<RT> cn, int n, int nch, long long elem_stri
     __syncthreads();
     // carries over ALL earlier / later chunks; chunk-end products from the per-element tables
     cd din = zero;
-    for (int i = 0; i < c && i < nch; ++i) din = cn_fma(cn.pf[i * CN_L + CN_L - 1], din, e0[i * GC + col]);
+    // (the carry is a Horner sum over the earlier chunk ends with factors < 1: the host counts the K terms that are
+    // above 2^-73 of the first, dbec_api.cu carry_terms; the rest is below the last bit of the sum)
+    for (int i = (c - K > 0 ? c - K : 0); i < c && i < nch; ++i) din = cn_fma(cn.pf[i * CN_L + CN_L - 1], din, e0[i * GC + col]);
     cn_chunk_backward<CT>(u, din, cn.h + jt, cn.pf + jt);
     if (pad) {
 #pragma unroll
@@ -201,7 +204,7 @@ k_gen_cn(cd* __restrict__ psi, CnTab<RT> cn, int n, int nch, long long elem_stri
     e1[c * GC + col] = u[0];
     __syncthreads();
     cd uin = zero;
-    for (int i = nch - 1; i > c; --i) uin = cn_fma(cn.pb[i * CN_L], uin, e1[i * GC + col]);
+    for (int i = (c + K < nch - 1 ? c + K : nch - 1); i > c; --i) uin = cn_fma(cn.pb[i * CN_L], uin, e1[i * GC + col]);
     cn_chunk_fix<CT>(u, uin, cn.pb + jt);
     double acc = 0.0;
 #pragma unroll
@@ -323,7 +326,7 @@ template <bool RT, bool NORM> static int launch_gen_cn(dbec_handle_s* h, int axi
     if (NORM && (long long)grid.x * grid.y > h->npartial) return (int)cudaErrorInvalidValue;
     const size_t sm = 2 * (size_t)(threads / GC) * GC * sizeof(cd);
     CK(launch_pdl(k_gen_cn<RT, NORM>, grid, dim3(threads), sm, h->stream, h->use_pdl, h->psi, make_cntab<RT>(h->ax[axis]), n, nch, es, cs, os,
-                  ncols, h->partial, h->ticket, h->scal, h->dV, h->nb));
+                  ncols, h->partial, h->ticket, h->scal, h->dV, h->nb, h->ax[axis].K16));
     h->launches++;
     return (int)cudaGetLastError();
 }
