@@ -101,16 +101,18 @@ template <class CT, int L> DBEC_HD void cn_chunk_fix2(cd (&u)[L], cd (&w)[L], cd
 
 // Carry into chunk c of the forward pass: D_in = d_{c*L-1}, from the zero-start chunk ends
 // e[i*es] = d~ at the last element of chunk i and pfend[i] = PF at that element.
-template <class CT> DBEC_HD cd cn_carry_forward(int c, const cd* e, int es, const CT* __restrict__ pfend) {
+// K: the number of terms that are above 2^-73 of the first (the factors are products of CN_L consecutive |h_j| < 1;
+// dbec_api.cu carry_terms) — the sum starts K chunks back; the default takes them all.
+template <class CT> DBEC_HD cd cn_carry_forward(int c, const cd* e, int es, const CT* __restrict__ pfend, int K = 1 << 30) {
     cd D = cmake(0.0, 0.0);
-    for (int i = 0; i < c; ++i) D = cn_fma(pfend[i], D, e[i * es]);
+    for (int i = (c - K > 0 ? c - K : 0); i < c; ++i) D = cn_fma(pfend[i], D, e[i * es]);
     return D;
 }
 
 // Carry into chunk c of the backward pass: U_in = u_{(c+1)*L}, from chunk starts
 // e[i*es] = u~ at the first element of chunk i and pbstart[i] = PB at that element.
-template <class CT> DBEC_HD cd cn_carry_backward(int c, int C, const cd* e, int es, const CT* __restrict__ pbstart) {
+template <class CT> DBEC_HD cd cn_carry_backward(int c, int C, const cd* e, int es, const CT* __restrict__ pbstart, int K = 1 << 30) {
     cd U = cmake(0.0, 0.0);
-    for (int i = C - 1; i > c; --i) U = cn_fma(pbstart[i], U, e[i * es]);
+    for (int i = (K < C - 1 - c ? c + K : C - 1); i > c; --i) U = cn_fma(pbstart[i], U, e[i * es]);
     return U;
 }

@@ -10,13 +10,14 @@ template <bool RT> struct CnTab {
     typedef typename CnCoef<RT>::type CT;
     const CT* h; const CT* pf; const CT* pb; const CT* pfe; const CT* pbs;
     CT kap;
+    int K;              // carry terms above 2^-73 of the first one (AxisTables::K16)
 };
 template <bool RT> inline CnTab<RT> make_cntab(const AxisTables& a);
 template <> inline CnTab<true> make_cntab<true>(const AxisTables& a) {
-    CnTab<true> t; t.h = a.h; t.pf = a.pf; t.pb = a.pb; t.pfe = a.pfe; t.pbs = a.pbs; t.kap = a.kap; return t;
+    CnTab<true> t; t.h = a.h; t.pf = a.pf; t.pb = a.pb; t.pfe = a.pfe; t.pbs = a.pbs; t.kap = a.kap; t.K = a.K16; return t;
 }
 template <> inline CnTab<false> make_cntab<false>(const AxisTables& a) {
-    CnTab<false> t; t.h = a.h_re; t.pf = a.pf_re; t.pb = a.pb_re; t.pfe = a.pfe_re; t.pbs = a.pbs_re; t.kap = a.kap.x;
+    CnTab<false> t; t.h = a.h_re; t.pf = a.pf_re; t.pb = a.pb_re; t.pfe = a.pfe_re; t.pbs = a.pbs_re; t.kap = a.kap.x; t.K = a.K16;
     return t;
 }
 

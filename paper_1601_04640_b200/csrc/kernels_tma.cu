@@ -193,11 +193,11 @@ k_cn_tma(const __grid_constant__ CUtensorMap map, CnTab<RT> cn, TileGeom tg, dou
             cn_chunk_forward<CT>(u, lo, hi, cs.kap, cs.h + t0);
             myends[c * TC + col] = u[CN_L - 1];
             named_bar_sync(1 + g, GT);
-            const cd din = cn_carry_forward<CT>(c, myends + col, TC, cs.pfe);
+            const cd din = cn_carry_forward<CT>(c, myends + col, TC, cs.pfe, cs.K);
             cn_chunk_backward<CT>(u, din, cs.h + t0, cs.pf + t0);
             myends[GT + c * TC + col] = u[0];
             named_bar_sync(1 + g, GT);
-            const cd uin = cn_carry_backward<CT>(c, NCH, myends + GT + col, TC, cs.pbs);
+            const cd uin = cn_carry_backward<CT>(c, NCH, myends + GT + col, TC, cs.pbs, cs.K);
             cn_chunk_fix<CT>(u, uin, cs.pb + t0);
 #pragma unroll
             for (int k = 0; k < CN_L; ++k) {

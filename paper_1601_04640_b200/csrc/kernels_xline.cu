@@ -177,11 +177,11 @@ k_xline_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, const cd* __re
             cn_chunk_forward<CT>(u, lo, hi, cs.kap, cs.h + 17 * c);
             e0[c * XR + r] = u[CN_L - 1];
             named_bar_sync(1 + g, GT);
-            const cd din = cn_carry_forward<CT>(c, e0 + r, XR, cs.pfe);
+            const cd din = cn_carry_forward<CT>(c, e0 + r, XR, cs.pfe, cs.K);
             cn_chunk_backward<CT>(u, din, cs.h + 17 * c, cs.pf + 17 * c);
             e1[c * XR + r] = u[0];
             named_bar_sync(1 + g, GT);
-            const cd uin = cn_carry_backward<CT>(c, NCH, e1 + r, XR, cs.pbs);
+            const cd uin = cn_carry_backward<CT>(c, NCH, e1 + r, XR, cs.pbs, cs.K);
             cn_chunk_fix<CT>(u, uin, cs.pb + 17 * c);
 #pragma unroll
             for (int k = 0; k < CN_L; ++k) line[k] = u[k];
