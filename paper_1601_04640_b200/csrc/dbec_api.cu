@@ -357,8 +357,9 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
     h->ticket = (unsigned int*)(w + L.ticket);
     h->obs_dev = (double*)(w + L.obs);
     h->npartial = (int)L.npartial;
-    // the only three switches (all exercised by tests/test_gpu_parity.py): the CUDA graph of a step, the x sweep
-    // fused into the nonlinear kernel, and the one-launch step of small grids (CTAs per cluster; 0 = off)
+    // the only four switches (all exercised by tests/test_gpu_parity.py): the CUDA graph of a step, the x sweep
+    // fused into the nonlinear kernel, the one-launch step of small grids (DBEC_CLUSTER: CTAs per cluster; 0 = off) and
+    // the pacing of the streaming passes (DBEC_PACE, below)
     const char* fe = getenv("DBEC_FUSE_CNX");
     h->fuse_cnx = fe ? atoi(fe) : 1;
     const char* ge = getenv("DBEC_GRAPH");
