@@ -418,6 +418,10 @@ def run_ours(args, w):
                     "fused_pipeline": {"bytes_per_point": fused, "achieved_GBps": fused * pts_per_ns,
                                        "frac": fused * pts_per_ns / peak,
                                        "note": "algorithmic bytes of this repository's own seven-pass pipeline"}}
+        # the x-line kernel (inverse FFT-x + calcnu + calclux) is the one pass whose time is set by the fp64 pipe rather
+        # than by memory; its HBM fraction is still what the step pays for it
+        roofline["secondary"] = ("fp64 pipe: 63 DFMA/clk/SM measured (profiles/r2_fp64_probe.md); the x-line kernel runs at about "
+                                 "55 % of it with 79 DP instructions per grid point (profiles/r2_step_ncu_full.md)")
         tr = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram__bytes_{read,write}.sum per launch
         if os.path.exists(tr):
             import csv
