@@ -286,7 +286,7 @@ k_xwarp2_nonlin(const __grid_constant__ CUtensorMap map_psi, const cd* __restric
                 float pol_ld, float pol_st, float pol_spec, PaceArgs pace) {
     typedef typename CnCoef<RT>::type CT;
     typedef WPlan512 P;
-    constexpr int N = 512, NLW_C = NlwBatch<RT>::C;
+    constexpr int N = 512, NLW_C = RT ? 2 : NlwBatch<RT>::C;
     constexpr int T = P::T;                                          // 64 threads per pair
     constexpr int CPL = N / WL;                                      // 64 chunks per line: two per lane
     constexpr int NXHP = w_nxhp(N);
