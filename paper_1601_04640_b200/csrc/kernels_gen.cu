@@ -23,7 +23,7 @@
 // a1, x axis: n = |s psi|^2 -> half spectrum, two real lines per complex transform
 // ------------------------------------------------------------------------------------------------
 // Block = LP line pairs; shared memory: two buffers of LP lines of n complex values.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(512, 2)
 k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twN, double* __restrict__ scal,
                    const __grid_constant__ GenPlanP pl, int LP, int npairs, int nxhp, int pairs_per_member, int nb, int advance) {
     extern __shared__ cd gsm[];
@@ -70,7 +70,7 @@ k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* 
 // A tile is `cols` neighbouring columns (8: one 128-byte row per line point; 4 for lines longer than 512 points,
 // so that two buffers of n x cols values fit), element (j, col) at j*cols + col in shared memory.
 template <int MODE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(512, 2)
 k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twN, const __grid_constant__ GenPlanP pl, int cols,
                   long long line_stride, long long outer_stride, int ntiles_x, long long ntiles, int nxhp, int ny3,
                   long long vdd_line_stride) {
@@ -107,7 +107,7 @@ k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const c
 // a3 (x axis, complex-to-real, two lines per transform) + a4 calcnu, or Phi_dd written out
 // ------------------------------------------------------------------------------------------------
 template <bool RT, bool PHI>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(512, 2)
 k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out, const cd* __restrict__ twN,
                    const double* __restrict__ scal, const double* __restrict__ vx, const double* __restrict__ vy,
                    const double* __restrict__ vz, double dt, const __grid_constant__ GenPlanP pl, int LP, int npairs, int nxhp, int ny, int nz) {
@@ -247,8 +247,7 @@ static GenPlanP plan_of(const dbec_handle_s* h, int axis) {
     int n = h->ax[axis].n, k = 0;
     pl.n = n;
     for (int i = 0; i < 12; ++i) pl.fac[i] = 0;
-    while (n % 16 == 0) { pl.fac[k++] = 16; n /= 16; }
-    if (n % 8 == 0) { pl.fac[k++] = 8; n /= 8; }
+    while (n % 8 == 0) { pl.fac[k++] = 8; n /= 8; }
     k += dbec_gen_factor(n, pl.fac + k);
     pl.nfac = k;
     GenPlanP pp;
@@ -269,7 +268,7 @@ int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance) {
     const int LP = gen_lp(pl.n), ppm = h->ny * h->nz / 2, npairs = ppm * h->nb;
     const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
     CK((cudaError_t)gen_smem(k_gen_density_fftx, sm));
-    CK(launch_pdl(k_gen_density_fftx, dim3((npairs + LP - 1) / LP), dim3(256), sm, h->stream, h->use_pdl, (const cd*)h->psi, h->spec,
+    CK(launch_pdl(k_gen_density_fftx, dim3((npairs + LP - 1) / LP), dim3(512), sm, h->stream, h->use_pdl, (const cd*)h->psi, h->spec,
                   h->ax[0].twN, h->scal, pl, LP, npairs, h->nxhp, ppm, h->nb, advance));
     h->launches++;
     return (int)cudaGetLastError();
@@ -287,7 +286,7 @@ template <int MODE> static int launch_gen_fft(dbec_handle_s* h, int axis) {
     const size_t sm = 2 * (size_t)pl.n * cols * sizeof(cd);
     auto k = k_gen_fft_strided<MODE>;
     CK((cudaError_t)gen_smem(k, sm));
-    CK(launch_pdl(k, dim3((unsigned)ntiles), dim3(256), sm, h->stream, h->use_pdl, h->spec, (const double*)h->vdd, h->ax[axis].twN, pl,
+    CK(launch_pdl(k, dim3((unsigned)ntiles), dim3(512), sm, h->stream, h->use_pdl, h->spec, (const double*)h->vdd, h->ax[axis].twN, pl,
                   cols, line_stride, outer_stride, ntx, ntiles, h->nxhp, ny3, vls));
     h->launches++;
     return (int)cudaGetLastError();
@@ -303,7 +302,7 @@ template <bool RT, bool PHI> static int launch_gen_nonlin(dbec_handle_s* h, doub
     const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
     auto k = k_gen_ifftx_nonlin<RT, PHI>;
     CK((cudaError_t)gen_smem(k, sm));
-    CK(launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(256), sm, h->stream, h->use_pdl, (const cd*)h->spec, h->psi, phi, h->ax[0].twN,
+    CK(launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(512), sm, h->stream, h->use_pdl, (const cd*)h->spec, h->psi, phi, h->ax[0].twN,
                   (const double*)h->scal, h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, pl, LP, npairs, h->nxhp, h->ny, h->nz));
     h->launches++;
     return (int)cudaGetLastError();
