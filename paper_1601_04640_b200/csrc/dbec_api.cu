@@ -166,21 +166,25 @@ static int upload_axis(dbec_handle h, int axis, int n, double d, double omega, c
     CU(h, put(pbs_re.data(), sizeof(double) * 64, (const void**)&A.pbs_re));
     A.K8 = 0;
     A.K16 = std::max(1, std::max(carry_terms(pfe, npad / CN_L), carry_terms(pbs, npad / CN_L)));
-    if (axis == 0 && n >= 16 && n % 8 == 0 && n / 8 <= 128) {
-        // the x axis again with chunks of 8 points (one 128-byte row of psi per lane, kernels_xwarp.cu)
+    if (n >= 3) {
+        // the same tables for chunks of 8 points: the x axis of kernels_xwarp.cu (one 128-byte row of psi per lane) and
+        // every axis of kernels_gen.cu (half the registers per thread, twice the threads per line); padded with zeros
+        // to whole chunks like the tables above
+        const int npad8 = (n + 7) / 8 * 8;
         std::vector<zc> h8, pf8, pb8, pfe8(128, zc(0, 0)), pbs8(128, zc(0, 0));
         make_cn(n, 8, a, h8, pf8, pb8);
-        for (int c = 0; c < n / 8; ++c) { pfe8[c] = pf8[c * 8 + 7]; pbs8[c] = pb8[c * 8]; }
+        pf8.resize(npad8, zc(0, 0)); pb8.resize(npad8, zc(0, 0));
+        for (int c = 0; c < npad8 / 8; ++c) { pfe8[c] = pf8[c * 8 + 7]; pbs8[c] = pb8[c * 8]; }
         std::vector<double> pf8_re = re(pf8), pb8_re = re(pb8), pfe8_re = re(pfe8), pbs8_re = re(pbs8);
-        CU(h, put(pf8.data(), sizeof(zc) * n, (const void**)&A.pf8));
-        CU(h, put(pb8.data(), sizeof(zc) * n, (const void**)&A.pb8));
+        CU(h, put(pf8.data(), sizeof(zc) * npad8, (const void**)&A.pf8));
+        CU(h, put(pb8.data(), sizeof(zc) * npad8, (const void**)&A.pb8));
         CU(h, put(pfe8.data(), sizeof(zc) * 128, (const void**)&A.pfe8));
         CU(h, put(pbs8.data(), sizeof(zc) * 128, (const void**)&A.pbs8));
-        CU(h, put(pf8_re.data(), sizeof(double) * n, (const void**)&A.pf8_re));
-        CU(h, put(pb8_re.data(), sizeof(double) * n, (const void**)&A.pb8_re));
+        CU(h, put(pf8_re.data(), sizeof(double) * npad8, (const void**)&A.pf8_re));
+        CU(h, put(pb8_re.data(), sizeof(double) * npad8, (const void**)&A.pb8_re));
         CU(h, put(pfe8_re.data(), sizeof(double) * 128, (const void**)&A.pfe8_re));
         CU(h, put(pbs8_re.data(), sizeof(double) * 128, (const void**)&A.pbs8_re));
-        A.K8 = std::max(carry_terms(pfe8, n / 8), carry_terms(pbs8, n / 8));
+        A.K8 = std::max(1, std::max(carry_terms(pfe8, npad8 / 8), carry_terms(pbs8, npad8 / 8)));
         CU(h, cudaStreamSynchronize(h->stream));          // the host vectors of this block go out of scope
     }
     // the host vectors must outlive the asynchronous copies from pageable memory: those copies are
