@@ -45,6 +45,7 @@ extern "C" {
 #define DBEC_EWORKSPACE  -3   /* workspace NULL, misaligned or smaller than dbec_workspace_bytes    */
 #define DBEC_ECUDA       -4   /* a CUDA call failed; dbec_last_cuda_error gives the CUDA code       */
 #define DBEC_ENODEVICE   -5   /* no CUDA device / not an sm_100 device                              */
+#define DBEC_ENOALLOC_SIZE -6 /* dbec_norm_noalloc: more than DBEC_NOALLOC_MAX_POINTS points         */
 
 typedef struct dbec_handle_s* dbec_handle;
 
@@ -173,6 +174,21 @@ const char* dbec_kernel_name(int slot);
  * shorter ones in the one-tile-per-block kernels; on a small grid the only slot is the last one,
  * "sscn_step<cluster>" (k_small_step). */
 const char* dbec_pass_kernel(dbec_handle h, int slot);
+
+/* calcnorm for callers that may not allocate (CUDA graph capture, serving loops): the norm
+ * integral dV * sum |psi|^2 of npoints complex128 values, written to *norm_dev.  No handle, no workspace: the
+ * block partial sums live in a device array of DBEC_NOALLOC_SCRATCH_BYTES that is part of the library image
+ * (held by every GPU that loads the library, until exit); the call issues no cudaMalloc / cudaFree.
+ *   psi_c128_dev, norm_dev: DEVICE pointers (inputs and outputs stay the caller's); cuda_stream: a cudaStream_t
+ *   (NULL = the default stream).  Asynchronous on that stream; one memset node and one kernel.
+ *   npoints > DBEC_NOALLOC_MAX_POINTS -> DBEC_ENOALLOC_SIZE;  NULL pointer, npoints < 1, dV <= 0 -> DBEC_EINVAL;
+ *   a failed CUDA call -> DBEC_ECUDA with the CUDA code in dbec_noalloc_last_cuda_error() (per host thread).
+ * All calls on a device share the one array: calls that overlap on the GPU (different streams, several host
+ * threads) race; put them on one stream or serialise them.  Same fixed-order sum on every GPU. */
+#define DBEC_NOALLOC_MAX_POINTS    134217728LL     /* 2^27 */
+#define DBEC_NOALLOC_SCRATCH_BYTES 262400          /* 32768 partial sums + a 256-byte ticket */
+int dbec_norm_noalloc(const void* psi_c128_dev, long long npoints, double dV, double* norm_dev, void* cuda_stream);
+int dbec_noalloc_last_cuda_error(void);
 
 int dbec_version(void);
 /* "DBEC_BUILD_ID=<hash of the sources this library was built from>" (paper_1601_04640_b200/build.py). */

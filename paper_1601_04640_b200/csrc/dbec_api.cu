@@ -300,6 +300,7 @@ const char* dbec_strerror(int code) {
         case DBEC_EWORKSPACE: return "workspace missing, misaligned or too small";
         case DBEC_ECUDA: return "CUDA error (see dbec_last_cuda_error)";
         case DBEC_ENODEVICE: return "no sm_100 CUDA device";
+        case DBEC_ENOALLOC_SIZE: return "dbec_norm_noalloc: more points than DBEC_NOALLOC_MAX_POINTS (2^27)";
         default: return "unknown error";
     }
 }

@@ -23,7 +23,8 @@ EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi"
            "dbec_phi_dd", "dbec_cn_sweep", "dbec_nonlinear", "dbec_normalize", "dbec_launch_count",
            "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel", "dbec_build_id",
            "dbec_set_ramp", "dbec_workspace_bytes_batch", "dbec_create_batch", "dbec_batch_size",
-           "dbec_set_coupling_batch", "dbec_observables_batch", "dbec_density_1d", "dbec_density_2d"]
+           "dbec_set_coupling_batch", "dbec_observables_batch", "dbec_density_1d", "dbec_density_2d",
+           "dbec_norm_noalloc", "dbec_noalloc_last_cuda_error"]
 KERNEL_SLOTS = 9
 
 
@@ -98,6 +99,8 @@ def lib():
         L.dbec_density_2d.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.dbec_build_id.argtypes = []
         L.dbec_build_id.restype = C.c_char_p
+        L.dbec_norm_noalloc.argtypes = [vp, C.c_longlong, C.c_double, vp, vp]
+        L.dbec_noalloc_last_cuda_error.argtypes = []
         _lib = L
     return _lib
 
@@ -273,3 +276,23 @@ class Dbec:
 
     def synchronize(self):
         self.stream.synchronize()
+
+
+NOALLOC_MAX_POINTS = 1 << 27       # include/dbec.h: DBEC_NOALLOC_MAX_POINTS
+
+
+def norm_noalloc(psi, dV: float, out=None, stream=None):
+    """dbec_norm_noalloc: dV * sum |psi|^2 of a CUDA complex128 tensor, written into `out` (a one-element CUDA
+    float64 tensor, made here if not given — the C call itself allocates nothing).  Asynchronous on `stream`
+    (default: torch's current stream).  Calls that overlap on the GPU share one scratch array and race."""
+    import torch
+    assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous()
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=psi.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1
+    with torch.cuda.device(psi.device):
+        st = stream if stream is not None else torch.cuda.current_stream(psi.device)
+        rc = lib().dbec_norm_noalloc(psi.data_ptr(), psi.numel(), float(dV), out.data_ptr(), st.cuda_stream)
+    if rc:
+        raise DbecError(rc, "dbec_norm_noalloc", lib().dbec_noalloc_last_cuda_error())
+    return out
