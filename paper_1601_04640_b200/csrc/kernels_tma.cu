@@ -35,6 +35,8 @@ struct TileGeom {
     PaceState* pace;               // the launch's shared lag word
     int ystep;       // z passes: rows of y per tile (1, or 2 when a tile is 8 columns x 2 rows of y: k_cn_tma with TC = 16)
     int rev;         // walk the tiles last to first (so that a pass starts on what the previous one left in L2)
+    int fold_pairs;  // fused z pass: outer coordinates in the order 0, 1, NY-1, 2, NY-2, ... so that the two rows k_y and
+                     // NY - k_y, which read the same V_dd tile, are worked on at the same time (the second read hits L2)
     float pol_ld, pol_st;   // L2 eviction policy codes of the tile loads / stores (tma_pipe.cuh: l2_policy_code)
 };
 
@@ -58,7 +60,9 @@ template <int NST> __device__ __forceinline__ PipeBars pipe_init(uint64_t* bars,
 
 __device__ __forceinline__ void tile_coords(const TileGeom& tg, int t, int b, int inner, int& c0, int& c1, int& c2) {
     if (tg.rev) t = tg.ntiles - 1 - t;
-    const int tx = t % tg.ntiles_x, o = t / tg.ntiles_x + tg.outer0;
+    const int tx = t % tg.ntiles_x;
+    int o = t / tg.ntiles_x + tg.outer0;
+    if (tg.fold_pairs && o > 0) o = (o & 1) ? (o + 1) >> 1 : tg.fold_pairs - (o >> 1);
     c0 = tx * inner;
     c1 = tg.axis == 1 ? b * tg.box_rows : o * tg.ystep;
     c2 = tg.axis == 1 ? o : b * tg.box_rows;
@@ -395,6 +399,7 @@ static TileGeom geom_of(const dbec_handle_s* h, int axis, bool sp, int z0, int n
     TileGeom tg;
     tg.rev = h->rev_next;
     tg.ystep = 1;
+    tg.fold_pairs = 0;
     tg.pace_ns = 0; tg.pace_head = 0; tg.pace_head_ns = 0; tg.pace = nullptr;
     const int row_elems = sp ? h->nxhp : h->nx;          // a pass over the half spectrum or over psi
     tg.pol_ld = h->pol[sp ? POL_FFT_LD : POL_CN_LD];
@@ -497,6 +502,8 @@ template <int N, int MODE, int NG, int NST> static int launch_fft_tma(dbec_handl
     constexpr int GT = P::T * TCOLS;
     constexpr int STAGE = N * TCOLS * (int)sizeof(cd) + (MODE == 2 ? fmi_extra_bytes(N) : 0);
     TileGeom tg = geom_of(h, axis, true, z0, nzs);
+    // (measured: the step 480.3 -> 478.7 us at 256^3, 1951.7 -> 1949.5 at 512 x 512 x 256)
+    if (MODE == 2 && axis == 2 && h->ny % 2 == 0) tg.fold_pairs = h->ny;
     const int grid = grid_of(h, tg.ntiles);
     set_pace(h, &tg, grid, (size_t)STAGE + N * TCOLS * sizeof(cd), 16.0 * (double)h->SP * h->nb);
     const size_t sm = 128 + (size_t)NST * STAGE + (3 * NST + 4) * sizeof(uint64_t) + 2 * N * sizeof(cd);
