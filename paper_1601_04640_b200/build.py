@@ -18,7 +18,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdbec.so")
-SOURCES = ["kernels_fft.cu", "kernels_cn.cu", "kernels_tma.cu", "kernels_xline.cu", "kernels_xwarp.cu", "kernels_gen.cu", "kernels_small.cu", "kernels_noalloc.cu", "dbec_api.cu"]
+SOURCES = ["kernels_fft.cu", "kernels_cn.cu", "kernels_tma.cu", "kernels_xline.cu", "kernels_xwarp.cu", "kernels_gen.cu", "kernels_small.cu", "kernels_small_p2.cu", "kernels_noalloc.cu", "dbec_api.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

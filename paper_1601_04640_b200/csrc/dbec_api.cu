@@ -418,6 +418,10 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
         if (req > 0 && req != 1 && req != 2 && req != 4 && req != 8 && req != 16) req = -1;
         h->use_cluster = dbec_small_choose(h, req);
         h->use_small = h->use_cluster > 0;
+        // the automatic choice takes the compiled power-of-two variant where there is one (DBEC_SMALL_P2=0: never)
+        const char* p2 = getenv("DBEC_SMALL_P2");
+        h->use_small_p2 = 0;
+        if (req < 0 && !(p2 && atoi(p2) == 0) && dbec_small_p2_choose(h)) { h->use_small_p2 = 1; h->use_small = 1; h->use_cluster = 16; }
     }
     if (h->use_tma) TRY((cudaError_t)dbec_make_tensor_maps(h));
     if (init_scalars(h)) FAIL(DBEC_ECUDA);
@@ -657,7 +661,7 @@ const char* dbec_kernel_name(int slot) {
 const char* dbec_pass_kernel(dbec_handle h, int slot) {
     if (!h || slot < 0 || slot >= DBEC_MAX_KERNELS) return "";
     const int last_axis = h->p.ndim == 3 ? 2 : 1;
-    if (h->use_small) return slot == KS_SMALL_STEP ? "k_small_step" : "";      // dbec_step launches nothing else
+    if (h->use_small) return slot == KS_SMALL_STEP ? (h->use_small_p2 ? "k_small_p2" : "k_small_step") : "";      // dbec_step launches nothing else
     switch (slot) {
         case KS_DENS_FFTX: return h->gen[0] ? "k_gen_density_fftx" : dbec_xline_supported(h) ? "k_xline_density" : "k_density_fftx";
         case KS_FFT_Y_FWD: case KS_FFT_Y_INV:

@@ -123,6 +123,7 @@ struct dbec_handle_s {
                                     // env DBEC_CLUSTER = 0 / 1 / 2 / 4 / 8 / 16 overrides the choice)
     int use_small;                  // 1: dbec_step runs k_small_step (use_cluster > 0)
     int small_max_clusters;         // clusters of k_small_step that can be resident at once (0: not asked yet)
+    int use_small_p2;               // 1: the small-grid step runs in k_small_p2 (kernels_small_p2.cu: compiled power-of-two shapes)
     double pace_gbs;                // bandwidth the streaming passes are paced to, GB/s (tma_pipe.cuh: pace_wait); 0 = off
     long long l2_bytes;             // L2 cache size of the device
     double pace_head_speed;         // time per tile of the L2-resident head of a pass relative to the paced time
@@ -173,6 +174,8 @@ int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance);  
 // the whole step of a small grid in one launch by one thread-block cluster (kernels_small.cu)
 int dbec_small_choose(dbec_handle_s* h, int request);     // CTAs per cluster (0: multi-launch path); request < 0: auto
 int dbec_launch_small_step(dbec_handle_s* h, int nsteps);
+int dbec_small_p2_choose(dbec_handle_s* h);               // 1: k_small_p2 serves this handle (sets small_max_clusters)
+int dbec_launch_small_p2(dbec_handle_s* h, int nsteps);
 // one warp per line pair (kernels_xwarp.cu): a3 (x) + a4 + a5 for lines of 128 / 256 points
 int dbec_xwarp_supported(const dbec_handle_s* h);
 int dbec_launch_xwarp_nonlin(dbec_handle_s* h);

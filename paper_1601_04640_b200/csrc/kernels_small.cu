@@ -468,5 +468,6 @@ template <bool RT> static int launch_small(dbec_handle_s* h, int nsteps) {
 }
 
 int dbec_launch_small_step(dbec_handle_s* h, int nsteps) {
+    if (h->use_small_p2) return dbec_launch_small_p2(h, nsteps);
     return h->p.time_mode == 1 ? launch_small<true>(h, nsteps) : launch_small<false>(h, nsteps);
 }

@@ -208,6 +208,10 @@ def one_step_pair(gp, ob, w, psi0, steps=1):
     return sim, o, got, ref
 
 
+# shapes kernels_small_p2.cu is compiled for (the one-launch step with compile-time power-of-two lengths)
+P2_SHAPES = [(16, 16, 16), (32, 32, 32), (32, 32, 64), (64, 64, 16)]
+
+
 def small_step_cases():
     """(workload, cluster): "auto" = small 3-D grids take the one-launch cluster step (kernels_small.cu), everything
     else the multi-launch path; "0" = the multi-launch path also on the grids "auto" gives to the cluster step."""
@@ -216,6 +220,8 @@ def small_step_cases():
         out.append((w, "auto"))
         if w.ndim == 3 and w.npoints <= 65536:
             out.append((w, "0"))
+            if (w.nx, w.ny, w.nz) in P2_SHAPES:
+                out.append((w, "general"))      # "auto" is k_small_p2 there: this one is k_small_step
     return out
 
 
@@ -223,8 +229,12 @@ def small_step_cases():
 def test_one_step_small_grids(gp, ob, w, cluster, monkeypatch):
     if cluster == "0":
         monkeypatch.setenv("DBEC_CLUSTER", "0")
+    if cluster == "general":
+        monkeypatch.setenv("DBEC_SMALL_P2", "0")
     psi0 = random_psi(w, 9) if w.time_mode == REAL else initial_psi(w)
     sim, o, got, ref = one_step_pair(gp, ob, w, psi0)
+    if cluster != "0" and (w.nx, w.ny, w.nz) in P2_SHAPES:
+        assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_step" if cluster == "general" else "k_small_p2"}
     assert relerr(got, ref) < PSI_TOL
     a, b = sim.observables(), o.observables()
     for k in b:
@@ -389,15 +399,18 @@ def test_cluster_step_matches_oracle_and_multi_launch(gp, ob, w, cs, monkeypatch
     ml.close()
 
 
-def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch):
+@pytest.mark.parametrize("p2", ["1", "0"])
+def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch, p2):
     """A batch on the cluster step (one cluster per member, per-member couplings, the NSTP ramp advancing inside a
-    launch) and the automatic choice: small 3-D grids only, and only while every member gets a resident cluster."""
+    launch) and the automatic choice: small 3-D grids only, and only while every member gets a resident cluster.
+    p2: with / without the variant compiled for power-of-two shapes (kernels_small_p2.cu)."""
     monkeypatch.delenv("DBEC_CLUSTER", raising=False)
+    monkeypatch.setenv("DBEC_SMALL_P2", p2)
     w = grid3(32, 32, 32, IMAG, G=0.0, D=0.0)
     nb = 3
     psis = np.stack([random_psi(w, 50 + m) for m in range(nb)])
     sim = gp.Dbec(gp.params_of(w), nbatch=nb)
-    assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_step"}
+    assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_p2" if p2 == "1" else "k_small_step"}
     sim.set_psi(psis)
     sim.set_ramp(4, 0.0, 0.0, 40.0, 25.0)
     sim.step(6)                                       # the ramp ends inside the launch
@@ -417,6 +430,32 @@ def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch):
         h = gp.Dbec(gp.params_of(wl), nbatch=nbatch)
         assert ("sscn_step<cluster>" in h.pass_kernels()) == small, (wid(wl), nbatch)
         h.close()
+
+
+@pytest.mark.parametrize("shape", P2_SHAPES)
+@pytest.mark.parametrize("mode", [IMAG, REAL])
+def test_power_of_two_cluster_step_matches_oracle_and_general_kernel(gp, ob, shape, mode, monkeypatch):
+    """k_small_p2 on every shape it is compiled for: five steps in one launch against the oracle (imaginary time:
+    the norm factor is carried from step to step inside the launch) and against k_small_step on the same input."""
+    monkeypatch.delenv("DBEC_CLUSTER", raising=False)
+    monkeypatch.delenv("DBEC_SMALL_P2", raising=False)
+    w = grid3(*shape, mode, d=(0.4, 0.35, 0.5))
+    psi0 = random_psi(w, 77) if mode == REAL else 1.3 * initial_psi(w)
+    sim, o, got, ref = one_step_pair(gp, ob, w, psi0, steps=5)
+    assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_p2"}
+    assert relerr(got, ref) < 5 * PSI_TOL
+    a, b = sim.observables(), o.observables()
+    for k in b:
+        assert abs(a[k] - b[k]) <= OBS_TOL * max(abs(b[k]), 1e-300), k
+    sim.close()
+    o.close()
+    monkeypatch.setenv("DBEC_SMALL_P2", "0")
+    gen = gp.Dbec(gp.params_of(w))
+    assert gen.pass_kernels() == {"sscn_step<cluster>": "k_small_step"}
+    gen.set_psi(psi0)
+    gen.step(5)
+    assert relerr(got, gen.get_psi()) < 5 * PSI_TOL
+    gen.close()
 
 
 @pytest.mark.parametrize("shape,mode", [((256, 128, 256), REAL), ((128, 128, 128), IMAG), ((256, 256, 64), IMAG),
