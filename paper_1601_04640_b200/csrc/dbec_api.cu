@@ -418,10 +418,15 @@ int dbec_create_batch(const dbec_params* p, int nbatch, void* dev_workspace, siz
         if (req > 0 && req != 1 && req != 2 && req != 4 && req != 8 && req != 16) req = -1;
         h->use_cluster = dbec_small_choose(h, req);
         h->use_small = h->use_cluster > 0;
-        // the automatic choice takes the compiled power-of-two variant where there is one (DBEC_SMALL_P2=0: never)
+        // the automatic choice takes the compiled power-of-two variant where there is one (DBEC_SMALL_P2=0: never;
+        // DBEC_SMALL_P2_CS=1, 4, 8, 16: only with that many CTAs per cluster)
         const char* p2 = getenv("DBEC_SMALL_P2");
+        const char* p2cs = getenv("DBEC_SMALL_P2_CS");
         h->use_small_p2 = 0;
-        if (req < 0 && !(p2 && atoi(p2) == 0) && dbec_small_p2_choose(h)) { h->use_small_p2 = 1; h->use_small = 1; h->use_cluster = 16; }
+        if (req < 0 && !(p2 && atoi(p2) == 0)) {
+            const int cs = dbec_small_p2_choose(h, p2cs ? atoi(p2cs) : -1);
+            if (cs > 0) { h->use_small_p2 = 1; h->use_small = 1; h->use_cluster = cs; }
+        }
     }
     if (h->use_tma) TRY((cudaError_t)dbec_make_tensor_maps(h));
     if (init_scalars(h)) FAIL(DBEC_ECUDA);

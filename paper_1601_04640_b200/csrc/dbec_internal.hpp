@@ -174,7 +174,7 @@ int dbec_launch_xline_density(dbec_handle_s* h, int z0, int nzs, int advance);  
 // the whole step of a small grid in one launch by one thread-block cluster (kernels_small.cu)
 int dbec_small_choose(dbec_handle_s* h, int request);     // CTAs per cluster (0: multi-launch path); request < 0: auto
 int dbec_launch_small_step(dbec_handle_s* h, int nsteps);
-int dbec_small_p2_choose(dbec_handle_s* h);               // 1: k_small_p2 serves this handle (sets small_max_clusters)
+int dbec_small_p2_choose(dbec_handle_s* h, int request);  // CTAs per cluster when k_small_p2 serves this handle, else 0 (sets small_max_clusters)
 int dbec_launch_small_p2(dbec_handle_s* h, int nsteps);
 // one warp per line pair (kernels_xwarp.cu): a3 (x) + a4 + a5 for lines of 128 / 256 points
 int dbec_xwarp_supported(const dbec_handle_s* h);

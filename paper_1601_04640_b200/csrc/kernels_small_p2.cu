@@ -22,7 +22,6 @@ namespace cg = cooperative_groups;
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
 constexpr int P2T = 512;            // threads per CTA
-constexpr int P2CS = 16;            // CTAs per cluster
 constexpr int P2L = 8;              // points per Crank-Nicolson chunk
 
 template <int N> struct P2Plan;
@@ -98,9 +97,10 @@ __device__ __forceinline__ double p2_block_sum_all(double x, double* red) {
 }
 
 // Shared-memory layout (elements of cd unless noted), the same on host and device.
-template <bool RT, int NX, int NY, int NZ> struct P2Lay {
+template <bool RT, int NX, int NY, int NZ, int CS> struct P2Lay {
+    static_assert(NZ % CS == 0 && (NZ / CS * NY) % 2 == 0, "whole planes and whole pairs of rows per CTA");
     typedef typename P2Plan<NX>::P PX; typedef typename P2Plan<NY>::P PY; typedef typename P2Plan<NZ>::P PZ;
-    static constexpr int PPC = NZ / P2CS;                 // planes per CTA
+    static constexpr int PPC = NZ / CS;                 // planes per CTA
     static constexpr int R = PPC * NY, NP = R / 2;        // rows / pairs of rows a CTA holds
     static constexpr int NXH1 = NX / 2 + 1;               // half-spectrum length
     // a psi row in shared memory: point x at x + x/8 (p2_skew: the chunks of a row start in different bank groups),
@@ -123,10 +123,10 @@ template <bool RT, int NX, int NY, int NZ> struct P2Lay {
     static constexpr size_t bytes = (size_t)total * sizeof(cd);
 };
 
-template <bool RT, int NX, int NY, int NZ>
+template <bool RT, int NX, int NY, int NZ, int CS>
 __global__ void __launch_bounds__(P2T, 1)
 k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, CnTab<RT> cnz_g) {
-    typedef P2Lay<RT, NX, NY, NZ> LY;
+    typedef P2Lay<RT, NX, NY, NZ, CS> LY;
     typedef typename LY::PX PX; typedef typename LY::PY PY; typedef typename LY::PZ PZ;
     typedef typename CnCoef<RT>::type CT;
     constexpr int R = LY::R, NP = LY::NP, NXH1 = LY::NXH1, PP = LY::PP, PPC = LY::PPC;
@@ -138,7 +138,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
     __shared__ double cpart;                    // this CTA's part of sum |psi|^2, read by the whole cluster
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (int)cluster.block_rank();
-    const int cid = (int)(blockIdx.x / P2CS), ncl = (int)(gridDim.x / P2CS);
+    const int cid = (int)(blockIdx.x / CS), ncl = (int)(gridDim.x / CS);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     cd* Pb = psm + LY::o_pb; cd* ZB = psm + LY::o_zb; cd* XB = psm + LY::o_xb;
     cd* scr = psm + LY::o_scr + warp * LY::SCRW;
@@ -161,7 +161,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
     const int nxhp = a.nxhp;
     const size_t ls_spec = (size_t)NY * nxhp, ls_psi = (size_t)NY * NX, vls = (size_t)a.nyf * nxhp;
     const int r0 = rank * R;                                     // this CTA's first row z NY + y
-    constexpr int QS = NY * NXH1, qs = (QS + P2CS - 1) / P2CS, QP = NY * NX, qp = (QP + P2CS - 1) / P2CS;
+    constexpr int QS = NY * NXH1, qs = (QS + CS - 1) / CS, QP = NY * NX, qp = (QP + CS - 1) / CS;
     const int qs_lo = min(QS, rank * qs), ncs = min(QS, qs_lo + qs) - qs_lo;      // last-axis columns of the spectrum
     const int qp_lo = min(QP, rank * qp), ncp = min(QP, qp_lo + qp) - qp_lo;      // ... of psi
     const cd zero = cmake(0.0, 0.0);
@@ -247,6 +247,15 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     for (int j = 0; j < 4; ++j) gc[(j * TZ + m) * ls_spec] = v[j];
                 }
             }
+            // psi of this CTA's rows for the first round of pass C: pass B does not touch psi, so the loads fly
+            // while the cluster barrier and the inverse y transforms run
+            cd q0[4], q1[4];
+            {
+                const int line = tid / TX, m = tid % TX;
+                const cd* g0 = psi + (size_t)(r0 + 2 * (line < NP ? line : 0)) * NX;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { q0[j] = p2_ldcg(g0 + j * TX + m); q1[j] = p2_ldcg(g0 + NX + j * TX + m); }
+            }
             cluster.sync();
             // ---------------- C: inverse FFT-y -> merge -> inverse FFT-x -> calcnu -> calclux -> calcluy ----------------
             for (int base = 0; base < (PPC * NXH1 + LPWY - 1) / LPWY * 32; base += P2T) {
@@ -273,12 +282,11 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     const cd* ra = XB + (2 * l) * NXH1;
                     const cd* rb = ra + NXH1;
                     const cd* g0 = psi + (size_t)(r0 + 2 * l) * NX;
-                    cd v[4], q0[4], q1[4];
+                    cd v[4];
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int kk = j * TX + m;
-                        q0[j] = act ? p2_ldcg(g0 + kk) : zero;
-                        q1[j] = act ? p2_ldcg(g0 + NX + kk) : zero;
+                        if (base > 0) { q0[j] = p2_ldcg(g0 + kk); q1[j] = p2_ldcg(g0 + NX + kk); }
                         // X_a + i X_b on 0 .. N/2, the conjugates above
                         if (kk <= NX / 2) { const cd p = ra[kk], q = rb[kk]; v[j] = cmake(p.x - q.y, p.y + q.x); }
                         else { const cd p = ra[NX - kk], q = rb[NX - kk]; v[j] = cmake(p.x + q.y, q.x - p.y); }
@@ -368,7 +376,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                 // calcnorm (reading S13): the CTAs' partial sums in rank order, the same in every CTA
                 if (tid == 0) {
                     double tot = 0.0;
-                    for (int r = 0; r < P2CS; ++r) tot += *cluster.map_shared_rank(&cpart, r);
+                    for (int r = 0; r < CS; ++r) tot += *cluster.map_shared_rank(&cpart, r);
                     const double sf = 1.0 / sqrt(tot * a.dV);
                     sc[SC_S] = sf; sc[SC_S2] = sf * sf;
                 }
@@ -395,24 +403,24 @@ template <> CnTab<false> p2_cntab8<false>(const AxisTables& a) {
     return t;
 }
 
-static void p2_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, size_t smem, int nclusters, cudaStream_t st) {
+static void p2_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, size_t smem, int cs, int nclusters, cudaStream_t st) {
     *cfg = cudaLaunchConfig_t();
-    cfg->gridDim = dim3(P2CS * nclusters); cfg->blockDim = dim3(P2T); cfg->dynamicSmemBytes = smem; cfg->stream = st;
+    cfg->gridDim = dim3(cs * nclusters); cfg->blockDim = dim3(P2T); cfg->dynamicSmemBytes = smem; cfg->stream = st;
     at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = P2CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg->attrs = at; cfg->numAttrs = 1;
 }
 
 // what = 0: clusters of this instantiation that can be resident at once (0: cannot run); what = 1: launch nsteps steps
-template <bool RT, int NX, int NY, int NZ> static int p2_run(dbec_handle_s* h, int what, int nsteps) {
-    auto k = k_small_p2<RT, NX, NY, NZ>;
-    const size_t smem = P2Lay<RT, NX, NY, NZ>::bytes;
+template <bool RT, int NX, int NY, int NZ, int CS> static int p2_run(dbec_handle_s* h, int what, int nsteps) {
+    auto k = k_small_p2<RT, NX, NY, NZ, CS>;
+    const size_t smem = P2Lay<RT, NX, NY, NZ, CS>::bytes;
     cudaLaunchConfig_t cfg;
     cudaLaunchAttribute at[1];
     if (what == 0) {
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
             cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
-        p2_config(&cfg, at, smem, 1, h->stream);
+        p2_config(&cfg, at, smem, CS, 1, h->stream);
         int n = 0;
         if (cudaOccupancyMaxActiveClusters(&n, k, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
         return n;
@@ -424,32 +432,50 @@ template <bool RT, int NX, int NY, int NZ> static int p2_run(dbec_handle_s* h, i
     a.dt = h->p.dt; a.dV = h->dV; a.P = h->P; a.SP = h->SP;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    p2_config(&cfg, at, smem, h->nb < h->small_max_clusters ? h->nb : h->small_max_clusters, h->stream);
+    p2_config(&cfg, at, smem, CS, h->nb < h->small_max_clusters ? h->nb : h->small_max_clusters, h->stream);
     CK(cudaLaunchKernelEx(&cfg, k, a, p2_cntab8<RT>(h->ax[0]), p2_cntab8<RT>(h->ax[1]), p2_cntab8<RT>(h->ax[2])));
     h->launches++;
     return (int)cudaGetLastError();
 }
 
-// the shapes this file is compiled for
-#define P2_SHAPES(X) X(16, 16, 16) X(32, 32, 32) X(32, 32, 64) X(64, 64, 16)
+// the shapes and cluster sizes this file is compiled for (NX, NY, NZ, CTAs per cluster); a smaller cluster gives
+// a member fewer SMs and a batch more members in flight
+#define P2_SHAPES(X) X(16, 16, 16, 16) X(16, 16, 16, 4) X(16, 16, 16, 1) X(32, 32, 32, 16) X(32, 32, 32, 8) \
+                     X(32, 32, 64, 16) X(64, 64, 16, 16)
+static const int p2_cluster_sizes[] = {16, 8, 4, 1};
 
-static int p2_dispatch(dbec_handle_s* h, int what, int nsteps) {
+static int p2_dispatch(dbec_handle_s* h, int cs, int what, int nsteps) {
     const bool rt = h->p.time_mode == 1;
-#define P2_CASE(NX, NY, NZ) \
-    if (h->nx == NX && h->ny == NY && h->nz == NZ) return rt ? p2_run<true, NX, NY, NZ>(h, what, nsteps) : p2_run<false, NX, NY, NZ>(h, what, nsteps);
+#define P2_CASE(NX, NY, NZ, CS) \
+    if (h->nx == NX && h->ny == NY && h->nz == NZ && cs == CS) \
+        return rt ? p2_run<true, NX, NY, NZ, CS>(h, what, nsteps) : p2_run<false, NX, NY, NZ, CS>(h, what, nsteps);
     P2_SHAPES(P2_CASE)
 #undef P2_CASE
     return what == 0 ? 0 : (int)cudaErrorInvalidValue;
 }
 
-// 1 (and h->small_max_clusters set) when dbec_step of this handle can run in k_small_p2: a 3-D grid of one of the
-// compiled shapes, the 8-point chunk tables built, every batch member a resident cluster of its own.
-int dbec_small_p2_choose(dbec_handle_s* h) {
+// CTAs per cluster (and h->small_max_clusters set) when dbec_step of this handle can run in k_small_p2 — a 3-D grid
+// of one of the compiled shapes with the 8-point chunk tables built — else 0.  request > 0: that cluster size or
+// nothing.  Otherwise the choice is by the time one step of the whole batch takes: a cluster works through
+// ceil(nb / resident clusters) members one after the other, and a member's step on CS CTAs costs about
+// p2_step_cost(CS) relative to 16 CTAs (measured on B200: 32^3 16.9 us on 16 CTAs, 23.3 on 8; 16^3 11.3 us on 16,
+// 11.8 on 4, 20.7 on 1 — so 64 members of 32^3 go through 8-CTA clusters, 117 us per batch step against 169 on 16 CTAs
+// and 151 through the seven launches, and 256 members of 16^3 through single CTAs, 42 us against 149).
+static double p2_step_cost(int cs) { return cs >= 16 ? 1.0 : cs == 8 ? 1.4 : cs == 4 ? 1.05 : 1.85; }
+
+int dbec_small_p2_choose(dbec_handle_s* h, int request) {
     if (h->p.ndim != 3 || h->ax[0].K8 < 1 || h->ax[1].K8 < 1 || h->ax[2].K8 < 1) return 0;
-    const int n = p2_dispatch(h, 0, 0);
-    if (n < 1 || n < h->nb) return 0;
-    h->small_max_clusters = n;
-    return 1;
+    int best = 0, best_n = 0;
+    double best_t = 0.0;
+    for (int cs : p2_cluster_sizes) {
+        if (request > 0 && cs != request) continue;
+        const int n = p2_dispatch(h, cs, 0, 0);
+        if (n < 1) continue;
+        const double t = (double)((h->nb + n - 1) / n) * p2_step_cost(cs);
+        if (!best || t < best_t) { best = cs; best_n = n; best_t = t; }
+    }
+    if (best) h->small_max_clusters = best_n;
+    return best;
 }
 
-int dbec_launch_small_p2(dbec_handle_s* h, int nsteps) { return p2_dispatch(h, 1, nsteps); }
+int dbec_launch_small_p2(dbec_handle_s* h, int nsteps) { return p2_dispatch(h, h->use_cluster, 1, nsteps); }

@@ -425,7 +425,8 @@ def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch, p2):
             o.step(1)
         assert relerr(got[m], o.get_psi()) < PSI_TOL, m
         o.close()
-    for wl, nbatch, small in ((grid3(32, 32, 32, REAL), 1, True), (grid3(32, 32, 32, REAL), 200, False),
+    # (k_small_p2 walks a batch through its resident clusters, k_small_step wants a cluster per member)
+    for wl, nbatch, small in ((grid3(32, 32, 32, REAL), 1, True), (grid3(32, 32, 32, REAL), 200, p2 == "1"),
                               (grid2(128, 128, REAL), 1, False), (grid3(64, 64, 32, IMAG), 1, False)):
         h = gp.Dbec(gp.params_of(wl), nbatch=nbatch)
         assert ("sscn_step<cluster>" in h.pass_kernels()) == small, (wid(wl), nbatch)
@@ -456,6 +457,34 @@ def test_power_of_two_cluster_step_matches_oracle_and_general_kernel(gp, ob, sha
     gen.step(5)
     assert relerr(got, gen.get_psi()) < 5 * PSI_TOL
     gen.close()
+
+
+@pytest.mark.parametrize("n,cs,nb", [(32, 8, 1), (32, 8, 40), (32, 16, 21), (16, 4, 1), (16, 1, 1), (16, 1, 300), (16, 4, 75)])
+@pytest.mark.parametrize("mode", [IMAG, REAL])
+def test_power_of_two_cluster_step_cluster_sizes_and_batches(gp, ob, n, cs, nb, mode, monkeypatch):
+    """k_small_p2 with fewer CTAs per cluster (DBEC_SMALL_P2_CS) and with more batch members than resident clusters
+    (a cluster then works through several members one after the other): four steps in one launch against the
+    oracle on the first, a middle and the last member."""
+    monkeypatch.delenv("DBEC_CLUSTER", raising=False)
+    monkeypatch.delenv("DBEC_SMALL_P2", raising=False)
+    monkeypatch.setenv("DBEC_SMALL_P2_CS", str(cs))
+    w = grid3(n, n, n, mode, d=(0.5, 0.45, 0.4))
+    rng = np.random.default_rng(7)
+    scale = 1.0 + 0.5 * rng.random(nb)
+    base = random_psi(w, 31) if mode == REAL else initial_psi(w)
+    psis = np.stack([scale[m] * base for m in range(nb)]) if nb > 1 else base
+    sim = gp.Dbec(gp.params_of(w), nbatch=nb)
+    assert sim.pass_kernels() == {"sscn_step<cluster>": "k_small_p2"}
+    sim.set_psi(psis)
+    sim.step(4)
+    got = sim.get_psi()
+    sim.close()
+    for m in sorted({0, nb // 2, nb - 1}):
+        o = ob.Oracle(ob.params_of(w))
+        o.set_psi(psis[m] if nb > 1 else psis)
+        o.step(4)
+        assert relerr(got[m] if nb > 1 else got, o.get_psi()) < 5 * PSI_TOL, m
+        o.close()
 
 
 @pytest.mark.parametrize("shape,mode", [((256, 128, 256), REAL), ((128, 128, 128), IMAG), ((256, 256, 64), IMAG),
