@@ -88,6 +88,19 @@ int dbec_set_psi(dbec_handle h, const void* psi_c128, int on_device);
 /* Copy psi out (same pointer rules), with the deferred imaginary-time norm factor applied. */
 int dbec_get_psi(dbec_handle h, void* psi_c128, int on_device);
 
+/* The same two copies for PINNED host buffers (cudaHostAlloc / cudaHostRegister), without the host synchronisation:
+ * the copy is enqueued on the handle's stream and the call returns at once, so the transfers of one handle overlap
+ * the steps and the opposite-direction transfers of another (two handles on two streams keep both directions of
+ * the host link busy — how bench.py's end-to-end leg feeds the GPU).  The buffer must stay valid and untouched
+ * until the stream has passed the copy: dbec_synchronize, or the caller's own event on that stream.  With pageable
+ * memory CUDA stages the copy and the call may block; the result is the same.  Only the state handed over
+ * changes hands ("only wave function array is returned"); nothing else crosses the link. */
+int dbec_set_psi_async(dbec_handle h, const void* psi_c128_host);
+int dbec_get_psi_async(dbec_handle h, void* psi_c128_host);
+
+/* Block the calling host thread until everything enqueued on the handle's stream has finished. */
+int dbec_synchronize(dbec_handle h);
+
 /* Change G and D (quench, reading S18).  Takes effect from the next step; ends a running ramp.  On a batch
  * handle every member gets the same pair. */
 int dbec_set_coupling(dbec_handle h, double G, double D);

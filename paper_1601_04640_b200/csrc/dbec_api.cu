@@ -474,6 +474,26 @@ int dbec_get_psi(dbec_handle h, void* psi, int on_device) {
     return DBEC_OK;
 }
 
+int dbec_set_psi_async(dbec_handle h, const void* psi) {
+    if (!h || !psi) return DBEC_EINVAL;
+    CU(h, cudaMemcpyAsync(h->psi, psi, sizeof(cd) * h->P * h->nb, cudaMemcpyHostToDevice, h->stream));
+    LAUNCH(h, dbec_launch_reset_scale(h));             // a fresh field carries no deferred norm factor
+    return DBEC_OK;
+}
+
+int dbec_get_psi_async(dbec_handle h, void* psi) {
+    if (!h || !psi) return DBEC_EINVAL;
+    if (h->p.time_mode == 0) LAUNCH(h, dbec_launch_apply_scale(h));
+    CU(h, cudaMemcpyAsync(psi, h->psi, sizeof(cd) * h->P * h->nb, cudaMemcpyDeviceToHost, h->stream));
+    return DBEC_OK;
+}
+
+int dbec_synchronize(dbec_handle h) {
+    if (!h) return DBEC_EINVAL;
+    CU(h, cudaStreamSynchronize(h->stream));
+    return DBEC_OK;
+}
+
 // Columns SC_G .. SC_RN of every member: the current (G, D), then a ramp G0, D0, G1, D1, k = 0, n.
 static int write_couplings(dbec_handle h, const double* G, int gs, const double* D, int ds, int nstp, const double* G0,
                            const double* D0) {

@@ -24,7 +24,8 @@ EXPORTS = ["dbec_workspace_bytes", "dbec_create", "dbec_set_psi", "dbec_get_psi"
            "dbec_version", "dbec_step_profile", "dbec_kernel_name", "dbec_pass_kernel", "dbec_build_id",
            "dbec_set_ramp", "dbec_workspace_bytes_batch", "dbec_create_batch", "dbec_batch_size",
            "dbec_set_coupling_batch", "dbec_observables_batch", "dbec_density_1d", "dbec_density_2d",
-           "dbec_norm_noalloc", "dbec_noalloc_last_cuda_error"]
+           "dbec_norm_noalloc", "dbec_noalloc_last_cuda_error", "dbec_set_psi_async", "dbec_get_psi_async",
+           "dbec_synchronize"]
 KERNEL_SLOTS = 9
 
 
@@ -97,6 +98,9 @@ def lib():
         L.dbec_observables_batch.argtypes = [vp, C.POINTER(DbecObs)]
         L.dbec_density_1d.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.dbec_density_2d.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
+        L.dbec_set_psi_async.argtypes = [vp, vp]
+        L.dbec_get_psi_async.argtypes = [vp, vp]
+        L.dbec_synchronize.argtypes = [vp]
         L.dbec_build_id.argtypes = []
         L.dbec_build_id.restype = C.c_char_p
         L.dbec_norm_noalloc.argtypes = [vp, C.c_longlong, C.c_double, vp, vp]
@@ -197,6 +201,21 @@ class Dbec:
         if dev:
             self._torch.cuda.current_stream(self.device).wait_stream(self.stream)
         return out
+
+    def set_psi_async(self, host):
+        """dbec_set_psi_async: `host` a pinned CPU tensor / array of npoints complex128; returns at once."""
+        ptr, dev = self._ptr(host)
+        assert not dev, "set_psi_async takes a host buffer (device buffers: set_psi is asynchronous already)"
+        self._ck(lib().dbec_set_psi_async(self._h, C.c_void_p(ptr)), "dbec_set_psi_async")
+
+    def get_psi_async(self, host):
+        """dbec_get_psi_async: the copy into `host` (pinned) is complete after wait()."""
+        ptr, dev = self._ptr(host)
+        assert not dev, "get_psi_async takes a host buffer"
+        self._ck(lib().dbec_get_psi_async(self._h, C.c_void_p(ptr)), "dbec_get_psi_async")
+
+    def wait(self):
+        self._ck(lib().dbec_synchronize(self._h), "dbec_synchronize")
 
     def set_coupling(self, G, D):
         """Scalars: every member; sequences of nbatch values: per member."""

@@ -459,6 +459,37 @@ def test_power_of_two_cluster_step_matches_oracle_and_general_kernel(gp, ob, sha
     gen.close()
 
 
+@pytest.mark.parametrize("mode", [IMAG, REAL])
+def test_async_host_copies_on_two_handles_match_the_synchronous_calls(gp, mode):
+    """dbec_set_psi_async / dbec_get_psi_async / dbec_synchronize with pinned host buffers, two handles on two
+    streams taking turns (the end-to-end leg of bench.py): every result is bitwise what dbec_set_psi, dbec_step,
+    dbec_get_psi give on one handle."""
+    import torch
+    w = grid3(64, 32, 128, mode, d=(0.4, 0.3, 0.5))
+    inputs = [random_psi(w, 90 + i) for i in range(5)]
+    one = gp.Dbec(gp.params_of(w))
+    want = []
+    for psi in inputs:
+        one.set_psi(psi)
+        one.step(2)
+        want.append(one.get_psi().copy())
+    one.close()
+    pair = [gp.Dbec(gp.params_of(w)) for _ in range(2)]
+    h_in = [torch.from_numpy(psi.copy()).pin_memory() for psi in inputs]
+    h_out = [torch.empty_like(h_in[0]).pin_memory() for _ in inputs]
+    for i in range(len(inputs)):
+        s = pair[i & 1]
+        s.set_psi_async(h_in[i])
+        s.step(2)
+        s.get_psi_async(h_out[i])
+    for s in pair:
+        s.wait()
+    for i in range(len(inputs)):
+        assert np.array_equal(h_out[i].numpy(), want[i]), i
+    for s in pair:
+        s.close()
+
+
 @pytest.mark.parametrize("n,cs,nb", [(32, 8, 1), (32, 8, 40), (32, 16, 21), (16, 4, 1), (16, 1, 1), (16, 1, 300), (16, 4, 75)])
 @pytest.mark.parametrize("mode", [IMAG, REAL])
 def test_power_of_two_cluster_step_cluster_sizes_and_batches(gp, ob, n, cs, nb, mode, monkeypatch):
