@@ -10,6 +10,17 @@
 //   * global loads and stores go straight from / to the registers of the lane that needs them.
 // Six block barriers and four cluster barriers per step.  Results agree with k_small_step to round-off (another
 // summation order in the transforms); tests/test_gpu_parity.py runs both against the oracle.
+//
+// Cubes (NY == NZ) need only THREE cluster barriers per step: the roles of y and z alternate from step to step.
+// An even step works as described (planes of fixed z in A and C, lines along z in B and D) and ends with every
+// CTA holding, after its calcluz, all x and z for its own rows of y; the odd step that follows starts right
+// there, without a barrier: its "planes" are those of fixed y (A: density, FFT-x, FFT-z; C: inverse FFT-z,
+// inverse FFT-x, calcnu, calclux, calcluz) and its lines run along y (B: FFT-y, x V_dd, inverse; D: calcluy), which
+// leaves every CTA with the planes of fixed z the next even step begins on.  The transforms of the three axes
+// are applied in another order and calcluy / calcluz swap places — the sweeps act on different indices and
+// commute exactly (pinned for the oracle by tests/test_oracle_pins.py), so the difference is round-off.  In
+// imaginary time the norm factor is then read one barrier later (after pass A, whose density is linear in it:
+// pass B multiplies by s^2 instead).
 #include <cooperative_groups.h>
 #include "dbec_internal.hpp"
 #include "fft_linev.cuh"
@@ -159,12 +170,12 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
     for (int k = tid; k < NCHY; k += P2T) { tcy[3 * EY + k] = cny_g.pfe[k]; tcy[3 * EY + NCHY + k] = cny_g.pbs[k]; }
     for (int k = tid; k < NCHZ; k += P2T) { tcz[3 * EZ + k] = cnz_g.pfe[k]; tcz[3 * EZ + NCHZ + k] = cnz_g.pbs[k]; }
     const int nxhp = a.nxhp;
-    const size_t ls_spec = (size_t)NY * nxhp, ls_psi = (size_t)NY * NX, vls = (size_t)a.nyf * nxhp;
-    const int r0 = rank * R;                                     // this CTA's first row z NY + y
+    const size_t ls_spec = (size_t)NY * nxhp, vls = (size_t)a.nyf * nxhp;
     constexpr int QS = NY * NXH1, qs = (QS + CS - 1) / CS, QP = NY * NX, qp = (QP + CS - 1) / CS;
     const int qs_lo = min(QS, rank * qs), ncs = min(QS, qs_lo + qs) - qs_lo;      // last-axis columns of the spectrum
     const int qp_lo = min(QP, rank * qp), ncp = min(QP, qp_lo + qp) - qp_lo;      // ... of psi
     const cd zero = cmake(0.0, 0.0);
+    constexpr bool SWAP = NY == NZ;           // y and z may trade places (header comment)
 
     for (int mem = cid; mem < a.nb; mem += ncl) {
         cd* psi = a.psi + (size_t)mem * a.P;
@@ -173,22 +184,34 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
         __syncthreads();
         if (tid < SC_COUNT) sc[tid] = scal[tid];
         __syncthreads();
+        bool pending = false;           // imaginary time: the CTAs' parts of the last norm wait in cpart
         for (int step = 0; step < a.nsteps; ++step) {
             if (tid == 0) ramp_advance(sc);                      // reading S26 (G, D are used in pass C)
+            // this step's geometry: sw = y and z trade places.  Element strides of psi / spec: from plane to plane
+            // of this CTA's slab (psP, spP) and from row to row inside a plane (psQ, spQ); the lines of passes B
+            // and D run along the slab direction.  V_dd table: vQ per row, vL along the line.
+            const bool sw = SWAP && (step & 1);
+            const int psP = sw ? NX : NY * NX, psQ = sw ? NY * NX : NX;
+            const size_t spP = sw ? (size_t)nxhp : ls_spec, spQ = sw ? ls_spec : (size_t)nxhp;
+            const size_t vQ = sw ? vls : (size_t)nxhp, vL = sw ? (size_t)nxhp : vls;
+            const CT* tq = sw ? tcz : tcy; const CT* tl = sw ? tcy : tcz;       // Crank-Nicolson tables: in-plane, line
+            const CT kq = sw ? cnz_g.kap : cny_g.kap, kl = sw ? cny_g.kap : cnz_g.kap;
+            const double* vq = sw ? vzs : vys; const double* vp = sw ? vys : vzs;
             // ---------------- A: density -> FFT-x -> split -> FFT-y -> spectrum ----------------
             {
-                const cd* g = psi + (size_t)r0 * NX;
-                const double s2 = sc[SC_S2];
+                // (|psi|^2 without the norm factor: pass B multiplies by s^2)
                 for (int base = 0; base < NP * TX; base += P2T) {
                     const int item = base + tid, line = item / TX, m = item % TX;
                     const bool act = line < NP;
+                    const int r = act ? 2 * line : 0;
+                    const cd* g = psi + (size_t)(rank * PPC + r / NY) * psP + (size_t)(r % NY) * psQ;
                     cd v[4];
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         v[j] = zero;
                         if (act) {
-                            const cd p0 = p2_ldcg(g + (2 * line) * NX + j * TX + m), p1 = p2_ldcg(g + (2 * line + 1) * NX + j * TX + m);
-                            v[j] = cmake(s2 * cnorm2(p0), s2 * cnorm2(p1));
+                            const cd p0 = p2_ldcg(g + j * TX + m), p1 = p2_ldcg(g + psQ + j * TX + m);
+                            v[j] = cmake(cnorm2(p0), cnorm2(p1));
                         }
                     }
                     __syncwarp();
@@ -216,25 +239,38 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                 fftv_line_warp<PY, -1>(v, m, scr + (lane % LPWY) * LY::SY, twAy, tw2y);
                 if (act) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) spec[(size_t)(r0 + p * NY + j * TY + m) * nxhp + k] = v[j];
+                    for (int j = 0; j < 4; ++j) spec[(size_t)(rank * PPC + p) * spP + (size_t)(j * TY + m) * spQ + k] = v[j];
                 }
             }
             cluster.sync();
+            if (pending) {
+                // calcnorm of the previous step (reading S13): the CTAs' partial sums in rank order, the
+                // same in every CTA
+                if (tid == 0) {
+                    double tot = 0.0;
+                    for (int r = 0; r < CS; ++r) tot += *cluster.map_shared_rank(&cpart, r);
+                    const double sf = 1.0 / sqrt(tot * a.dV);
+                    sc[SC_S] = sf; sc[SC_S2] = sf * sf;
+                }
+                __syncthreads();
+                pending = false;
+            }
             // ---------------- B: FFT-z, x V_dd(k)/P, inverse FFT-z, all in registers ----------------
             for (int base = 0; base < (ncs + LPWZ - 1) / LPWZ * 32; base += P2T) {
                 const int col = ((base + tid) >> 5) * LPWZ + lane % LPWZ, m = lane / LPWZ;
                 const bool act = col < ncs;
                 const int q = qs_lo + (act ? col : 0), y = q / NXH1, k = q % NXH1;
-                cd* gc = spec + (size_t)y * nxhp + k;
+                cd* gc = spec + (size_t)y * spQ + k;
                 // folded table (dbec_internal.hpp): index m and N - m share an entry
-                const double* vd = a.vdd + (size_t)(y < NY - y ? y : NY - y) * nxhp + k;
+                const double* vd = a.vdd + (size_t)(y < NY - y ? y : NY - y) * vQ + k;
+                const double s2 = sc[SC_S2];
                 cd v[4];
                 double w[4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int z = j * TZ + m;
-                    v[j] = act ? p2_ldcg(gc + z * ls_spec) : zero;
-                    w[j] = act ? __ldg(vd + (size_t)(z < NZ - z ? z : NZ - z) * vls) : 0.0;
+                    v[j] = act ? p2_ldcg(gc + z * spP) : zero;
+                    w[j] = act ? s2 * __ldg(vd + (size_t)(z < NZ - z ? z : NZ - z) * vL) : 0.0;
                 }
                 __syncwarp();
                 fftv_line_warp<PZ, -1>(v, m, scr + (lane % LPWZ) * LY::SZ, twAz, tw2z);
@@ -244,17 +280,17 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                 fftv_line_warp<PZ, +1>(v, m, scr + (lane % LPWZ) * LY::SZ, twAz, tw2z);
                 if (act) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) gc[(j * TZ + m) * ls_spec] = v[j];
+                    for (int j = 0; j < 4; ++j) gc[(j * TZ + m) * spP] = v[j];
                 }
             }
             // psi of this CTA's rows for the first round of pass C: pass B does not touch psi, so the loads fly
             // while the cluster barrier and the inverse y transforms run
             cd q0[4], q1[4];
             {
-                const int line = tid / TX, m = tid % TX;
-                const cd* g0 = psi + (size_t)(r0 + 2 * (line < NP ? line : 0)) * NX;
+                const int line = tid / TX, m = tid % TX, r = line < NP ? 2 * line : 0;
+                const cd* g0 = psi + (size_t)(rank * PPC + r / NY) * psP + (size_t)(r % NY) * psQ;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) { q0[j] = p2_ldcg(g0 + j * TX + m); q1[j] = p2_ldcg(g0 + NX + j * TX + m); }
+                for (int j = 0; j < 4; ++j) { q0[j] = p2_ldcg(g0 + j * TX + m); q1[j] = p2_ldcg(g0 + psQ + j * TX + m); }
             }
             cluster.sync();
             // ---------------- C: inverse FFT-y -> merge -> inverse FFT-x -> calcnu -> calclux -> calcluy ----------------
@@ -264,7 +300,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                 const int p = act ? line / NXH1 : 0, k = act ? line % NXH1 : 0;
                 cd v[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) v[j] = act ? p2_ldcg(spec + (size_t)(r0 + p * NY + j * TY + m) * nxhp + k) : zero;
+                for (int j = 0; j < 4; ++j) v[j] = act ? p2_ldcg(spec + (size_t)(rank * PPC + p) * spP + (size_t)(j * TY + m) * spQ + k) : zero;
                 __syncwarp();
                 fftv_line_warp<PY, +1>(v, m, scr + (lane % LPWY) * LY::SY, twAy, tw2y);
                 if (act) {
@@ -281,12 +317,12 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     const int l = act ? line : 0;
                     const cd* ra = XB + (2 * l) * NXH1;
                     const cd* rb = ra + NXH1;
-                    const cd* g0 = psi + (size_t)(r0 + 2 * l) * NX;
+                    const cd* g0 = psi + (size_t)(rank * PPC + (2 * l) / NY) * psP + (size_t)((2 * l) % NY) * psQ;
                     cd v[4];
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int kk = j * TX + m;
-                        if (base > 0) { q0[j] = p2_ldcg(g0 + kk); q1[j] = p2_ldcg(g0 + NX + kk); }
+                        if (base > 0) { q0[j] = p2_ldcg(g0 + kk); q1[j] = p2_ldcg(g0 + psQ + kk); }
                         // X_a + i X_b on 0 .. N/2, the conjugates above
                         if (kk <= NX / 2) { const cd p = ra[kk], q = rb[kk]; v[j] = cmake(p.x - q.y, p.y + q.x); }
                         else { const cd p = ra[NX - kk], q = rb[NX - kk]; v[j] = cmake(p.x + q.y, q.x - p.y); }
@@ -301,7 +337,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                             for (int j = 0; j < 4; ++j) {
                                 const int x = j * TX + m;
                                 const cd q = hr ? q1[j] : q0[j];
-                                const double u = dt * (vxs[x] + vys[y] + vzs[zz] + G * (s2 * cnorm2(q)) + D * (hr ? v[j].y : v[j].x));
+                                const double u = dt * (vxs[x] + vq[y] + vp[zz] + G * (s2 * cnorm2(q)) + D * (hr ? v[j].y : v[j].x));
                                 cd w;
                                 if (RT) { double sn, cs; sincos_cw(u, &sn, &cs); w = cmul(s, cmul(q, cmake(cs, -sn))); }
                                 else w = cmul(s * exp_cw(-u), q);
@@ -336,7 +372,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     cd u[P2L];
 #pragma unroll
                     for (int i = 0; i < P2L; ++i) u[i] = g[i * PP];
-                    p2_cn<RT, NCHY>(u, c, lane % LPW, LPW, tcy, tcy + EY, tcy + 2 * EY, tcy + 3 * EY, tcy + 3 * EY + NCHY, cny_g.kap);
+                    p2_cn<RT, NCHY>(u, c, lane % LPW, LPW, tq, tq + EY, tq + 2 * EY, tq + 3 * EY, tq + 3 * EY + NCHY, kq);
                     if (act) {
 #pragma unroll
                         for (int i = 0; i < P2L; ++i) g[i * PP] = u[i];
@@ -345,8 +381,10 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
             }
             __syncthreads();
             {
-                cd* g = psi + (size_t)r0 * NX;
-                for (int idx = tid; idx < R * NX; idx += P2T) g[idx] = Pb[(idx / NX) * PP + p2_skew(idx % NX)];
+                for (int idx = tid; idx < R * NX; idx += P2T) {
+                    const int r = idx / NX, x = idx % NX;
+                    psi[(size_t)(rank * PPC + r / NY) * psP + (size_t)(r % NY) * psQ + x] = Pb[r * PP + p2_skew(x)];
+                }
             }
             cluster.sync();
             // ---------------- D: calcluz from / to global memory (+ calcnorm) ----------------
@@ -356,31 +394,33 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                 for (int base = 0; base < (ncp + LPW - 1) / LPW * 32; base += P2T) {
                     const int col = ((base + tid) >> 5) * LPW + lane % LPW, c = lane / LPW;
                     const bool act = col < ncp;
-                    cd* g = psi + (size_t)(c * P2L) * ls_psi + qp_lo + (act ? col : 0);
+                    const int qq = qp_lo + (act ? col : 0);
+                    cd* g = psi + (size_t)(c * P2L) * psP + (size_t)(qq / NX) * psQ + qq % NX;
                     cd u[P2L];
 #pragma unroll
-                    for (int i = 0; i < P2L; ++i) u[i] = act ? p2_ldcg(g + i * ls_psi) : zero;
-                    p2_cn<RT, NCHZ>(u, c, lane % LPW, LPW, tcz, tcz + EZ, tcz + 2 * EZ, tcz + 3 * EZ, tcz + 3 * EZ + NCHZ, cnz_g.kap);
+                    for (int i = 0; i < P2L; ++i) u[i] = act ? p2_ldcg(g + i * psP) : zero;
+                    p2_cn<RT, NCHZ>(u, c, lane % LPW, LPW, tl, tl + EZ, tl + 2 * EZ, tl + 3 * EZ, tl + 3 * EZ + NCHZ, kl);
                     if (act) {
 #pragma unroll
-                        for (int i = 0; i < P2L; ++i) { g[i * ls_psi] = u[i]; acc += cnorm2(u[i]); }
+                        for (int i = 0; i < P2L; ++i) { g[i * psP] = u[i]; acc += cnorm2(u[i]); }
                     }
                 }
             }
             if (a.imag) {
                 const double part = p2_block_sum_all(acc, red);
                 if (tid == 0) cpart = part;
+                pending = true;             // read after the next cluster barrier
             }
+            // a cube's next step starts on what this CTA has just written (header comment): block barrier only
+            if (SWAP) __syncthreads(); else cluster.sync();
+        }
+        if (pending) {
             cluster.sync();
-            if (a.imag) {
-                // calcnorm (reading S13): the CTAs' partial sums in rank order, the same in every CTA
-                if (tid == 0) {
-                    double tot = 0.0;
-                    for (int r = 0; r < CS; ++r) tot += *cluster.map_shared_rank(&cpart, r);
-                    const double sf = 1.0 / sqrt(tot * a.dV);
-                    sc[SC_S] = sf; sc[SC_S2] = sf * sf;
-                }
-                __syncthreads();
+            if (tid == 0) {
+                double tot = 0.0;
+                for (int r = 0; r < CS; ++r) tot += *cluster.map_shared_rank(&cpart, r);
+                const double sf = 1.0 / sqrt(tot * a.dV);
+                sc[SC_S] = sf; sc[SC_S2] = sf * sf;
             }
         }
         // the member's scalars back to global memory (norm factor, ramp state)
