@@ -383,12 +383,13 @@ def run_ours(args, w):
     # ---- end to end through the C ABI with host buffers ----
     # Every step's input comes from pinned host memory and its result goes back there, inside the timed region.
     # A single handle does this one copy after the other (`serial`).  The headline figure feeds the GPU the way a
-    # serving loop would: two handles on two streams, dbec_set_psi_async / dbec_get_psi_async, so that the upload of
-    # one step's input runs while the other handle's result goes down (both directions of the host link busy) and
+    # serving loop would: three handles on three streams, dbec_set_psi_async / dbec_get_psi_async, so that the upload of
+    # one step's input runs while another handle's result goes down (both directions of the host link busy) and
     # the steps hide behind the copies.  Every step is still one full upload, one dbec_step(1), one full download.
-    e2e_steps = max(4, min(args.steps, 20)) // 2 * 2
+    e2e_steps = max(6, min(args.steps, 24)) // 3 * 3
     host_in = torch.from_numpy(psi0.copy()).pin_memory()
-    host_out = [torch.empty_like(host_in).pin_memory() for _ in range(2)]
+    NRING = 3                              # handles taking turns in the pipelined leg
+    host_out = [torch.empty_like(host_in).pin_memory() for _ in range(NRING)]
     for _ in range(2):
         sim.set_psi(host_in.numpy())
         sim.step(1)
@@ -403,32 +404,34 @@ def run_ours(args, w):
     e2e_serial_s = time.perf_counter() - t0
     e2e_serial = whole_job_value(w.npoints, e2e_steps, world, max_over_ranks(e2e_serial_s, world, dev))
     ref_out = host_out[0].clone()
-    sim2 = dbec.Dbec(dbec.params_of(w), device=dev)
-    if (w.G_run, w.D_run) != (w.G, w.D):
-        sim2.set_coupling(w.G_run, w.D_run)
-    pair = (sim, sim2)
+    extra = [dbec.Dbec(dbec.params_of(w), device=dev) for _ in range(NRING - 1)]
+    for s_ in extra:
+        if (w.G_run, w.D_run) != (w.G, w.D):
+            s_.set_coupling(w.G_run, w.D_run)
+    ring = [sim] + extra
 
     def pipelined(nsteps):
         for i in range(nsteps):
-            s_ = pair[i & 1]
-            if i >= 2:
+            s_ = ring[i % NRING]
+            if i >= NRING:
                 s_.wait()                  # this handle's previous result has landed in its host buffer
             s_.set_psi_async(host_in)
             s_.step(1)
-            s_.get_psi_async(host_out[i & 1])
-        for s_ in pair:
+            s_.get_psi_async(host_out[i % NRING])
+        for s_ in ring:
             s_.wait()
 
-    pipelined(4)
-    assert torch.equal(host_out[0], ref_out) and torch.equal(host_out[1], ref_out), "pipelined e2e leg differs from the serial one"
+    pipelined(2 * NRING)
+    assert all(torch.equal(h_, ref_out) for h_ in host_out), "pipelined e2e leg differs from the serial one"
     barrier()
     t0 = time.perf_counter()
     pipelined(e2e_steps)
     barrier()
     e2e_s = time.perf_counter() - t0
     e2e_value = whole_job_value(w.npoints, e2e_steps, world, max_over_ranks(e2e_s, world, dev))
-    sim2.close()
-    del sim2
+    for s_ in extra:
+        s_.close()
+    del extra, ring
 
     # ---- per-kernel roofline (rank 0) ----
     line = None
@@ -515,8 +518,8 @@ def run_ours(args, w):
                 "clocks": sampler.summary(clock_note),
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.npoints,
                         "d2h_bytes_per_step": 16 * w.npoints, "steps": e2e_steps,
-                        "how": "two handles on two streams, dbec_set_psi_async / dbec_step(1) / dbec_get_psi_async per step "
-                               "from / to pinned host buffers: uploads overlap the other handle's downloads",
+                        "how": "three handles on three streams taking turns, dbec_set_psi_async / dbec_step(1) / dbec_get_psi_async "
+                               "per step from / to pinned host buffers: uploads overlap the other handles' downloads",
                         "serial": {"value": e2e_serial, "unit": UNIT,
                                    "how": "one handle: dbec_set_psi, dbec_step(1), dbec_get_psi one after the other"}},
                 "gpu_launches": launches,

@@ -90,8 +90,8 @@ int dbec_get_psi(dbec_handle h, void* psi_c128, int on_device);
 
 /* The same two copies for PINNED host buffers (cudaHostAlloc / cudaHostRegister), without the host synchronisation:
  * the copy is enqueued on the handle's stream and the call returns at once, so the transfers of one handle overlap
- * the steps and the opposite-direction transfers of another (two handles on two streams keep both directions of
- * the host link busy — how bench.py's end-to-end leg feeds the GPU).  The buffer must stay valid and untouched
+ * the steps and the opposite-direction transfers of another (a few handles on streams of their own taking turns
+ * keep both directions of the host link busy — how bench.py's end-to-end leg feeds the GPU).  The buffer must stay valid and untouched
  * until the stream has passed the copy: dbec_synchronize, or the caller's own event on that stream.  With pageable
  * memory CUDA stages the copy and the call may block; the result is the same.  Only the state handed over
  * changes hands ("only wave function array is returned"); nothing else crosses the link. */
