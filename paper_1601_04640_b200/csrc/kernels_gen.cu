@@ -17,13 +17,18 @@
 #include "norm_finish.cuh"
 #include "trig.cuh"
 
+// Blocks of the FFT kernels: 256 threads, four per SM (64 registers).  Measured against 512 x 2 with the tile sizes
+// below: 384^3 4.91 -> 4.57 ms per step, 320^3 2.60 -> 2.45, 192^3 0.579 -> 0.547 (more, smaller blocks overlap each
+// other's load, transform and store phases; 256 x 3 with 80 registers spills less and is slower: 5.10 ms).
+#define GEN_T 256
+#define GEN_B 4
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return (int)e_; } while (0)
 
 // ------------------------------------------------------------------------------------------------
 // a1, x axis: n = |s psi|^2 -> half spectrum, two real lines per complex transform
 // ------------------------------------------------------------------------------------------------
 // Block = LP line pairs; shared memory: two buffers of LP lines of n complex values.
-__global__ void __launch_bounds__(512, 2)
+__global__ void __launch_bounds__(GEN_T, GEN_B)
 k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* __restrict__ twN, double* __restrict__ scal,
                    const __grid_constant__ GenPlanP pl, int LP, int npairs, int nxhp, int pairs_per_member, int nb, int advance) {
     extern __shared__ cd gsm[];
@@ -67,10 +72,11 @@ k_gen_density_fftx(const cd* __restrict__ psi, cd* __restrict__ spec, const cd* 
 // ------------------------------------------------------------------------------------------------
 // a1 / a3 along y or z on the half spectrum; MODE 2 = forward * V_dd(k)/P * inverse (a2 fused)
 // ------------------------------------------------------------------------------------------------
-// A tile is `cols` neighbouring columns (8: one 128-byte row per line point; 4 for lines longer than 512 points,
-// so that two buffers of n x cols values fit), element (j, col) at j*cols + col in shared memory.
+// A tile is `cols` neighbouring columns (8: one 128-byte row per line point; 4 for lines longer than 256 points,
+// so that four blocks with two buffers of n x cols values each fit an SM), element (j, col) at j*cols + col in
+// shared memory.
 template <int MODE>
-__global__ void __launch_bounds__(512, 2)
+__global__ void __launch_bounds__(GEN_T, GEN_B)
 k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const cd* __restrict__ twN, const __grid_constant__ GenPlanP pl, int cols,
                   long long line_stride, long long outer_stride, int ntiles_x, long long ntiles, int nxhp, int ny3,
                   long long vdd_line_stride) {
@@ -107,7 +113,7 @@ k_gen_fft_strided(cd* __restrict__ spec, const double* __restrict__ vdd, const c
 // a3 (x axis, complex-to-real, two lines per transform) + a4 calcnu, or Phi_dd written out
 // ------------------------------------------------------------------------------------------------
 template <bool RT, bool PHI>
-__global__ void __launch_bounds__(512, 2)
+__global__ void __launch_bounds__(GEN_T, GEN_B)
 k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __restrict__ phi_out, const cd* __restrict__ twN,
                    const double* __restrict__ scal, const double* __restrict__ vx, const double* __restrict__ vy,
                    const double* __restrict__ vz, double dt, const __grid_constant__ GenPlanP pl, int LP, int npairs, int nxhp, int ny, int nz) {
@@ -161,8 +167,9 @@ k_gen_ifftx_nonlin(const cd* __restrict__ spec, cd* __restrict__ psi, double* __
 // L: points per chunk — 8 (tables pf8 / pb8: 32 registers of psi per thread, up to 1024 threads per tile) for every
 // axis; 16 stays available for comparison.
 constexpr int GC = 8;
-template <bool RT, bool NORM, int L>
-__global__ void __launch_bounds__(L == 8 ? 1024 : 512)
+// REGS: register cap (L = 8: 64, or 56 where that lets one more block of the tile's size onto the SM)
+template <bool RT, bool NORM, int L, int REGS>
+__global__ void __launch_bounds__(L == 8 ? 1024 : 512) __maxnreg__(REGS)
 k_gen_cn(cd* __restrict__ psi, CnTab<RT> cn, int n, int nch, long long elem_stride, long long col_stride, long long outer_stride,
          long long ncols, double* __restrict__ partial, unsigned int* ticket, double* __restrict__ scal, double dV, int nb, int K) {
     typedef typename CnCoef<RT>::type CT;
@@ -262,15 +269,15 @@ template <class K> static int gen_smem(K kernel, size_t bytes) {
     return 0;
 }
 
-// line pairs per block of the x kernels: two buffers of LP lines within 64 KiB
-static int gen_lp(int n) { int lp = 2048 / n; return lp < 1 ? 1 : (lp > 8 ? 8 : lp); }
+// line pairs per block of the x kernels: two buffers of LP lines within 48 KiB (four blocks per SM)
+static int gen_lp(int n) { int lp = 1536 / n; return lp < 1 ? 1 : (lp > 8 ? 8 : lp); }
 
 int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance) {
     const GenPlanP pl = plan_of(h, 0);
     const int LP = gen_lp(pl.n), ppm = h->ny * h->nz / 2, npairs = ppm * h->nb;
     const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
     CK((cudaError_t)gen_smem(k_gen_density_fftx, sm));
-    CK(launch_pdl(k_gen_density_fftx, dim3((npairs + LP - 1) / LP), dim3(512), sm, h->stream, h->use_pdl, (const cd*)h->psi, h->spec,
+    CK(launch_pdl(k_gen_density_fftx, dim3((npairs + LP - 1) / LP), dim3(GEN_T), sm, h->stream, h->use_pdl, (const cd*)h->psi, h->spec,
                   h->ax[0].twN, h->scal, pl, LP, npairs, h->nxhp, ppm, h->nb, advance));
     h->launches++;
     return (int)cudaGetLastError();
@@ -278,7 +285,7 @@ int dbec_launch_gen_density_fftx(dbec_handle_s* h, int advance) {
 
 template <int MODE> static int launch_gen_fft(dbec_handle_s* h, int axis) {
     const GenPlanP pl = plan_of(h, axis);
-    const int cols = pl.n <= 512 ? 8 : 4;
+    const int cols = pl.n <= 256 ? 8 : 4;          // two buffers of n x cols values within 48 KiB up to n = 384
     long long line_stride, outer_stride, ntiles;
     int ntx;
     if (axis == 1) { line_stride = h->nxhp; outer_stride = (long long)h->ny * h->nxhp; ntx = h->nxhp / cols; ntiles = (long long)ntx * h->nplanes; }
@@ -288,7 +295,7 @@ template <int MODE> static int launch_gen_fft(dbec_handle_s* h, int axis) {
     const size_t sm = 2 * (size_t)pl.n * cols * sizeof(cd);
     auto k = k_gen_fft_strided<MODE>;
     CK((cudaError_t)gen_smem(k, sm));
-    CK(launch_pdl(k, dim3((unsigned)ntiles), dim3(512), sm, h->stream, h->use_pdl, h->spec, (const double*)h->vdd, h->ax[axis].twN, pl,
+    CK(launch_pdl(k, dim3((unsigned)ntiles), dim3(GEN_T), sm, h->stream, h->use_pdl, h->spec, (const double*)h->vdd, h->ax[axis].twN, pl,
                   cols, line_stride, outer_stride, ntx, ntiles, h->nxhp, ny3, vls));
     h->launches++;
     return (int)cudaGetLastError();
@@ -304,7 +311,7 @@ template <bool RT, bool PHI> static int launch_gen_nonlin(dbec_handle_s* h, doub
     const size_t sm = 2 * (size_t)LP * pl.n * sizeof(cd);
     auto k = k_gen_ifftx_nonlin<RT, PHI>;
     CK((cudaError_t)gen_smem(k, sm));
-    CK(launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(512), sm, h->stream, h->use_pdl, (const cd*)h->spec, h->psi, phi, h->ax[0].twN,
+    CK(launch_pdl(k, dim3((npairs + LP - 1) / LP), dim3(GEN_T), sm, h->stream, h->use_pdl, (const cd*)h->spec, h->psi, phi, h->ax[0].twN,
                   (const double*)h->scal, h->ax[0].vtrap, h->ax[1].vtrap, h->ax[2].vtrap, h->p.dt, pl, LP, npairs, h->nxhp, h->ny, h->nz));
     h->launches++;
     return (int)cudaGetLastError();
@@ -327,7 +334,7 @@ template <> CnTab<false> cntab8<false>(const AxisTables& a) {
 
 // Chunks of 8 points along y and z (measured at 384^3 and 320^3: 5 - 20 % faster than 16), of 16 along x, where a
 // thread's chunk is contiguous in memory and 8-point chunks leave half of every 256 bytes to another warp.
-template <bool RT, bool NORM, int L> static int launch_gen_cn_l(dbec_handle_s* h, int axis) {
+template <bool RT, bool NORM, int L, int REGS> static int launch_gen_cn_l(dbec_handle_s* h, int axis) {
     const int n = h->ax[axis].n, nch = (n + L - 1) / L;
     const int threads = (nch * GC + 31) / 32 * 32;
     long long es, cs, os, ncols;
@@ -338,7 +345,7 @@ template <bool RT, bool NORM, int L> static int launch_gen_cn_l(dbec_handle_s* h
     dim3 grid((unsigned)((ncols + GC - 1) / GC), (unsigned)nouter);
     if (NORM && (long long)grid.x * grid.y > h->npartial) return (int)cudaErrorInvalidValue;
     const size_t sm = 2 * (size_t)(threads / GC) * GC * sizeof(cd);
-    CK(launch_pdl(k_gen_cn<RT, NORM, L>, grid, dim3(threads), sm, h->stream, h->use_pdl, h->psi,
+    CK(launch_pdl(k_gen_cn<RT, NORM, L, REGS>, grid, dim3(threads), sm, h->stream, h->use_pdl, h->psi,
                   L == 8 ? cntab8<RT>(h->ax[axis]) : make_cntab<RT>(h->ax[axis]), n, nch, es, cs, os,
                   ncols, h->partial, h->ticket, h->scal, h->dV, h->nb, L == 8 ? h->ax[axis].K8 : h->ax[axis].K16));
     h->launches++;
@@ -346,7 +353,13 @@ template <bool RT, bool NORM, int L> static int launch_gen_cn_l(dbec_handle_s* h
 }
 
 template <bool RT, bool NORM> static int launch_gen_cn(dbec_handle_s* h, int axis) {
-    return axis == 0 ? launch_gen_cn_l<RT, NORM, 16>(h, axis) : launch_gen_cn_l<RT, NORM, 8>(h, axis);
+    if (axis == 0) return launch_gen_cn_l<RT, NORM, 16, 128>(h, axis);
+    // 8-point chunks: 64 registers hold a chunk without spilling much; 56 cost a few more spills and pay when they
+    // let one more block onto the SM (measured at 384^3: 384 threads per block, 2 -> 3 blocks, sweeps 515 -> 447 us;
+    // at 320^3, 3 blocks either way, 258 -> 284 us)
+    const int threads = ((h->ax[axis].n + 7) / 8 * GC + 31) / 32 * 32;
+    const bool r56 = 65536 / (threads * 56) > 65536 / (threads * 64);
+    return r56 ? launch_gen_cn_l<RT, NORM, 8, 56>(h, axis) : launch_gen_cn_l<RT, NORM, 8, 64>(h, axis);
 }
 
 int dbec_launch_gen_cn(dbec_handle_s* h, int axis, int with_norm) {
