@@ -73,6 +73,9 @@ def test_null_handles_are_rejected(gp):
     assert L.dbec_set_psi(None, None, 0) == gp.DBEC_EINVAL
     assert L.dbec_observables(None, None) == gp.DBEC_EINVAL
     assert L.dbec_destroy(None) == gp.DBEC_EINVAL
+    assert L.dbec_set_psi_async(None, None) == gp.DBEC_EINVAL
+    assert L.dbec_get_psi_async(None, None) == gp.DBEC_EINVAL
+    assert L.dbec_synchronize(None) == gp.DBEC_EINVAL
     assert L.dbec_last_cuda_error(None) == 0
 
 
