@@ -374,16 +374,11 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     for (int i = 0; i < P2L; ++i) u[i] = g[i * PP];
                     p2_cn<RT, NCHY>(u, c, lane % LPW, LPW, tq, tq + EY, tq + 2 * EY, tq + 3 * EY, tq + 3 * EY + NCHY, kq);
                     if (act) {
+                        // straight to global memory: the LPW neighbouring columns of a chunk are one contiguous piece
+                        cd* go = psi + (size_t)(rank * PPC + p) * psP + (size_t)(c * P2L) * psQ + x;
 #pragma unroll
-                        for (int i = 0; i < P2L; ++i) g[i * PP] = u[i];
+                        for (int i = 0; i < P2L; ++i) go[(size_t)i * psQ] = u[i];
                     }
-                }
-            }
-            __syncthreads();
-            {
-                for (int idx = tid; idx < R * NX; idx += P2T) {
-                    const int r = idx / NX, x = idx % NX;
-                    psi[(size_t)(rank * PPC + r / NY) * psP + (size_t)(r % NY) * psQ + x] = Pb[r * PP + p2_skew(x)];
                 }
             }
             cluster.sync();
