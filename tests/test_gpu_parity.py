@@ -209,7 +209,7 @@ def one_step_pair(gp, ob, w, psi0, steps=1):
 
 
 # shapes kernels_small_p2.cu is compiled for (the one-launch step with compile-time power-of-two lengths)
-P2_SHAPES = [(16, 16, 16), (32, 32, 32), (32, 32, 64), (64, 64, 16)]
+P2_SHAPES = [(a, b, c) for a in (16, 32, 64) for b in (16, 32, 64) for c in (16, 32, 64) if a * b * c <= 65536]
 
 
 def small_step_cases():
