@@ -8,7 +8,7 @@
 //   * the split / merge of the two-real-lines transform happens while loading the next transform;
 //   * Crank-Nicolson sweeps on chunks of 8 points, N/8 lanes per line, neighbours and carries by warp shuffles;
 //   * global loads and stores go straight from / to the registers of the lane that needs them.
-// Six block barriers and four cluster barriers per step.  Results agree with k_small_step to round-off (another
+// Five block barriers (two more for the norm in imaginary time) and four cluster barriers per step.  Results agree with k_small_step to round-off (another
 // summation order in the transforms); tests/test_gpu_parity.py runs both against the oracle.
 //
 // Cubes (NY == NZ) need only THREE cluster barriers per step: the roles of y and z alternate from step to step.
