@@ -108,11 +108,22 @@ __device__ __forceinline__ double p2_block_sum_all(double x, double* red) {
 }
 
 // Shared-memory layout (elements of cd unless noted), the same on host and device.
+// Planes of a CTA's slab that passes A and C hold in shared memory at a time: all NZ / CS of them if they fit, else
+// the largest power-of-two part that does (a small cluster then walks its slab in several rounds).
+__host__ __device__ constexpr int p2_pps(int nx, int ny, int nz, int cs) {
+    int pps = nz / cs;
+    while (pps > 1 && (pps % 2 == 0) &&
+           (size_t)(pps * ny) * ((nx + nx / 8 + 3) / 8 * 8 + 4 + nx / 2 + nx / 2 + 1) * sizeof(cd) > 170 * 1024) pps /= 2;
+    return pps;
+}
+
 template <bool RT, int NX, int NY, int NZ, int CS> struct P2Lay {
     static_assert(NZ % CS == 0 && (NZ / CS * NY) % 2 == 0, "whole planes and whole pairs of rows per CTA");
     typedef typename P2Plan<NX>::P PX; typedef typename P2Plan<NY>::P PY; typedef typename P2Plan<NZ>::P PZ;
     static constexpr int PPC = NZ / CS;                 // planes per CTA
-    static constexpr int R = PPC * NY, NP = R / 2;        // rows / pairs of rows a CTA holds
+    static constexpr int PPS = p2_pps(NX, NY, NZ, CS);  // ... of which passes A and C work on at a time
+    static_assert(PPC % PPS == 0 && (PPS * NY) % 2 == 0, "whole rounds, whole pairs of rows");
+    static constexpr int R = PPS * NY, NP = R / 2;        // rows / pairs of rows of one round
     static constexpr int NXH1 = NX / 2 + 1;               // half-spectrum length
     // a psi row in shared memory: point x at x + x/8 (p2_skew: the chunks of a row start in different bank groups),
     // row pitch = 4 mod 8 (two neighbouring rows complement each other)
@@ -140,7 +151,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
     typedef P2Lay<RT, NX, NY, NZ, CS> LY;
     typedef typename LY::PX PX; typedef typename LY::PY PY; typedef typename LY::PZ PZ;
     typedef typename CnCoef<RT>::type CT;
-    constexpr int R = LY::R, NP = LY::NP, NXH1 = LY::NXH1, PP = LY::PP, PPC = LY::PPC;
+    constexpr int R = LY::R, NP = LY::NP, NXH1 = LY::NXH1, PP = LY::PP, PPC = LY::PPC, PPS = LY::PPS, NSUB = PPC / PPS;
     constexpr int TX = PX::T, TY = PY::T, TZ = PZ::T, LPWY = 32 / TY, LPWZ = 32 / TZ;
     constexpr int NCHX = NX / P2L, NCHY = NY / P2L, NCHZ = NZ / P2L;
     extern __shared__ __align__(16) cd psm[];
@@ -198,13 +209,14 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
             const CT kq = sw ? cnz_g.kap : cny_g.kap, kl = sw ? cny_g.kap : cnz_g.kap;
             const double* vq = sw ? vzs : vys; const double* vp = sw ? vys : vzs;
             // ---------------- A: density -> FFT-x -> split -> FFT-y -> spectrum ----------------
-            {
+            for (int ss = 0; ss < NSUB; ++ss) {
+                const int pl0 = rank * PPC + ss * PPS;                  // first plane of this round
                 // (|psi|^2 without the norm factor: pass B multiplies by s^2)
                 for (int base = 0; base < NP * TX; base += P2T) {
                     const int item = base + tid, line = item / TX, m = item % TX;
                     const bool act = line < NP;
                     const int r = act ? 2 * line : 0;
-                    const cd* g = psi + (size_t)(rank * PPC + r / NY) * psP + (size_t)(r % NY) * psQ;
+                    const cd* g = psi + (size_t)(pl0 + r / NY) * psP + (size_t)(r % NY) * psQ;
                     cd v[4];
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
@@ -221,11 +233,10 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                         for (int j = 0; j < 4; ++j) ZB[line * NX + j * TX + m] = v[j];
                     }
                 }
-            }
             __syncthreads();
-            for (int base = 0; base < (PPC * NXH1 + LPWY - 1) / LPWY * 32; base += P2T) {
+            for (int base = 0; base < (PPS * NXH1 + LPWY - 1) / LPWY * 32; base += P2T) {
                 const int line = ((base + tid) >> 5) * LPWY + lane % LPWY, m = lane / LPWY;
-                const bool act = line < PPC * NXH1;
+                const bool act = line < PPS * NXH1;
                 const int p = act ? line / NXH1 : 0, k = act ? line % NXH1 : 0;
                 cd v[4];
 #pragma unroll
@@ -239,8 +250,10 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                 fftv_line_warp<PY, -1>(v, m, scr + (lane % LPWY) * LY::SY, twAy, tw2y);
                 if (act) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) spec[(size_t)(rank * PPC + p) * spP + (size_t)(j * TY + m) * spQ + k] = v[j];
+                    for (int j = 0; j < 4; ++j) spec[(size_t)(pl0 + p) * spP + (size_t)(j * TY + m) * spQ + k] = v[j];
                 }
+            }
+            if (NSUB > 1) __syncthreads();              // the next round overwrites ZB
             }
             cluster.sync();
             if (pending) {
@@ -286,7 +299,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
             // psi of this CTA's rows for the first round of pass C: pass B does not touch psi, so the loads fly
             // while the cluster barrier and the inverse y transforms run
             cd q0[4], q1[4];
-            {
+            if (NSUB == 1) {
                 const int line = tid / TX, m = tid % TX, r = line < NP ? 2 * line : 0;
                 const cd* g0 = psi + (size_t)(rank * PPC + r / NY) * psP + (size_t)(r % NY) * psQ;
 #pragma unroll
@@ -294,13 +307,15 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
             }
             cluster.sync();
             // ---------------- C: inverse FFT-y -> merge -> inverse FFT-x -> calcnu -> calclux -> calcluy ----------------
-            for (int base = 0; base < (PPC * NXH1 + LPWY - 1) / LPWY * 32; base += P2T) {
+            for (int ss = 0; ss < NSUB; ++ss) {
+            const int pl0 = rank * PPC + ss * PPS;                      // first plane of this round
+            for (int base = 0; base < (PPS * NXH1 + LPWY - 1) / LPWY * 32; base += P2T) {
                 const int line = ((base + tid) >> 5) * LPWY + lane % LPWY, m = lane / LPWY;
-                const bool act = line < PPC * NXH1;
+                const bool act = line < PPS * NXH1;
                 const int p = act ? line / NXH1 : 0, k = act ? line % NXH1 : 0;
                 cd v[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) v[j] = act ? p2_ldcg(spec + (size_t)(rank * PPC + p) * spP + (size_t)(j * TY + m) * spQ + k) : zero;
+                for (int j = 0; j < 4; ++j) v[j] = act ? p2_ldcg(spec + (size_t)(pl0 + p) * spP + (size_t)(j * TY + m) * spQ + k) : zero;
                 __syncwarp();
                 fftv_line_warp<PY, +1>(v, m, scr + (lane % LPWY) * LY::SY, twAy, tw2y);
                 if (act) {
@@ -317,12 +332,12 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     const int l = act ? line : 0;
                     const cd* ra = XB + (2 * l) * NXH1;
                     const cd* rb = ra + NXH1;
-                    const cd* g0 = psi + (size_t)(rank * PPC + (2 * l) / NY) * psP + (size_t)((2 * l) % NY) * psQ;
+                    const cd* g0 = psi + (size_t)(pl0 + (2 * l) / NY) * psP + (size_t)((2 * l) % NY) * psQ;
                     cd v[4];
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int kk = j * TX + m;
-                        if (base > 0) { q0[j] = p2_ldcg(g0 + kk); q1[j] = p2_ldcg(g0 + psQ + kk); }
+                        if (NSUB > 1 || base > 0) { q0[j] = p2_ldcg(g0 + kk); q1[j] = p2_ldcg(g0 + psQ + kk); }
                         // X_a + i X_b on 0 .. N/2, the conjugates above
                         if (kk <= NX / 2) { const cd p = ra[kk], q = rb[kk]; v[j] = cmake(p.x - q.y, p.y + q.x); }
                         else { const cd p = ra[NX - kk], q = rb[NX - kk]; v[j] = cmake(p.x + q.y, q.x - p.y); }
@@ -332,7 +347,7 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     if (act) {
 #pragma unroll
                         for (int hr = 0; hr < 2; ++hr) {
-                            const int row = 2 * l + hr, y = row % NY, zz = rank * PPC + row / NY;
+                            const int row = 2 * l + hr, y = row % NY, zz = pl0 + row / NY;
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
                                 const int x = j * TX + m;
@@ -364,9 +379,9 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
             __syncthreads();
             {
                 constexpr int LPW = 32 / NCHY;                                    // calcluy: lane = chunk LPW + column
-                for (int base = 0; base < (PPC * NX + LPW - 1) / LPW * 32; base += P2T) {
+                for (int base = 0; base < (PPS * NX + LPW - 1) / LPW * 32; base += P2T) {
                     const int col = ((base + tid) >> 5) * LPW + lane % LPW, c = lane / LPW;
-                    const bool act = col < PPC * NX;
+                    const bool act = col < PPS * NX;
                     const int p = act ? col / NX : 0, x = act ? col % NX : 0;
                     cd* g = Pb + (p * NY + c * P2L) * PP + p2_skew(x);
                     cd u[P2L];
@@ -375,11 +390,13 @@ k_small_p2(const __grid_constant__ P2Args a, CnTab<RT> cnx_g, CnTab<RT> cny_g, C
                     p2_cn<RT, NCHY>(u, c, lane % LPW, LPW, tq, tq + EY, tq + 2 * EY, tq + 3 * EY, tq + 3 * EY + NCHY, kq);
                     if (act) {
                         // straight to global memory: the LPW neighbouring columns of a chunk are one contiguous piece
-                        cd* go = psi + (size_t)(rank * PPC + p) * psP + (size_t)(c * P2L) * psQ + x;
+                        cd* go = psi + (size_t)(pl0 + p) * psP + (size_t)(c * P2L) * psQ + x;
 #pragma unroll
                         for (int i = 0; i < P2L; ++i) go[(size_t)i * psQ] = u[i];
                     }
                 }
+            }
+            if (NSUB > 1) __syncthreads();              // the next round overwrites XB and Pb
             }
             cluster.sync();
             // ---------------- D: calcluz from / to global memory (+ calcnorm) ----------------
@@ -481,8 +498,8 @@ template <bool RT, int NX, int NY, int NZ, int CS> static int p2_run(dbec_handle
                      X(32, 16, 32, 16) X(32, 16, 64, 16) X(32, 32, 16, 16) X(32, 32, 32, 16) X(32, 32, 64, 16) \
                      X(32, 64, 16, 16) X(32, 64, 32, 16) X(64, 16, 16, 16) X(64, 16, 32, 16) X(64, 16, 64, 16) \
                      X(64, 32, 16, 16) X(64, 32, 32, 16) X(64, 64, 16, 16) X(16, 16, 16, 4) X(16, 16, 16, 1) \
-                     X(32, 32, 32, 8)
-static const int p2_cluster_sizes[] = {16, 8, 4, 1};
+                     X(32, 32, 32, 8) X(32, 32, 32, 4) X(32, 32, 32, 2)
+static const int p2_cluster_sizes[] = {16, 8, 4, 2, 1};
 
 static int p2_dispatch(dbec_handle_s* h, int cs, int what, int nsteps) {
     const bool rt = h->p.time_mode == 1;
@@ -497,11 +514,12 @@ static int p2_dispatch(dbec_handle_s* h, int cs, int what, int nsteps) {
 // CTAs per cluster (and h->small_max_clusters set) when dbec_step of this handle can run in k_small_p2 — a 3-D grid
 // of one of the compiled shapes with the 8-point chunk tables built — else 0.  request > 0: that cluster size or
 // nothing.  Otherwise the choice is by the time one step of the whole batch takes: a cluster works through
-// ceil(nb / resident clusters) members one after the other, and a member's step on CS CTAs costs about
-// p2_step_cost(CS) relative to 16 CTAs (measured on B200: 32^3 16.9 us on 16 CTAs, 23.3 on 8; 16^3 11.3 us on 16,
-// 11.8 on 4, 20.7 on 1 — so 64 members of 32^3 go through 8-CTA clusters, 117 us per batch step against 169 on 16 CTAs
-// and 151 through the seven launches, and 256 members of 16^3 through single CTAs, 42 us against 149).
-static double p2_step_cost(int cs) { return cs >= 16 ? 1.0 : cs == 8 ? 1.4 : cs == 4 ? 1.05 : 1.85; }
+// ceil(nb / resident clusters) members one after the other, and a member's step costs about 9 us + 4.1 ns per grid
+// point of a CTA's share (measured on B200 — 16^3: 10.7 us on 16 CTAs, 11.5 on 4, 20.6 on 1; 32^3: 16.2 us on 16,
+// 23.1 on 8, 41.0 on 4, 76.0 on 2).  So one 32^3 grid takes 16 CTAs, 64 of them take clusters of 2 (76.8 us per
+// batch step against 161 on 16 CTAs, of which 8 are resident, and 151 through the seven launches), 256 grids of 16^3
+// single CTAs (41 us against 149).
+static double p2_step_cost(const dbec_handle_s* h, int cs) { return 9.0 + 0.0041 * (double)h->P / cs; }
 
 int dbec_small_p2_choose(dbec_handle_s* h, int request) {
     if (h->p.ndim != 3 || h->ax[0].K8 < 1 || h->ax[1].K8 < 1 || h->ax[2].K8 < 1) return 0;
@@ -511,7 +529,7 @@ int dbec_small_p2_choose(dbec_handle_s* h, int request) {
         if (request > 0 && cs != request) continue;
         const int n = p2_dispatch(h, cs, 0, 0);
         if (n < 1) continue;
-        const double t = (double)((h->nb + n - 1) / n) * p2_step_cost(cs);
+        const double t = (double)((h->nb + n - 1) / n) * p2_step_cost(h, cs);
         if (!best || t < best_t) { best = cs; best_n = n; best_t = t; }
     }
     if (best) h->small_max_clusters = best_n;

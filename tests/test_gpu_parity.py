@@ -490,7 +490,8 @@ def test_async_host_copies_on_two_handles_match_the_synchronous_calls(gp, mode):
         s.close()
 
 
-@pytest.mark.parametrize("n,cs,nb", [(32, 8, 1), (32, 8, 40), (32, 16, 21), (16, 4, 1), (16, 1, 1), (16, 1, 300), (16, 4, 75)])
+@pytest.mark.parametrize("n,cs,nb", [(32, 8, 1), (32, 8, 40), (32, 16, 21), (16, 4, 1), (16, 1, 1), (16, 1, 300), (16, 4, 75),
+                                     (32, 4, 1), (32, 2, 1), (32, 2, 90), (32, 4, 50)])
 @pytest.mark.parametrize("mode", [IMAG, REAL])
 def test_power_of_two_cluster_step_cluster_sizes_and_batches(gp, ob, n, cs, nb, mode, monkeypatch):
     """k_small_p2 with fewer CTAs per cluster (DBEC_SMALL_P2_CS) and with more batch members than resident clusters
