@@ -112,10 +112,10 @@ int dbec_set_coupling(dbec_handle h, double G, double D);
  * CUDA graph of a step sees it; dbec_observables / dbec_phi_dd do not advance it. */
 int dbec_set_ramp(dbec_handle h, int nstp, double G0, double D0, double G1, double D1);
 
-/* nsteps SSCN steps, asynchronous on the handle's stream, no host sync.  Grids of up to
- * 65536 points (per batch member) run all nsteps steps in ONE launch by one thread-block cluster per member
- * (PAPER.md:79 on launch overhead; environment DBEC_CLUSTER=0 at dbec_create switches that off);
- * larger grids replay a CUDA graph of the step's seven launches. */
+/* nsteps SSCN steps, asynchronous on the handle's stream, no host sync.  3-D grids of up
+ * to 65536 points per batch member (131072 when every length is 16, 32 or 64) run all nsteps steps in ONE launch by
+ * thread-block clusters, one member per cluster at a time (PAPER.md:79 on launch overhead; environment
+ * DBEC_CLUSTER=0 at dbec_create switches that off); larger grids replay a CUDA graph of the step's seven launches. */
 int dbec_step(dbec_handle h, int nsteps);
 
 /* calcmuen + calcrms on the current psi.  host_out: HOST pointer.  Synchronises

@@ -1,5 +1,5 @@
 // kernels_small_p2.cu — the one-launch cluster step (kernels_small.cu) for small 3-D grids whose three lengths are
-// powers of two known at compile time (16, 32 or 64 each, up to 64 Ki points: BASELINE.json's 32^3 config).  Same passes A - D, same data flow through L2,
+// powers of two known at compile time (16, 32 or 64 each, up to 128 Ki points: BASELINE.json's 32^3 config).  Same passes A - D, same data flow through L2,
 // same cluster barriers; what changes is how a line is worked on.  k_small_step serves any length, so its transforms
 // are Stockham passes through shared memory with a block barrier after each (about 40 per step, 900 cycles per
 // pass) and its code does not fit the instruction cache.  Here a line of N points belongs to N/4 lanes of ONE warp:
@@ -490,15 +490,16 @@ template <bool RT, int NX, int NY, int NZ, int CS> static int p2_run(dbec_handle
     return (int)cudaGetLastError();
 }
 
-// the shapes and cluster sizes this file is compiled for (NX, NY, NZ, CTAs per cluster): every grid of up to 64 Ki
-// points whose lengths are 16, 32 or 64, on 16 CTAs; the cubes also on smaller clusters, which give a member fewer
-// SMs and a batch more members in flight
+// the shapes and cluster sizes this file is compiled for (NX, NY, NZ, CTAs per cluster): every grid of up to 128 Ki
+// points whose lengths are 16, 32 or 64, on 16 CTAs (64^3 is left to the multi-launch path: 62 us per step there,
+// 97 here); the cubes also on smaller clusters, which give a member fewer SMs and a batch more members in flight
 #define P2_SHAPES(X) X(16, 16, 16, 16) X(16, 16, 32, 16) X(16, 16, 64, 16) X(16, 32, 16, 16) X(16, 32, 32, 16) \
                      X(16, 32, 64, 16) X(16, 64, 16, 16) X(16, 64, 32, 16) X(16, 64, 64, 16) X(32, 16, 16, 16) \
                      X(32, 16, 32, 16) X(32, 16, 64, 16) X(32, 32, 16, 16) X(32, 32, 32, 16) X(32, 32, 64, 16) \
                      X(32, 64, 16, 16) X(32, 64, 32, 16) X(64, 16, 16, 16) X(64, 16, 32, 16) X(64, 16, 64, 16) \
                      X(64, 32, 16, 16) X(64, 32, 32, 16) X(64, 64, 16, 16) X(16, 16, 16, 4) X(16, 16, 16, 1) \
-                     X(32, 32, 32, 8) X(32, 32, 32, 4) X(32, 32, 32, 2)
+                     X(32, 32, 32, 8) X(32, 32, 32, 4) X(32, 32, 32, 2) \
+                     X(64, 64, 32, 16) X(32, 64, 64, 16) X(64, 32, 64, 16)
 static const int p2_cluster_sizes[] = {16, 8, 4, 2, 1};
 
 static int p2_dispatch(dbec_handle_s* h, int cs, int what, int nsteps) {

@@ -209,7 +209,7 @@ def one_step_pair(gp, ob, w, psi0, steps=1):
 
 
 # shapes kernels_small_p2.cu is compiled for (the one-launch step with compile-time power-of-two lengths)
-P2_SHAPES = [(a, b, c) for a in (16, 32, 64) for b in (16, 32, 64) for c in (16, 32, 64) if a * b * c <= 65536]
+P2_SHAPES = [(a, b, c) for a in (16, 32, 64) for b in (16, 32, 64) for c in (16, 32, 64) if a * b * c <= 131072]
 
 
 def small_step_cases():
@@ -427,7 +427,8 @@ def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch, p2):
         o.close()
     # (k_small_p2 walks a batch through its resident clusters, k_small_step wants a cluster per member)
     for wl, nbatch, small in ((grid3(32, 32, 32, REAL), 1, True), (grid3(32, 32, 32, REAL), 200, p2 == "1"),
-                              (grid2(128, 128, REAL), 1, False), (grid3(64, 64, 32, IMAG), 1, False)):
+                              (grid2(128, 128, REAL), 1, False), (grid3(64, 64, 32, IMAG), 1, p2 == "1"),
+                              (grid3(64, 64, 64, IMAG), 1, False)):
         h = gp.Dbec(gp.params_of(wl), nbatch=nbatch)
         assert ("sscn_step<cluster>" in h.pass_kernels()) == small, (wid(wl), nbatch)
         h.close()
@@ -437,7 +438,8 @@ def test_cluster_step_batch_ramp_and_choice(gp, ob, monkeypatch, p2):
 @pytest.mark.parametrize("mode", [IMAG, REAL])
 def test_power_of_two_cluster_step_matches_oracle_and_general_kernel(gp, ob, shape, mode, monkeypatch):
     """k_small_p2 on every shape it is compiled for: five steps in one launch against the oracle (imaginary time:
-    the norm factor is carried from step to step inside the launch) and against k_small_step on the same input."""
+    the norm factor is carried from step to step inside the launch) and against k_small_step (beyond 64 Ki points:
+    the multi-launch path) on the same input."""
     monkeypatch.delenv("DBEC_CLUSTER", raising=False)
     monkeypatch.delenv("DBEC_SMALL_P2", raising=False)
     w = grid3(*shape, mode, d=(0.4, 0.35, 0.5))
@@ -452,7 +454,10 @@ def test_power_of_two_cluster_step_matches_oracle_and_general_kernel(gp, ob, sha
     o.close()
     monkeypatch.setenv("DBEC_SMALL_P2", "0")
     gen = gp.Dbec(gp.params_of(w))
-    assert gen.pass_kernels() == {"sscn_step<cluster>": "k_small_step"}
+    if w.npoints <= 65536:
+        assert gen.pass_kernels() == {"sscn_step<cluster>": "k_small_step"}
+    else:                                      # beyond k_small_step's 64 Ki points: the multi-launch path
+        assert "sscn_step<cluster>" not in gen.pass_kernels()
     gen.set_psi(psi0)
     gen.step(5)
     assert relerr(got, gen.get_psi()) < 5 * PSI_TOL
